@@ -1,0 +1,149 @@
+/*
+ * poisson.h -- C ABI of the B200-native (sm_100a) Fourier-space Poisson solve of arxiv 1211.5244
+ * (Dugan, Genovese, Goedecker, "A Customized 3D GPU Poisson Solver for Free Boundary Conditions").
+ *
+ * The library computes, for a real density rho on an nx*ny*nz grid,
+ *
+ *      V = IDFT3( K^F . DFT3( pad(rho) ) ) restricted to the physical box          (Eq. 3)
+ *
+ * on a grid zero-padded to S_i = 2 N_i along every free axis and S_i = N_i along every periodic
+ * axis, which equals the discrete convolution of Eq. 2
+ *
+ *      V[i] = sum_{i' in box} K[(i - i') mod S] rho[i'],   i in box.
+ *
+ * The transform is the paper's "customized 3D FFT": zero-padded regions are
+ * never read or transformed, the first processed axis is real-to-complex, the K^F multiply is
+ * fused between the last forward and first inverse 1D transforms, and only the physical
+ * octant / quarter / half is written back.  Every step runs in hand-written CUDA kernels;
+ * there is no cuFFT, no CPU fallback, and every entry point fails with a status code (never
+ * aborts, never throws) when it cannot run.
+ *
+ * Conventions (readings of the paper, DESIGN.md section "Readings"):
+ *   - arrays are dense C order [z][y][x], x fastest;
+ *   - data sits in the first half [0,N) of a padded axis, zeros in [N,2N)   (reading 1);
+ *   - forward DFT sign exp(-2 pi i jk/S); forward and inverse are unnormalised and the library
+ *     applies 1/(S_x S_y S_z) itself (reading 2); no h^3 volume element is applied (reading 3).
+ *
+ * Pointer kinds are stated per argument: "device" = CUDA device memory on the current device,
+ * "host" = ordinary or pinned host memory.  `stream` is a cudaStream_t passed as void*
+ * (NULL = the legacy default stream).
+ */
+#ifndef POISSON_B200_H
+#define POISSON_B200_H
+
+#include <stddef.h>
+
+#if defined(__GNUC__)
+#define POISSON_API __attribute__((visibility("default")))
+#else
+#define POISSON_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct poisson_plan poisson_plan; /* opaque; owned by the library */
+
+enum { POISSON_BC_FREE = 0, POISSON_BC_PERIODIC = 1 };          /* B_i = 2 / 1 of PAPER.md:51 */
+enum { POISSON_FP64 = 0, POISSON_FP32 = 1 };
+enum {
+    POISSON_OK = 0,
+    POISSON_EINVAL = 1,       /* null pointer, n <= 0, bc / precision out of range, bad h, misaligned pointer */
+    POISSON_EUNSUPPORTED = 2, /* odd N_i, or a padded length S_i with no compiled transform            */
+    POISSON_ENOMEM = 3,       /* host or device allocation failed                                        */
+    POISSON_ENOKERNEL = 4,    /* poisson_solve before poisson_set_kernel                                 */
+    POISSON_ECUDA = 5,        /* a CUDA call failed (sticky; text via poisson_last_error)                */
+    POISSON_EARCH = 6         /* no CUDA device, or the device is not compute capability 10.x            */
+};
+
+/* Pass indices of the fused 5-pass pipeline (DESIGN.md section "Kernels"):
+ * F1 = spread + 1DFFT (R2C) along the first processed axis a
+ * F2 = (transpose+)spread + 1DFFT along axis b
+ * F3 = spread + 1DFFT along axis c, K^F multiply, inverse 1DFFT along c, compactification
+ * I2 = inverse 1DFFT along b + compactification,  I1 = inverse 1DFFT (C2R) along a + compactification */
+enum { POISSON_PASS_F1 = 0, POISSON_PASS_F2 = 1, POISSON_PASS_F3 = 2, POISSON_PASS_I2 = 3, POISSON_PASS_I1 = 4 };
+
+/* Host-side description of a plan: what the planner decided and the algorithmic work it implies.
+ * Axis ids: 0 = x, 1 = y, 2 = z. */
+typedef struct poisson_plan_info {
+    int n[3];               /* physical grid N_x, N_y, N_z                                         */
+    int bc[3];              /* boundary condition per axis                                         */
+    int s[3];               /* padded transform lengths S_i = N_i * B_i  */
+    int precision;          /* POISSON_FP64 / POISSON_FP32                                         */
+    int order[3];           /* processing order (a, b, c): periodic axes first, free axes last
+                               (PAPER.md:51), and a != x so the half spectrum S_a/2+1 never lands on
+                               the contiguous axis       */
+    int half_len;           /* H = S_a/2 + 1 kept after the real-to-complex pass */
+    long long rows[5];      /* 1D transforms per pass (F3 counts a pencil once per direction)      */
+    long long length[5];    /* transform length of each pass                                        */
+    long long bytes[5];     /* algorithmic HBM bytes per pass (reads + writes, zeros never counted) */
+    long long bytes_total;  /* sum of bytes[]  (= B_5 of SURVEY.md 8d)                              */
+    long long workspace_bytes; /* device memory the plan owns: A1 + A2 + internal K^F + tables     */
+    double fft_fraction;    /* (sum over the 3 forward steps of rows*length) / (3 S_x S_y S_z):
+                               7/12 fully free, 2/3 surface, 7/12 wire */
+} poisson_plan_info;
+
+/* Planner only: fills *info for the given problem without touching any device (usable on a box
+ * with no GPU).  Errors: EINVAL, EUNSUPPORTED as for poisson_plan_create. */
+POISSON_API int poisson_plan_describe(int nx, int ny, int nz, const int bc[3] /* host; x,y,z */, int precision,
+                          poisson_plan_info *info /* host, out */);
+
+/* Creates a plan on the current CUDA device: validates, picks the axis order, allocates the
+ * workspace (A1, A2, internal K^F) and uploads the twiddle tables.  `h` (grid spacing) is recorded
+ * metadata only.  *out is set to NULL on failure.  Problem statement: PAPER.md:51. */
+POISSON_API int poisson_plan_create(poisson_plan **out /* host, out */, int nx, int ny, int nz,
+                        const int bc[3] /* host; x,y,z */, double h, int precision);
+
+/* dims = {S_z, S_y, S_x/2+1}: the shape of the K_f array poisson_set_kernel expects. */
+POISSON_API int poisson_plan_kernel_dims(const poisson_plan *plan, long long dims[3] /* host, out */);
+
+POISSON_API int poisson_plan_get_info(const poisson_plan *plan, poisson_plan_info *info /* host, out */);
+
+/* Installs the Green's-function spectrum K^F of Eq. 3.
+ *   K_f_dev: device, plan-precision REALS, C order [S_z][S_y][S_x/2+1] (numpy rfftn shape) = the
+ *            unnormalised forward DFT of a real kernel K on the padded grid with K(-r) = K(r)
+ *            (so K^F is real; the half not passed is K^F(-k) = K^F(k)).  16-byte aligned.
+ * The library re-lays it once into the order pass F3 streams it in, folding in 1/(S_x S_y S_z)
+ * ("a transposition of the associated kernel ... carried out only once").
+ * Asynchronous on `stream`; K_f_dev may be freed once that work has completed. */
+POISSON_API int poisson_set_kernel(poisson_plan *plan, const void *K_f_dev, void *stream);
+
+/* One solve (the 13 steps of PAPER.md:57-71 as 5 fused launches on `stream`).
+ *   rho_dev: device, plan-precision reals [nz][ny][nx], 16-byte aligned, not modified
+ *   V_dev  : device, same shape; may equal rho_dev (rho is consumed before V is written)
+ * Asynchronous, allocates nothing, never touches host memory.  One plan = one solve in flight
+ * (the workspace is shared).  Errors: EINVAL, ENOKERNEL, ECUDA. */
+POISSON_API int poisson_solve(poisson_plan *plan, const void *rho_dev, void *V_dev, void *stream);
+
+/* End-to-end variant with HOST buffers (the paper's usage: density on the host, potential wanted
+ * back on the host): H2D copy of rho, poisson_solve, D2H copy of V, then a stream
+ * synchronise.  rho_host / V_host: host memory (pinned for full speed), [nz][ny][nx] reals.
+ * The plan owns the two device staging buffers (allocated on first use). */
+POISSON_API int poisson_solve_host(poisson_plan *plan, const void *rho_host, void *V_host, void *stream);
+
+/* Debug/test access to the plan's intermediates (per-pass parity).  which = 0: A1,
+ * complex [.][.][.] after F1 (or after I2); which = 1: A2 after F2 / F3.  dims are the array
+ * extents in memory order (z-extent, y-extent, x-extent), each axis holding N_i, S_i or H. */
+POISSON_API int poisson_debug_workspace(const poisson_plan *plan, int which, void **ptr_dev /* out */,
+                            long long dims[3] /* host, out */);
+/* Runs passes [first, last] (POISSON_PASS_*) of a solve only; same arguments as poisson_solve. */
+POISSON_API int poisson_debug_run_passes(poisson_plan *plan, const void *rho_dev, void *V_dev, void *stream,
+                             int first_pass, int last_pass);
+
+/* Number of kernel launches one poisson_solve enqueues (bench.py's gpu_launches). */
+POISSON_API int poisson_plan_launches_per_solve(const poisson_plan *plan);
+
+POISSON_API size_t poisson_plan_workspace_bytes(const poisson_plan *plan);
+POISSON_API int poisson_plan_destroy(poisson_plan *plan);
+
+POISSON_API const char *poisson_status_string(int status);
+/* Text of the last CUDA error seen by this thread's most recent failing call ("" if none). */
+POISSON_API const char *poisson_last_error(void);
+/* "sm_100a" etc.: the architecture the kernels were compiled for. */
+POISSON_API const char *poisson_build_arch(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* POISSON_B200_H */

@@ -1,0 +1,217 @@
+"""paper_1211_5244_b200 -- thin Python binding of the C-ABI library in include/poisson.h.
+
+Argument marshalling only: every step of the solve runs in the hand-written sm_100a kernels of
+libpoisson_b200.so.  PyTorch is used by callers for device memory and streams; this module only
+needs `.data_ptr()` integers and a raw cudaStream_t.  There is no CPU fallback: if the library
+is missing or no B200 is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+__all__ = [
+    "FREE", "PERIODIC", "FP64", "FP32", "PoissonError", "PlanInfo", "lib_path", "load_library",
+    "poisson_plan_describe", "poisson_plan_create", "poisson_set_kernel", "poisson_solve",
+    "poisson_solve_host", "poisson_plan_destroy", "PoissonPlan", "EXPORTED_SYMBOLS",
+]
+
+FREE, PERIODIC = 0, 1
+FP64, FP32 = 0, 1
+PASS_NAMES = ("F1", "F2", "F3", "I2", "I1")
+
+EXPORTED_SYMBOLS = (
+    "poisson_plan_describe", "poisson_plan_create", "poisson_plan_kernel_dims", "poisson_plan_get_info",
+    "poisson_set_kernel", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
+    "poisson_debug_run_passes", "poisson_plan_launches_per_solve", "poisson_plan_workspace_bytes",
+    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch",
+)
+
+_PKG = Path(__file__).resolve().parent
+_LIB_PATH = _PKG / "libpoisson_b200.so"
+_lib = None
+
+
+class PoissonError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        self.status = status
+        super().__init__(f"{where}: status {status} ({detail})")
+
+
+class PlanInfo(ctypes.Structure):
+    """Mirror of `poisson_plan_info` (include/poisson.h)."""
+    _fields_ = [
+        ("n", ctypes.c_int * 3), ("bc", ctypes.c_int * 3), ("s", ctypes.c_int * 3),
+        ("precision", ctypes.c_int), ("order", ctypes.c_int * 3), ("half_len", ctypes.c_int),
+        ("rows", ctypes.c_longlong * 5), ("length", ctypes.c_longlong * 5), ("bytes", ctypes.c_longlong * 5),
+        ("bytes_total", ctypes.c_longlong), ("workspace_bytes", ctypes.c_longlong),
+        ("fft_fraction", ctypes.c_double),
+    ]
+
+    def as_dict(self):
+        return {
+            "n": list(self.n), "bc": list(self.bc), "s": list(self.s), "precision": self.precision,
+            "order": list(self.order), "half_len": self.half_len, "rows": list(self.rows),
+            "length": list(self.length), "bytes": list(self.bytes), "bytes_total": self.bytes_total,
+            "workspace_bytes": self.workspace_bytes, "fft_fraction": self.fft_fraction,
+        }
+
+
+def lib_path() -> Path:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen the in-tree library.  Fails loudly when it has not been built (no fallback exists)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        raise ImportError(
+            f"{_LIB_PATH} is missing: run `python -m paper_1211_5244_b200.build` (or __graft_entry__.build()). "
+            "The solve has no CPU or library fallback.")
+    lib = ctypes.CDLL(str(_LIB_PATH))
+    vp, i, ll = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong
+    i3 = ctypes.c_int * 3
+    lib.poisson_plan_describe.argtypes = [i, i, i, i3, i, ctypes.POINTER(PlanInfo)]
+    lib.poisson_plan_create.argtypes = [ctypes.POINTER(vp), i, i, i, i3, ctypes.c_double, i]
+    lib.poisson_plan_kernel_dims.argtypes = [vp, ll * 3]
+    lib.poisson_plan_get_info.argtypes = [vp, ctypes.POINTER(PlanInfo)]
+    lib.poisson_set_kernel.argtypes = [vp, vp, vp]
+    lib.poisson_solve.argtypes = [vp, vp, vp, vp]
+    lib.poisson_solve_host.argtypes = [vp, vp, vp, vp]
+    lib.poisson_debug_workspace.argtypes = [vp, i, ctypes.POINTER(vp), ll * 3]
+    lib.poisson_debug_run_passes.argtypes = [vp, vp, vp, vp, i, i]
+    lib.poisson_plan_launches_per_solve.argtypes = [vp]
+    lib.poisson_plan_workspace_bytes.argtypes = [vp]
+    lib.poisson_plan_workspace_bytes.restype = ctypes.c_size_t
+    lib.poisson_plan_destroy.argtypes = [vp]
+    lib.poisson_status_string.argtypes = [i]
+    lib.poisson_status_string.restype = ctypes.c_char_p
+    lib.poisson_last_error.restype = ctypes.c_char_p
+    lib.poisson_build_arch.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        lib = load_library()
+        msg = lib.poisson_status_string(status).decode()
+        extra = lib.poisson_last_error().decode()
+        raise PoissonError(status, where, msg + (f"; {extra}" if extra else ""))
+
+
+# ------------------------------------------------------------------ function-level API (same names as the C ABI)
+def poisson_plan_describe(nx: int, ny: int, nz: int, bc, precision: int = FP64) -> PlanInfo:
+    info = PlanInfo()
+    _check(load_library().poisson_plan_describe(nx, ny, nz, (ctypes.c_int * 3)(*bc), precision, ctypes.byref(info)),
+           "poisson_plan_describe")
+    return info
+
+
+def poisson_plan_create(nx: int, ny: int, nz: int, bc, h: float, precision: int = FP64) -> int:
+    """Returns the opaque plan handle (an integer address)."""
+    handle = ctypes.c_void_p()
+    _check(load_library().poisson_plan_create(ctypes.byref(handle), nx, ny, nz, (ctypes.c_int * 3)(*bc), float(h),
+                                              precision), "poisson_plan_create")
+    return handle.value
+
+
+def poisson_set_kernel(plan: int, K_f_dev_ptr: int, stream: int = 0) -> None:
+    _check(load_library().poisson_set_kernel(plan, K_f_dev_ptr, stream), "poisson_set_kernel")
+
+
+def poisson_solve(plan: int, rho_dev_ptr: int, V_dev_ptr: int, stream: int = 0) -> None:
+    _check(load_library().poisson_solve(plan, rho_dev_ptr, V_dev_ptr, stream), "poisson_solve")
+
+
+def poisson_solve_host(plan: int, rho_host_ptr: int, V_host_ptr: int, stream: int = 0) -> None:
+    _check(load_library().poisson_solve_host(plan, rho_host_ptr, V_host_ptr, stream), "poisson_solve_host")
+
+
+def poisson_plan_destroy(plan: int) -> None:
+    _check(load_library().poisson_plan_destroy(plan), "poisson_plan_destroy")
+
+
+# ------------------------------------------------------------------ small convenience wrapper over torch tensors
+class PoissonPlan:
+    """Owns a plan handle; takes torch CUDA tensors and forwards their pointers (no arithmetic here)."""
+
+    def __init__(self, n, bc, h: float, precision: int = FP64):
+        self.n = tuple(int(v) for v in n)          # (nx, ny, nz)
+        self.bc = tuple(int(v) for v in bc)
+        self.precision = precision
+        self._h = poisson_plan_create(self.n[0], self.n[1], self.n[2], self.bc, h, precision)
+        info = PlanInfo()
+        _check(load_library().poisson_plan_get_info(self._h, ctypes.byref(info)), "poisson_plan_get_info")
+        self.info = info
+        dims = (ctypes.c_longlong * 3)()
+        _check(load_library().poisson_plan_kernel_dims(self._h, dims), "poisson_plan_kernel_dims")
+        self.kernel_dims = tuple(dims)
+
+    @property
+    def handle(self) -> int:
+        return self._h
+
+    @staticmethod
+    def _stream(stream):
+        if stream is None:
+            import torch
+            return torch.cuda.current_stream().cuda_stream
+        return int(getattr(stream, "cuda_stream", stream))
+
+    def _dtype(self):
+        import torch
+        return torch.float64 if self.precision == FP64 else torch.float32
+
+    def set_kernel(self, K_f, stream=None):
+        assert K_f.is_cuda and K_f.is_contiguous() and K_f.dtype == self._dtype()
+        assert tuple(K_f.shape) == self.kernel_dims, (tuple(K_f.shape), self.kernel_dims)
+        poisson_set_kernel(self._h, K_f.data_ptr(), self._stream(stream))
+
+    def solve(self, rho, V=None, stream=None):
+        import torch
+        assert rho.is_cuda and rho.is_contiguous() and rho.dtype == self._dtype()
+        assert tuple(rho.shape) == (self.n[2], self.n[1], self.n[0])
+        if V is None:
+            V = torch.empty_like(rho)
+        assert V.is_cuda and V.is_contiguous() and V.dtype == rho.dtype and V.shape == rho.shape
+        poisson_solve(self._h, rho.data_ptr(), V.data_ptr(), self._stream(stream))
+        return V
+
+    def solve_host(self, rho_host, V_host, stream=None):
+        """rho_host / V_host: CPU tensors (pinned for full speed); H2D + solve + D2H + sync inside the C call."""
+        assert not rho_host.is_cuda and not V_host.is_cuda and rho_host.is_contiguous() and V_host.is_contiguous()
+        assert rho_host.dtype == self._dtype() and V_host.dtype == self._dtype()
+        poisson_solve_host(self._h, rho_host.data_ptr(), V_host.data_ptr(), self._stream(stream))
+        return V_host
+
+    def launches_per_solve(self) -> int:
+        return load_library().poisson_plan_launches_per_solve(self._h)
+
+    def workspace_bytes(self) -> int:
+        return load_library().poisson_plan_workspace_bytes(self._h)
+
+    def debug_workspace(self, which: int):
+        """(device pointer, (ez, ey, ex)) of intermediate A1 (which=0) or A2 (which=1)."""
+        ptr = ctypes.c_void_p()
+        dims = (ctypes.c_longlong * 3)()
+        _check(load_library().poisson_debug_workspace(self._h, which, ctypes.byref(ptr), dims), "poisson_debug_workspace")
+        return ptr.value, tuple(dims)
+
+    def debug_run_passes(self, rho, V, first: int, last: int, stream=None):
+        _check(load_library().poisson_debug_run_passes(
+            self._h, rho.data_ptr() if rho is not None else None, V.data_ptr() if V is not None else None,
+            self._stream(stream), first, last), "poisson_debug_run_passes")
+
+    def close(self):
+        if self._h:
+            poisson_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

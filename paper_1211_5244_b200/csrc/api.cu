@@ -1,0 +1,309 @@
+// api.cu -- the C ABI of include/poisson.h: plan creation, K^F re-layout, the 5-launch solve.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/poisson.h"
+#include "passes.cuh"
+#include "planner.hpp"
+#include "registry.hpp"
+#include "relayout.cuh"
+
+namespace pfft {
+
+std::vector<KernelEntry> &kernel_registry() {
+    static std::vector<KernelEntry> reg;
+    return reg;
+}
+
+const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int prec) {
+    for (const KernelEntry &e : kernel_registry())
+        if (e.kind == kind && e.S == S && e.pruned == pruned && e.lanes_p == lanes_p && e.prec == prec) return &e;
+    return nullptr;
+}
+
+static thread_local std::string g_last_error;
+
+static int cuda_fail(cudaError_t e, const char *what) {
+    g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
+    return POISSON_ECUDA;
+}
+#define PF_CUDA(call)                                          \
+    do {                                                       \
+        cudaError_t pf_e = (call);                             \
+        if (pf_e != cudaSuccess) return cuda_fail(pf_e, #call); \
+    } while (0)
+
+template <typename T>
+__global__ void relayout_kernel(const T *__restrict__ kuser, T *__restrict__ kint, const RelayoutParams q) {
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < q.total;
+         idx += (long long)gridDim.x * blockDim.x)
+        kint[idx] = relayout_value<T>(kuser, q, idx);
+}
+
+}  // namespace pfft
+
+using namespace pfft;
+
+struct poisson_plan {
+    PlanDesc d;
+    double h;
+    int device;
+    int num_sms;
+    const KernelEntry *k[5];
+    int grid[5];
+    int n_tiles[5], tiles_per_g[5];
+    void *a1, *a2, *kint;
+    void *tw[3];          // per axis id
+    void *rho_stage, *v_stage;
+    size_t elem_real;     // bytes per real
+    long long kint_elems;
+    size_t workspace_bytes;
+    bool kernel_set;
+};
+
+static void fill_twiddles(std::vector<unsigned char> &buf, int S, int prec) {
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    buf.resize((size_t)S * (prec == POISSON_FP64 ? 16 : 8));
+    for (int m = 0; m < S; ++m) {
+        long double c, s;
+        if ((4LL * m) % S == 0) {  // exact on the axes
+            const int qt = (int)((4LL * m) / S);
+            c = qt == 0 ? 1.0L : (qt == 2 ? -1.0L : 0.0L);
+            s = qt == 1 ? -1.0L : (qt == 3 ? 1.0L : 0.0L);
+        } else {
+            const long double ang = two_pi * (long double)m / (long double)S;
+            c = cosl(ang); s = -sinl(ang);  // exp(-2 pi i m / S)
+        }
+        if (prec == POISSON_FP64) { double *o = reinterpret_cast<double *>(buf.data()) + 2 * m; o[0] = (double)c; o[1] = (double)s; }
+        else { float *o = reinterpret_cast<float *>(buf.data()) + 2 * m; o[0] = (float)c; o[1] = (float)s; }
+    }
+}
+
+static void free_plan(poisson_plan *pl) {
+    if (!pl) return;
+    cudaFree(pl->a1); cudaFree(pl->a2); cudaFree(pl->kint);
+    for (int q = 0; q < 3; ++q) cudaFree(pl->tw[q]);
+    cudaFree(pl->rho_stage); cudaFree(pl->v_stage);
+    delete pl;
+}
+
+extern "C" {
+
+const char *poisson_status_string(int st) {
+    switch (st) {
+        case POISSON_OK: return "ok";
+        case POISSON_EINVAL: return "invalid argument";
+        case POISSON_EUNSUPPORTED: return "unsupported grid size (odd N, or no compiled transform for a padded length)";
+        case POISSON_ENOMEM: return "out of memory";
+        case POISSON_ENOKERNEL: return "poisson_solve called before poisson_set_kernel";
+        case POISSON_ECUDA: return "CUDA error (see poisson_last_error)";
+        case POISSON_EARCH: return "no CUDA device of compute capability 10.x (kernels are built for sm_100a)";
+        default: return "unknown status";
+    }
+}
+
+const char *poisson_last_error(void) { return g_last_error.c_str(); }
+
+const char *poisson_build_arch(void) { return "sm_100a"; }
+
+int poisson_plan_describe(int nx, int ny, int nz, const int bc[3], int precision, poisson_plan_info *info) {
+    if (!info) return POISSON_EINVAL;
+    PlanDesc d;
+    const int st = plan_build(nx, ny, nz, bc, precision, d);
+    if (st != POISSON_OK) return st;
+    for (int q = 0; q < 5; ++q)
+        if (!find_kernel(d.pass[q].kind, d.pass[q].S, d.pass[q].pruned, d.pass[q].lanes_p, precision))
+            return POISSON_EUNSUPPORTED;
+    *info = d.info;
+    return POISSON_OK;
+}
+
+int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc[3], double h, int precision) {
+    if (!out) return POISSON_EINVAL;
+    *out = nullptr;
+    if (!(h > 0.0) || !std::isfinite(h)) return POISSON_EINVAL;
+    PlanDesc d;
+    int st = plan_build(nx, ny, nz, bc, precision, d);
+    if (st != POISSON_OK) return st;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        g_last_error = "no CUDA device";
+        return POISSON_EARCH;
+    }
+    int dev = 0;
+    PF_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    PF_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) {
+        g_last_error = "device is sm_" + std::to_string(prop.major * 10 + prop.minor) + ", kernels are sm_100a";
+        return POISSON_EARCH;
+    }
+
+    poisson_plan *pl = new (std::nothrow) poisson_plan();
+    if (!pl) return POISSON_ENOMEM;
+    std::memset(static_cast<void *>(pl), 0, sizeof(*pl));
+    pl->d = d; pl->h = h; pl->device = dev; pl->num_sms = prop.multiProcessorCount;
+    pl->elem_real = precision == POISSON_FP64 ? 8 : 4;
+
+    for (int q = 0; q < 5; ++q) {
+        const PassDesc &ps = d.pass[q];
+        const KernelEntry *e = find_kernel(ps.kind, ps.S, ps.pruned, ps.lanes_p, precision);
+        if (!e) { free_plan(pl); return POISSON_EUNSUPPORTED; }
+        pl->k[q] = e;
+        pl->tiles_per_g[q] = (int)((ps.n_p + e->P - 1) / e->P);
+        pl->n_tiles[q] = (int)(ps.n_g * pl->tiles_per_g[q]);
+        cudaError_t ce = cudaFuncSetAttribute(e->func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e->smem_bytes);
+        if (ce != cudaSuccess) { free_plan(pl); return cuda_fail(ce, "cudaFuncSetAttribute(smem)"); }
+        int occ = 0;
+        ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, e->func, e->NT, e->smem_bytes);
+        if (ce != cudaSuccess || occ < 1) { free_plan(pl); return cuda_fail(ce, "occupancy query"); }
+        const long long resident = (long long)occ * pl->num_sms;
+        pl->grid[q] = (int)(pl->n_tiles[q] < resident ? pl->n_tiles[q] : resident);  // persistent CTAs
+    }
+
+    const size_t cplx = 2 * pl->elem_real;
+    pl->kint_elems = (long long)pl->n_tiles[2] * pl->k[2]->V * pl->k[2]->NT;
+    size_t ws = 0;
+    cudaError_t ce = cudaMalloc(&pl->a1, (size_t)d.a1_elems * cplx); ws += (size_t)d.a1_elems * cplx;
+    if (ce == cudaSuccess) { ce = cudaMalloc(&pl->a2, (size_t)d.a2_elems * cplx); ws += (size_t)d.a2_elems * cplx; }
+    if (ce == cudaSuccess) { ce = cudaMalloc(&pl->kint, (size_t)pl->kint_elems * pl->elem_real); ws += (size_t)pl->kint_elems * pl->elem_real; }
+    for (int q = 0; q < 3 && ce == cudaSuccess; ++q) {
+        std::vector<unsigned char> host;
+        fill_twiddles(host, d.s[q], precision);
+        ce = cudaMalloc(&pl->tw[q], host.size());
+        if (ce == cudaSuccess) ce = cudaMemcpy(pl->tw[q], host.data(), host.size(), cudaMemcpyHostToDevice);
+        ws += host.size();
+    }
+    if (ce != cudaSuccess) {
+        free_plan(pl);
+        if (ce == cudaErrorMemoryAllocation) { cudaGetLastError(); return POISSON_ENOMEM; }
+        return cuda_fail(ce, "workspace allocation");
+    }
+    pl->workspace_bytes = ws;
+    pl->d.info.workspace_bytes = (long long)ws;
+    *out = pl;
+    return POISSON_OK;
+}
+
+int poisson_plan_kernel_dims(const poisson_plan *pl, long long dims[3]) {
+    if (!pl || !dims) return POISSON_EINVAL;
+    dims[0] = pl->d.s[2]; dims[1] = pl->d.s[1]; dims[2] = pl->d.s[0] / 2 + 1;
+    return POISSON_OK;
+}
+
+int poisson_plan_get_info(const poisson_plan *pl, poisson_plan_info *info) {
+    if (!pl || !info) return POISSON_EINVAL;
+    *info = pl->d.info;
+    return POISSON_OK;
+}
+
+size_t poisson_plan_workspace_bytes(const poisson_plan *pl) { return pl ? pl->workspace_bytes : 0; }
+
+int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? 5 : 0; }
+
+int poisson_plan_destroy(poisson_plan *pl) {
+    if (!pl) return POISSON_EINVAL;
+    free_plan(pl);
+    return POISSON_OK;
+}
+
+int poisson_set_kernel(poisson_plan *pl, const void *K_f_dev, void *stream) {
+    if (!pl || !K_f_dev) return POISSON_EINVAL;
+    if (reinterpret_cast<size_t>(K_f_dev) % 16) return POISSON_EINVAL;
+    const PlanDesc &d = pl->d;
+    const KernelEntry *e = pl->k[2];
+    RelayoutParams q;
+    q.RA = e->RA; q.RB = e->RB; q.TPP = e->TPP; q.P = e->P; q.V = e->V; q.NT = e->NT; q.lanes_p = e->lanes_p;
+    q.tiles_per_g = pl->tiles_per_g[2]; q.n_p = (int)d.pass[2].n_p;
+    q.a_axis = d.order[0]; q.c_axis = d.order[2];
+    q.ext2y = d.ext2[1];
+    q.sx = d.s[0]; q.sy = d.s[1]; q.sz = d.s[2];
+    q.total = pl->kint_elems;
+    q.scale = 1.0 / ((double)d.s[0] * (double)d.s[1] * (double)d.s[2]);  // reading 2: one 1/(SxSySz)
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    const int threads = 256;
+    long long blocks = (q.total + threads - 1) / threads;
+    if (blocks > 148LL * 32) blocks = 148LL * 32;
+    if (d.prec == POISSON_FP64)
+        relayout_kernel<double><<<(int)blocks, threads, 0, st>>>(static_cast<const double *>(K_f_dev), static_cast<double *>(pl->kint), q);
+    else
+        relayout_kernel<float><<<(int)blocks, threads, 0, st>>>(static_cast<const float *>(K_f_dev), static_cast<float *>(pl->kint), q);
+    PF_CUDA(cudaGetLastError());
+    pl->kernel_set = true;
+    return POISSON_OK;
+}
+
+static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t st, int first, int last) {
+    const PlanDesc &d = pl->d;
+    for (int q = first; q <= last; ++q) {
+        const PassDesc &ps = d.pass[q];
+        const KernelEntry *e = pl->k[q];
+        PassParams prm;
+        switch (q) {
+            case POISSON_PASS_F1: prm.in = rho; prm.out = pl->a1; break;
+            case POISSON_PASS_F2: prm.in = pl->a1; prm.out = pl->a2; break;
+            case POISSON_PASS_F3: prm.in = pl->a2; prm.out = pl->a2; break;
+            case POISSON_PASS_I2: prm.in = pl->a2; prm.out = pl->a1; break;
+            default: prm.in = pl->a1; prm.out = V; break;
+        }
+        prm.kint = pl->kint;
+        prm.tw = pl->tw[ps.axis];
+        prm.gs_in = ps.gs_in; prm.ns_in = ps.ns_in; prm.ps_in = ps.ps_in;
+        prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;
+        prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q];
+        void *args[] = {&prm};
+        PF_CUDA(cudaLaunchKernel(e->func, dim3(pl->grid[q]), dim3(e->NT), args, e->smem_bytes, st));
+    }
+    return POISSON_OK;
+}
+
+int poisson_solve(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stream) {
+    if (!pl || !rho_dev || !V_dev) return POISSON_EINVAL;
+    if (reinterpret_cast<size_t>(rho_dev) % 16 || reinterpret_cast<size_t>(V_dev) % 16) return POISSON_EINVAL;
+    if (!pl->kernel_set) return POISSON_ENOKERNEL;
+    return run_passes(pl, rho_dev, V_dev, reinterpret_cast<cudaStream_t>(stream), 0, 4);
+}
+
+int poisson_debug_run_passes(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stream, int first, int last) {
+    if (!pl || first < 0 || last > 4 || first > last) return POISSON_EINVAL;
+    if (first == 0 && !rho_dev) return POISSON_EINVAL;
+    if (last == 4 && !V_dev) return POISSON_EINVAL;
+    if (first <= 2 && last >= 2 && !pl->kernel_set) return POISSON_ENOKERNEL;
+    return run_passes(pl, rho_dev, V_dev, reinterpret_cast<cudaStream_t>(stream), first, last);
+}
+
+int poisson_debug_workspace(const poisson_plan *pl, int which, void **ptr, long long dims[3]) {
+    if (!pl || !ptr || !dims || (which != 0 && which != 1)) return POISSON_EINVAL;
+    const long long *ext = which == 0 ? pl->d.ext1 : pl->d.ext2;
+    *ptr = which == 0 ? pl->a1 : pl->a2;
+    dims[0] = ext[2]; dims[1] = ext[1]; dims[2] = ext[0];
+    return POISSON_OK;
+}
+
+int poisson_solve_host(poisson_plan *pl, const void *rho_host, void *V_host, void *stream) {
+    if (!pl || !rho_host || !V_host) return POISSON_EINVAL;
+    if (!pl->kernel_set) return POISSON_ENOKERNEL;
+    const size_t bytes = (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * pl->elem_real;
+    if (!pl->rho_stage) {
+        cudaError_t ce = cudaMalloc(&pl->rho_stage, bytes);
+        if (ce == cudaSuccess) ce = cudaMalloc(&pl->v_stage, bytes);
+        if (ce != cudaSuccess) { cudaGetLastError(); return ce == cudaErrorMemoryAllocation ? POISSON_ENOMEM : cuda_fail(ce, "staging allocation"); }
+    }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    PF_CUDA(cudaMemcpyAsync(pl->rho_stage, rho_host, bytes, cudaMemcpyHostToDevice, st));
+    const int rc = run_passes(pl, pl->rho_stage, pl->v_stage, st, 0, 4);
+    if (rc != POISSON_OK) return rc;
+    PF_CUDA(cudaMemcpyAsync(V_host, pl->v_stage, bytes, cudaMemcpyDeviceToHost, st));
+    PF_CUDA(cudaStreamSynchronize(st));
+    return POISSON_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,236 @@
+// fft_core.cuh -- in-register building blocks of the customised FFT:
+// complex arithmetic, compile-time twiddles, small DFTs of radix 2..32 held entirely in one
+// thread's registers, and the two "pruned" variants that implement the paper's spread /
+// compactification without ever touching the zero half:
+//   * dft_pruned_in  : DFT of a length-R sequence whose upper half is zero   (spread,  PAPER.md:53)
+//   * dft_pruned_out : DFT of a length-R sequence keeping only outputs n<R/2 (compactification)
+// Everything is __host__ __device__ so the index algebra can be exercised on a CPU during
+// development; the product only ever runs the __global__ kernels built from it.
+#pragma once
+
+#include <cstddef>
+#include <utility>
+
+#include "twiddle_consts.cuh"
+
+#if defined(__CUDACC__)
+#define PF_HD __host__ __device__ __forceinline__
+#define PF_CE __host__ __device__ constexpr
+#else
+#define PF_HD inline __attribute__((always_inline))
+#define PF_CE constexpr
+#endif
+
+namespace pfft {
+
+// ------------------------------------------------------------------ complex number
+template <typename T>
+struct alignas(2 * sizeof(T)) cx {
+    T re, im;
+};
+
+template <typename T> PF_HD cx<T> mk(T re, T im) { cx<T> r; r.re = re; r.im = im; return r; }
+template <typename T> PF_HD cx<T> operator+(cx<T> a, cx<T> b) { return mk<T>(a.re + b.re, a.im + b.im); }
+template <typename T> PF_HD cx<T> operator-(cx<T> a, cx<T> b) { return mk<T>(a.re - b.re, a.im - b.im); }
+template <typename T> PF_HD cx<T> operator*(cx<T> a, cx<T> b) {
+    return mk<T>(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re);
+}
+template <typename T> PF_HD cx<T> scale(cx<T> a, T s) { return mk<T>(a.re * s, a.im * s); }
+template <typename T> PF_HD cx<T> conj(cx<T> a) { return mk<T>(a.re, -a.im); }
+template <typename T> PF_HD cx<T> mul_conj(cx<T> a, cx<T> w) {  // a * conj(w)
+    return mk<T>(a.re * w.re + a.im * w.im, a.im * w.re - a.re * w.im);
+}
+// multiply by -i (forward quarter turn) or +i
+template <typename T> PF_HD cx<T> mul_mi(cx<T> a) { return mk<T>(a.im, -a.re); }
+template <typename T> PF_HD cx<T> mul_pi(cx<T> a) { return mk<T>(-a.im, a.re); }
+
+// ------------------------------------------------------------------ compile-time loops
+template <int... Is, typename F>
+PF_HD void static_for_impl(std::integer_sequence<int, Is...>, F &&f) {
+    (f(std::integral_constant<int, Is>{}), ...);
+}
+template <int N, typename F>
+PF_HD void static_for(F &&f) {
+    static_for_impl(std::make_integer_sequence<int, N>{}, static_cast<F &&>(f));
+}
+
+// ------------------------------------------------------------------ compile-time twiddles
+// cos/sin(2 pi m / R) for R | 480, reduced to the first octant of a 61-entry literal table.
+PF_CE double oct_cos(int j) { constexpr double t[61] = {PFFT_OCT_COS_LIST}; return t[j]; }
+PF_CE double oct_sin(int j) { constexpr double t[61] = {PFFT_OCT_SIN_LIST}; return t[j]; }
+
+PF_CE double cos480(int j) {  // j in [0, 480)
+    if (j > 240) j = 480 - j;               // cos(-x) = cos(x)
+    bool neg = false;
+    if (j > 120) { j = 240 - j; neg = true; }  // cos(pi - x) = -cos(x)
+    double v = (j <= 60) ? oct_cos(j) : oct_sin(120 - j);
+    if (j == 120) v = 0.0;
+    return neg ? -v : v;
+}
+PF_CE double sin480(int j) {  // j in [0, 480)
+    bool neg = false;
+    if (j > 240) { j = 480 - j; neg = true; }  // sin(-x) = -sin(x)
+    if (j > 120) j = 240 - j;                   // sin(pi - x) = sin(x)
+    double v = (j <= 60) ? oct_sin(j) : oct_cos(120 - j);
+    if (j == 0 || j == 240) v = 0.0;
+    return neg ? -v : v;
+}
+PF_CE bool divides480(int R) { return R > 0 && 480 % R == 0; }
+// real / imaginary part of exp(-2 pi i m / R)   (forward sign)
+PF_CE double tw_re(int m, int R) { return cos480((((m % R) + R) % R) * (480 / R)); }
+PF_CE double tw_im(int m, int R) { return -sin480((((m % R) + R) % R) * (480 / R)); }
+
+// a * exp(-/+ 2 pi i M / R) with M, R compile-time: trivial cases cost no multiply.
+template <int M_, int R, bool INV, typename T>
+PF_HD cx<T> mul_tw(cx<T> a) {
+    static_assert(divides480(R), "radix must divide 480");
+    constexpr int M = ((M_ % R) + R) % R;
+    if constexpr (M == 0) {
+        return a;
+    } else if constexpr (4 * M == R) {
+        return INV ? mul_pi(a) : mul_mi(a);
+    } else if constexpr (2 * M == R) {
+        return mk<T>(-a.re, -a.im);
+    } else if constexpr (4 * M == 3 * R) {
+        return INV ? mul_mi(a) : mul_pi(a);
+    } else if constexpr (8 * M == R || 8 * M == 3 * R || 8 * M == 5 * R || 8 * M == 7 * R) {
+        // (+-1 +- i)/sqrt(2): two adds and two multiplies
+        constexpr T h = (T)0.70710678118654752440084436210484903928;
+        constexpr double c = tw_re(M, R), s = INV ? -tw_im(M, R) : tw_im(M, R);
+        // result = (c + i s)(re + i im) with |c| = |s| = h
+        const T p = a.re - a.im, q = a.re + a.im;  // re*1 - im*1 ; re*1 + im*1
+        if constexpr (c > 0 && s > 0) return mk<T>(h * p, h * q);         //  (1+i)/r2
+        else if constexpr (c > 0 && s < 0) return mk<T>(h * q, -(h * p)); //  (1-i)/r2
+        else if constexpr (c < 0 && s > 0) return mk<T>(-(h * q), h * p); // (-1+i)/r2
+        else return mk<T>(-(h * p), -(h * q));                            // (-1-i)/r2
+    } else {
+        constexpr T c = (T)tw_re(M, R);
+        constexpr T s = (T)(INV ? -tw_im(M, R) : tw_im(M, R));
+        return mk<T>(a.re * c - a.im * s, a.re * s + a.im * c);
+    }
+}
+
+// ------------------------------------------------------------------ small DFTs (natural order in, natural order out)
+// X[k] = sum_n x[n] exp(-/+ 2 pi i n k / R)   (INV: + sign, unnormalised)
+template <typename T, int R, bool INV> struct Dft;
+
+template <typename T, bool INV> struct Dft<T, 1, INV> { static PF_HD void run(cx<T> *) {} };
+
+template <typename T, bool INV> struct Dft<T, 2, INV> {
+    static PF_HD void run(cx<T> *x) {
+        const cx<T> a = x[0], b = x[1];
+        x[0] = a + b; x[1] = a - b;
+    }
+};
+
+template <typename T, bool INV> struct Dft<T, 3, INV> {
+    static PF_HD void run(cx<T> *x) {
+        constexpr T s3 = (T)0.86602540378443864676372317075293618347;  // sin(2 pi/3)
+        const cx<T> t1 = x[1] + x[2];
+        const cx<T> t2 = mk<T>(x[0].re - (T)0.5 * t1.re, x[0].im - (T)0.5 * t1.im);
+        const cx<T> d = x[1] - x[2];
+        // forward: X1 = t2 - i s3 d ; X2 = t2 + i s3 d
+        const cx<T> t3 = INV ? mk<T>(-s3 * d.im, s3 * d.re) : mk<T>(s3 * d.im, -(s3 * d.re));
+        x[0] = x[0] + t1; x[1] = t2 + t3; x[2] = t2 - t3;
+    }
+};
+
+template <typename T, bool INV> struct Dft<T, 4, INV> {
+    static PF_HD void run(cx<T> *x) {
+        const cx<T> a = x[0] + x[2], b = x[0] - x[2], c = x[1] + x[3], d = x[1] - x[3];
+        const cx<T> jd = INV ? mul_pi(d) : mul_mi(d);  // forward: -i d
+        x[0] = a + c; x[1] = b + jd; x[2] = a - c; x[3] = b - jd;
+    }
+};
+
+template <typename T, bool INV> struct Dft<T, 5, INV> {
+    static PF_HD void run(cx<T> *x) {
+        constexpr T c1 = (T)0.30901699437494742410229341718281905886;   // cos(2 pi/5)
+        constexpr T c2 = (T)-0.80901699437494742410229341718281905886;  // cos(4 pi/5)
+        constexpr T s1 = (T)0.95105651629515357211643933337938214340;   // sin(2 pi/5)
+        constexpr T s2 = (T)0.58778525229247312916870595463907276860;   // sin(4 pi/5)
+        const cx<T> a1 = x[1] + x[4], b1 = x[1] - x[4], a2 = x[2] + x[3], b2 = x[2] - x[3];
+        const cx<T> m1 = mk<T>(x[0].re + c1 * a1.re + c2 * a2.re, x[0].im + c1 * a1.im + c2 * a2.im);
+        const cx<T> m2 = mk<T>(x[0].re + c2 * a1.re + c1 * a2.re, x[0].im + c2 * a1.im + c1 * a2.im);
+        const cx<T> u1 = mk<T>(s1 * b1.re + s2 * b2.re, s1 * b1.im + s2 * b2.im);
+        const cx<T> u2 = mk<T>(s2 * b1.re - s1 * b2.re, s2 * b1.im - s1 * b2.im);
+        // forward: X1 = m1 - i u1, X4 = m1 + i u1, X2 = m2 - i u2, X3 = m2 + i u2
+        const cx<T> v1 = INV ? mul_pi(u1) : mul_mi(u1);
+        const cx<T> v2 = INV ? mul_pi(u2) : mul_mi(u2);
+        x[0] = x[0] + a1 + a2;
+        x[1] = m1 + v1; x[4] = m1 - v1; x[2] = m2 + v2; x[3] = m2 - v2;
+    }
+};
+
+// first factor A of the Cooley-Tukey split R = A * B used for composite radices
+PF_CE int split_a(int R) {
+    return R == 6 ? 2 : R == 8 ? 2 : R == 10 ? 2 : R == 12 ? 3 : R == 16 ? 4 : R == 20 ? 4
+         : R == 24 ? 3 : R == 32 ? 4 : 0;
+}
+
+// Composite: n = n1 + B n2, k = k2 + A k1;  X[k2 + A k1] = sum_n1 w_B^{n1 k1} [ w_R^{n1 k2} sum_n2 x[n1 + B n2] w_A^{n2 k2} ]
+template <typename T, int R, bool INV> struct Dft {
+    static constexpr int A = split_a(R), B = R / A;
+    static_assert(A > 1 && A * B == R, "unsupported in-register radix");
+    static PF_HD void run(cx<T> *x) {
+        cx<T> y[R];  // y[n1 * A + k2]
+        static_for<B>([&](auto n1c) {
+            constexpr int n1 = decltype(n1c)::value;
+            cx<T> u[A];
+            static_for<A>([&](auto n2c) { constexpr int n2 = decltype(n2c)::value; u[n2] = x[n1 + B * n2]; });
+            Dft<T, A, INV>::run(u);
+            static_for<A>([&](auto k2c) {
+                constexpr int k2 = decltype(k2c)::value;
+                y[n1 * A + k2] = mul_tw<n1 * k2, R, INV>(u[k2]);
+            });
+        });
+        static_for<A>([&](auto k2c) {
+            constexpr int k2 = decltype(k2c)::value;
+            cx<T> g[B];
+            static_for<B>([&](auto n1c) { constexpr int n1 = decltype(n1c)::value; g[n1] = y[n1 * A + k2]; });
+            Dft<T, B, INV>::run(g);
+            static_for<B>([&](auto k1c) { constexpr int k1 = decltype(k1c)::value; x[k2 + A * k1] = g[k1]; });
+        });
+    }
+};
+
+template <typename T, int R, bool INV> PF_HD void dft(cx<T> *x) { Dft<T, R, INV>::run(x); }
+
+// Spread in registers: x[0..R/2) hold data, x[R/2..R) are zeros that are never
+// stored anywhere.  X[2j] = DFT_{R/2}(x)[j],  X[2j+1] = DFT_{R/2}(x[n] w_R^n)[j].
+template <typename T, int R, bool INV> PF_HD void dft_pruned_in(cx<T> *x) {
+    static_assert(R % 2 == 0, "pruned radix must be even");
+    constexpr int Hh = R / 2;
+    cx<T> e[Hh], o[Hh];
+    static_for<Hh>([&](auto nc) {
+        constexpr int n = decltype(nc)::value;
+        e[n] = x[n];
+        o[n] = mul_tw<n, R, INV>(x[n]);
+    });
+    Dft<T, Hh, INV>::run(e);
+    Dft<T, Hh, INV>::run(o);
+    static_for<Hh>([&](auto jc) {
+        constexpr int j = decltype(jc)::value;
+        x[2 * j] = e[j]; x[2 * j + 1] = o[j];
+    });
+}
+
+// Compactification in registers: all R inputs, only outputs n < R/2 are formed:
+// y[n] = DFT_{R/2}(x_even)[n] + w_R^{n} DFT_{R/2}(x_odd)[n].  Results land in x[0..R/2).
+template <typename T, int R, bool INV> PF_HD void dft_pruned_out(cx<T> *x) {
+    static_assert(R % 2 == 0, "pruned radix must be even");
+    constexpr int Hh = R / 2;
+    cx<T> e[Hh], o[Hh];
+    static_for<Hh>([&](auto jc) {
+        constexpr int j = decltype(jc)::value;
+        e[j] = x[2 * j]; o[j] = x[2 * j + 1];
+    });
+    Dft<T, Hh, INV>::run(e);
+    Dft<T, Hh, INV>::run(o);
+    static_for<Hh>([&](auto nc) {
+        constexpr int n = decltype(nc)::value;
+        x[n] = e[n] + mul_tw<n, R, INV>(o[n]);
+    });
+}
+
+}  // namespace pfft

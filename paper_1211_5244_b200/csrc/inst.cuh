@@ -1,0 +1,70 @@
+// inst.cuh -- instantiates and registers every pass kernel for ONE transform length.
+// An inst_S<len>.cu file defines PF_S, PF_RA, PF_RB, PF_TPP and includes this header.
+#pragma once
+
+#include "passes.cuh"
+#include "registry.hpp"
+
+namespace pfft {
+
+template <class G, bool PRUNED, int KIND>
+__global__ void __launch_bounds__(G::NT) pass_kernel(const PassParams prm) {
+    extern __shared__ __align__(16) unsigned char pf_smem[];
+    const int bid = blockIdx.x, nb = gridDim.x, tid = threadIdx.x;
+    if constexpr (KIND == KIND_F1) body_f1<G, PRUNED>(prm, bid, nb, tid, pf_smem);
+    else if constexpr (KIND == KIND_F2) body_f2<G, PRUNED>(prm, bid, nb, tid, pf_smem);
+    else if constexpr (KIND == KIND_F3) body_f3<G, PRUNED>(prm, bid, nb, tid, pf_smem);
+    else if constexpr (KIND == KIND_I2) body_i2<G, PRUNED>(prm, bid, nb, tid, pf_smem);
+    else body_i1<G, PRUNED>(prm, bid, nb, tid, pf_smem);
+}
+
+template <class G, bool PRUNED, int KIND>
+static void reg_one(int prec) {
+    KernelEntry e;
+    e.kind = KIND; e.S = G::S; e.pruned = PRUNED ? 1 : 0; e.lanes_p = G::LANES_P ? 1 : 0; e.prec = prec;
+    e.RA = G::RA; e.RB = G::RB;
+    e.P = G::P; e.TPP = G::TPP; e.V = G::V; e.NT = G::NT; e.smem_bytes = G::SMEM_BYTES;
+    e.func = reinterpret_cast<const void *>(&pass_kernel<G, PRUNED, KIND>);
+    kernel_registry().push_back(e);
+}
+
+// pencils per CTA: >= 128 threads per CTA and tile rows of >= 128 bytes
+template <typename T, int TPP>
+constexpr int pencils_per_cta() {
+    constexpr int by_threads = 128 / TPP > 0 ? 128 / TPP : 1;
+    constexpr int by_line = 128 / (int)sizeof(cx<T>);
+    return by_threads > by_line ? by_threads : by_line;
+}
+
+template <typename T, int S, int RA, int RB, int TPP>
+static void reg_length(int prec) {
+    constexpr int P = pencils_per_cta<T, TPP>();
+    using GP = Geo<T, S, RA, RB, TPP, P, true>;
+    using GC = Geo<T, S, RA, RB, TPP, P, false>;
+    reg_one<GP, true, KIND_F1>(prec);  reg_one<GP, false, KIND_F1>(prec);
+    reg_one<GP, true, KIND_I1>(prec);  reg_one<GP, false, KIND_I1>(prec);
+    reg_one<GP, true, KIND_F2>(prec);  reg_one<GP, false, KIND_F2>(prec);
+    reg_one<GP, true, KIND_I2>(prec);  reg_one<GP, false, KIND_I2>(prec);
+    reg_one<GP, true, KIND_F3>(prec);  reg_one<GP, false, KIND_F3>(prec);
+    reg_one<GC, true, KIND_F2>(prec);  reg_one<GC, false, KIND_F2>(prec);
+    reg_one<GC, true, KIND_I2>(prec);  reg_one<GC, false, KIND_I2>(prec);
+    reg_one<GC, true, KIND_F3>(prec);  reg_one<GC, false, KIND_F3>(prec);
+}
+
+}  // namespace pfft
+
+#if defined(PF_S)
+namespace {
+struct PfRegistrar {
+    PfRegistrar() {
+#if !defined(PF_ONLY_F32)
+        pfft::reg_length<double, PF_S, PF_RA, PF_RB, PF_TPP>(0);
+#endif
+#if !defined(PF_ONLY_F64)
+        pfft::reg_length<float, PF_S, PF_RA, PF_RB, PF_TPP>(1);
+#endif
+    }
+};
+static PfRegistrar pf_registrar_instance;
+}  // namespace
+#endif

@@ -1,0 +1,28 @@
+// registry.hpp -- table of compiled pass kernels.  Each inst_*.cu translation unit registers the
+// instantiations it holds; api.cu looks kernels up by (kind, S, pruned, lanes_p, precision).
+#pragma once
+
+#include <cstddef>
+#include <vector>
+
+namespace pfft {
+
+enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4 };
+
+struct KernelEntry {
+    int kind;      // PassKind
+    int S;         // transform length
+    int pruned;    // 1: zero-padded axis (spread / compactification fused), 0: periodic axis
+    int lanes_p;   // 1: lanes along the pencil index (strided pencils), 0: lanes along the transform
+    int prec;      // 0 fp64, 1 fp32
+    int RA, RB;    // S = RA * RB: radix of the first / second register pass
+    int P, TPP, V, NT;
+    size_t smem_bytes;
+    const void *func;  // __global__ void (*)(PassParams)
+};
+
+std::vector<KernelEntry> &kernel_registry();
+const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int prec);
+bool length_supported(int S);
+
+}  // namespace pfft

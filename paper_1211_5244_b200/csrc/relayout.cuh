@@ -1,0 +1,44 @@
+// relayout.cuh -- where each slot of the internal K^F copy comes from ("a transposition
+// of the associated kernel ... carried out only once").
+// Internal order: kint[(tile*V + r)*NT + tid] -- exactly the order pass F3 reads it in, so the
+// multiply of Eq. 3 streams K^F with perfectly coalesced loads and no index arithmetic.
+#pragma once
+
+#include "fft_core.cuh"
+
+namespace pfft {
+
+struct RelayoutParams {
+    int RA, RB, TPP, P, V, NT, lanes_p;
+    int tiles_per_g, n_p;
+    int a_axis, c_axis;
+    long long ext2y;
+    int sx, sy, sz;
+    long long total;
+    double scale;  // 1/(S_x S_y S_z)
+};
+
+template <typename T>
+PF_HD T relayout_value(const T *kuser, const RelayoutParams &q, long long idx) {
+    const int tid = (int)(idx % q.NT);
+    const int r = (int)((idx / q.NT) % q.V);
+    const long long tile = idx / ((long long)q.NT * q.V);
+    int t, p;
+    if (q.lanes_p) { p = tid % q.P; t = tid / q.P; } else { t = tid % q.TPP; p = tid / q.TPP; }
+    const long long g = tile / q.tiles_per_g;
+    const long long pp = (tile % q.tiles_per_g) * q.P + p;
+    if (pp >= q.n_p) return (T)0;
+    const int i = r / q.RB, k1 = r % q.RB;
+    const int kc = (t + q.TPP * i) + q.RA * k1;  // layout B of passes.cuh: k = k2 + RA*k1
+    long long f[3];
+    if (!q.lanes_p) { f[0] = kc; f[1] = pp % q.ext2y; f[2] = pp / q.ext2y; }
+    else { f[0] = pp; f[q.c_axis] = kc; f[q.a_axis] = g; }
+    long long kx = f[0], ky = f[1], kz = f[2];
+    const int hx = q.sx / 2 + 1;
+    if (kx > q.sx / 2) {  // K^F(-k) = K^F(k): the half the caller did not pass
+        kx = q.sx - kx; ky = (q.sy - ky) % q.sy; kz = (q.sz - kz) % q.sz;
+    }
+    return (T)((double)kuser[(kz * q.sy + ky) * hx + kx] * q.scale);
+}
+
+}  // namespace pfft

@@ -131,6 +131,15 @@ POISSON_API int poisson_debug_workspace(const poisson_plan *plan, int which, voi
 POISSON_API int poisson_debug_run_passes(poisson_plan *plan, const void *rho_dev, void *V_dev, void *stream,
                              int first_pass, int last_pass);
 
+/* Per-pass device timing for the roofline report (bench.py): identical to poisson_solve, but a CUDA
+ * event is recorded on `stream` before the first pass and after every pass (6 events per solve,
+ * from a pool the plan owns; at most 512 profiled solves between two reads).
+ * poisson_profile_read synchronises on the recorded events, ADDS each pass's elapsed milliseconds
+ * over all solves profiled since the last read into ms_sum[5], stores their number in *n_solves,
+ * and resets the pool.  Errors: EINVAL, ENOKERNEL, ECUDA, ENOMEM (pool exhausted). */
+POISSON_API int poisson_solve_profiled(poisson_plan *plan, const void *rho_dev, void *V_dev, void *stream);
+POISSON_API int poisson_profile_read(poisson_plan *plan, double ms_sum[5] /* host, out */, int *n_solves /* host, out */);
+
 /* Number of kernel launches one poisson_solve enqueues (bench.py's gpu_launches). */
 POISSON_API int poisson_plan_launches_per_solve(const poisson_plan *plan);
 

@@ -23,7 +23,7 @@ PASS_NAMES = ("F1", "F2", "F3", "I2", "I1")
 EXPORTED_SYMBOLS = (
     "poisson_plan_describe", "poisson_plan_create", "poisson_plan_kernel_dims", "poisson_plan_get_info",
     "poisson_set_kernel", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
-    "poisson_debug_run_passes", "poisson_plan_launches_per_solve", "poisson_plan_workspace_bytes",
+    "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_plan_workspace_bytes",
     "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch",
 )
 
@@ -82,6 +82,8 @@ def load_library():
     lib.poisson_solve_host.argtypes = [vp, vp, vp, vp]
     lib.poisson_debug_workspace.argtypes = [vp, i, ctypes.POINTER(vp), ll * 3]
     lib.poisson_debug_run_passes.argtypes = [vp, vp, vp, vp, i, i]
+    lib.poisson_solve_profiled.argtypes = [vp, vp, vp, vp]
+    lib.poisson_profile_read.argtypes = [vp, ctypes.c_double * 5, ctypes.POINTER(i)]
     lib.poisson_plan_launches_per_solve.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.restype = ctypes.c_size_t
@@ -186,6 +188,18 @@ class PoissonPlan:
         assert rho_host.dtype == self._dtype() and V_host.dtype == self._dtype()
         poisson_solve_host(self._h, rho_host.data_ptr(), V_host.data_ptr(), self._stream(stream))
         return V_host
+
+    def solve_profiled(self, rho, V, stream=None):
+        _check(load_library().poisson_solve_profiled(self._h, rho.data_ptr(), V.data_ptr(), self._stream(stream)),
+               "poisson_solve_profiled")
+        return V
+
+    def profile_read(self):
+        """(per-pass milliseconds summed over the profiled solves, number of solves); resets the pool."""
+        ms = (ctypes.c_double * 5)()
+        n = ctypes.c_int()
+        _check(load_library().poisson_profile_read(self._h, ms, ctypes.byref(n)), "poisson_profile_read")
+        return list(ms), n.value
 
     def launches_per_solve(self) -> int:
         return load_library().poisson_plan_launches_per_solve(self._h)

@@ -65,6 +65,8 @@ struct poisson_plan {
     long long kint_elems;
     size_t workspace_bytes;
     bool kernel_set;
+    std::vector<cudaEvent_t> *prof_events;  // 6 per profiled solve
+    int prof_count;
 };
 
 static void fill_twiddles(std::vector<unsigned char> &buf, int S, int prec) {
@@ -90,6 +92,10 @@ static void free_plan(poisson_plan *pl) {
     cudaFree(pl->a1); cudaFree(pl->a2); cudaFree(pl->kint);
     for (int q = 0; q < 3; ++q) cudaFree(pl->tw[q]);
     cudaFree(pl->rho_stage); cudaFree(pl->v_stage);
+    if (pl->prof_events) {
+        for (cudaEvent_t e : *pl->prof_events) cudaEventDestroy(e);
+        delete pl->prof_events;
+    }
     delete pl;
 }
 
@@ -241,8 +247,10 @@ int poisson_set_kernel(poisson_plan *pl, const void *K_f_dev, void *stream) {
     return POISSON_OK;
 }
 
-static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t st, int first, int last) {
+static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t st, int first, int last,
+                      cudaEvent_t *ev = nullptr) {
     const PlanDesc &d = pl->d;
+    if (ev) PF_CUDA(cudaEventRecord(ev[0], st));
     for (int q = first; q <= last; ++q) {
         const PassDesc &ps = d.pass[q];
         const KernelEntry *e = pl->k[q];
@@ -261,6 +269,7 @@ static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t s
         prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q];
         void *args[] = {&prm};
         PF_CUDA(cudaLaunchKernel(e->func, dim3(pl->grid[q]), dim3(e->NT), args, e->smem_bytes, st));
+        if (ev) PF_CUDA(cudaEventRecord(ev[q + 1], st));
     }
     return POISSON_OK;
 }
@@ -270,6 +279,42 @@ int poisson_solve(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stre
     if (reinterpret_cast<size_t>(rho_dev) % 16 || reinterpret_cast<size_t>(V_dev) % 16) return POISSON_EINVAL;
     if (!pl->kernel_set) return POISSON_ENOKERNEL;
     return run_passes(pl, rho_dev, V_dev, reinterpret_cast<cudaStream_t>(stream), 0, 4);
+}
+
+int poisson_solve_profiled(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stream) {
+    if (!pl || !rho_dev || !V_dev) return POISSON_EINVAL;
+    if (reinterpret_cast<size_t>(rho_dev) % 16 || reinterpret_cast<size_t>(V_dev) % 16) return POISSON_EINVAL;
+    if (!pl->kernel_set) return POISSON_ENOKERNEL;
+    constexpr int kMaxProfiled = 512;
+    if (pl->prof_count >= kMaxProfiled) return POISSON_ENOMEM;
+    if (!pl->prof_events) pl->prof_events = new (std::nothrow) std::vector<cudaEvent_t>();
+    if (!pl->prof_events) return POISSON_ENOMEM;
+    while ((int)pl->prof_events->size() < 6 * (pl->prof_count + 1)) {
+        cudaEvent_t e;
+        PF_CUDA(cudaEventCreate(&e));
+        pl->prof_events->push_back(e);
+    }
+    cudaEvent_t *ev = pl->prof_events->data() + 6 * pl->prof_count;
+    const int rc = run_passes(pl, rho_dev, V_dev, reinterpret_cast<cudaStream_t>(stream), 0, 4, ev);
+    if (rc == POISSON_OK) pl->prof_count++;
+    return rc;
+}
+
+int poisson_profile_read(poisson_plan *pl, double ms_sum[5], int *n_solves) {
+    if (!pl || !ms_sum || !n_solves) return POISSON_EINVAL;
+    for (int q = 0; q < 5; ++q) ms_sum[q] = 0.0;
+    *n_solves = pl->prof_count;
+    for (int i = 0; i < pl->prof_count; ++i) {
+        cudaEvent_t *ev = pl->prof_events->data() + 6 * i;
+        PF_CUDA(cudaEventSynchronize(ev[5]));
+        for (int q = 0; q < 5; ++q) {
+            float ms = 0.f;
+            PF_CUDA(cudaEventElapsedTime(&ms, ev[q], ev[q + 1]));
+            ms_sum[q] += (double)ms;
+        }
+    }
+    pl->prof_count = 0;
+    return POISSON_OK;
 }
 
 int poisson_debug_run_passes(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stream, int first, int last) {

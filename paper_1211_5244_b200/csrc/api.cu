@@ -3,6 +3,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -21,10 +22,20 @@ std::vector<KernelEntry> &kernel_registry() {
     return reg;
 }
 
-const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int prec) {
+// variant < 0: the POISSON_VARIANT environment variable (tuning experiments), else the default 0.
+// A requested variant that was not compiled for this length falls back to variant 0.
+const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int prec, int variant) {
+    if (variant < 0) {
+        const char *env = std::getenv("POISSON_VARIANT");
+        variant = env ? std::atoi(env) : 0;
+    }
+    const KernelEntry *fallback = nullptr;
     for (const KernelEntry &e : kernel_registry())
-        if (e.kind == kind && e.S == S && e.pruned == pruned && e.lanes_p == lanes_p && e.prec == prec) return &e;
-    return nullptr;
+        if (e.kind == kind && e.S == S && e.pruned == pruned && e.lanes_p == lanes_p && e.prec == prec) {
+            if (e.variant == variant) return &e;
+            if (e.variant == 0) fallback = &e;
+        }
+    return fallback;
 }
 
 static thread_local std::string g_last_error;
@@ -65,6 +76,7 @@ struct poisson_plan {
     long long kint_elems;
     size_t workspace_bytes;
     bool kernel_set;
+    bool use_pdl;
     std::vector<cudaEvent_t> *prof_events;  // 6 per profiled solve
     int prof_count;
 };
@@ -158,6 +170,9 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     std::memset(static_cast<void *>(pl), 0, sizeof(*pl));
     pl->d = d; pl->h = h; pl->device = dev; pl->num_sms = prop.multiProcessorCount;
     pl->elem_real = precision == POISSON_FP64 ? 8 : 4;
+    // Programmatic dependent launch is opt-in (POISSON_PDL=1): measured on B200 it shortens back-to-back
+    // launches of one pass but lengthens the 5-pass solve ("What was tried").
+    { const char *env = std::getenv("POISSON_PDL"); pl->use_pdl = env && env[0] == '1'; }
 
     for (int q = 0; q < 5; ++q) {
         const PassDesc &ps = d.pass[q];
@@ -268,7 +283,14 @@ static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t s
         prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;
         prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q];
         void *args[] = {&prm};
-        PF_CUDA(cudaLaunchKernel(e->func, dim3(pl->grid[q]), dim3(e->NT), args, e->smem_bytes, st));
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(pl->grid[q]); cfg.blockDim = dim3(e->NT);
+        cfg.dynamicSmemBytes = e->smem_bytes; cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // PDL: prologue overlaps the previous pass's tail
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = pl->use_pdl ? 1 : 0;
+        PF_CUDA(cudaLaunchKernelExC(&cfg, e->func, args));
         if (ev) PF_CUDA(cudaEventRecord(ev[q + 1], st));
     }
     return POISSON_OK;

@@ -44,6 +44,61 @@ template <typename T> PF_HD cx<T> mul_conj(cx<T> a, cx<T> w) {  // a * conj(w)
 template <typename T> PF_HD cx<T> mul_mi(cx<T> a) { return mk<T>(a.im, -a.re); }
 template <typename T> PF_HD cx<T> mul_pi(cx<T> a) { return mk<T>(-a.im, a.re); }
 
+// ------------------------------------------------------------------ streaming global accesses
+// Data that is touched once per solve (rho, K^F, V, and the last read of an intermediate) is
+// loaded / stored with the evict-first policy (ld.global.cs / st.global.cs) so that it does not
+// push the intermediates A1 / A2, which ARE reused by the next pass, out of the 126 MB L2.
+PF_HD cx<double> ld_stream(const cx<double> *p) {
+#if defined(__CUDA_ARCH__)
+    const double2 v = __ldcs(reinterpret_cast<const double2 *>(p));
+    return mk<double>(v.x, v.y);
+#else
+    return *p;
+#endif
+}
+PF_HD cx<float> ld_stream(const cx<float> *p) {
+#if defined(__CUDA_ARCH__)
+    const float2 v = __ldcs(reinterpret_cast<const float2 *>(p));
+    return mk<float>(v.x, v.y);
+#else
+    return *p;
+#endif
+}
+PF_HD double ld_stream(const double *p) {
+#if defined(__CUDA_ARCH__)
+    return __ldcs(p);
+#else
+    return *p;
+#endif
+}
+PF_HD float ld_stream(const float *p) {
+#if defined(__CUDA_ARCH__)
+    return __ldcs(p);
+#else
+    return *p;
+#endif
+}
+PF_HD void st_stream(cx<double> *p, cx<double> v) {
+#if defined(__CUDA_ARCH__)
+    __stcs(reinterpret_cast<double2 *>(p), make_double2(v.re, v.im));
+#else
+    *p = v;
+#endif
+}
+PF_HD void st_stream(cx<float> *p, cx<float> v) {
+#if defined(__CUDA_ARCH__)
+    __stcs(reinterpret_cast<float2 *>(p), make_float2(v.re, v.im));
+#else
+    *p = v;
+#endif
+}
+template <bool STREAM, typename E> PF_HD E ld_hint(const E *p) {
+    if constexpr (STREAM) return ld_stream(p); else return *p;
+}
+template <bool STREAM, typename E> PF_HD void st_hint(E *p, E v) {
+    if constexpr (STREAM) st_stream(p, v); else *p = v;
+}
+
 // ------------------------------------------------------------------ compile-time loops
 template <int... Is, typename F>
 PF_HD void static_for_impl(std::integer_sequence<int, Is...>, F &&f) {

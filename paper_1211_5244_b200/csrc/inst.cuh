@@ -1,5 +1,6 @@
 // inst.cuh -- instantiates and registers every pass kernel for ONE transform length.
-// An inst_S<len>.cu file defines PF_S, PF_RA, PF_RB, PF_TPP and includes this header.
+// An inst_S<len>_<prec>.cu file defines PF_S, PF_RA, PF_RB, PF_TPP (and optionally the tuning knobs
+// PF_NBUF, PF_TWS, PF_MINB, PF_PREF, PF_EXTRA_VARIANTS) and includes this header.
 #pragma once
 
 #include "passes.cuh"
@@ -8,7 +9,7 @@
 namespace pfft {
 
 template <class G, bool PRUNED, int KIND>
-__global__ void __launch_bounds__(G::NT) pass_kernel(const PassParams prm) {
+__global__ void __launch_bounds__(G::NT, G::MINB) pass_kernel(const PassParams prm) {
     extern __shared__ __align__(16) unsigned char pf_smem[];
     const int bid = blockIdx.x, nb = gridDim.x, tid = threadIdx.x;
     if constexpr (KIND == KIND_F1) body_f1<G, PRUNED>(prm, bid, nb, tid, pf_smem);
@@ -19,9 +20,10 @@ __global__ void __launch_bounds__(G::NT) pass_kernel(const PassParams prm) {
 }
 
 template <class G, bool PRUNED, int KIND>
-static void reg_one(int prec) {
+static void reg_one(int prec, int variant) {
     KernelEntry e;
     e.kind = KIND; e.S = G::S; e.pruned = PRUNED ? 1 : 0; e.lanes_p = G::LANES_P ? 1 : 0; e.prec = prec;
+    e.variant = variant; e.nbuf = G::NBUF; e.tws = G::TWS ? 1 : 0; e.minb = G::MINB; e.pref = G::PREF;
     e.RA = G::RA; e.RB = G::RB;
     e.P = G::P; e.TPP = G::TPP; e.V = G::V; e.NT = G::NT; e.smem_bytes = G::SMEM_BYTES;
     e.func = reinterpret_cast<const void *>(&pass_kernel<G, PRUNED, KIND>);
@@ -36,32 +38,54 @@ constexpr int pencils_per_cta() {
     return by_threads > by_line ? by_threads : by_line;
 }
 
-template <typename T, int S, int RA, int RB, int TPP>
-static void reg_length(int prec) {
+template <typename T, int S, int RA, int RB, int TPP, int NBUF, bool TWS, int MINB, int PREF, bool KLATE>
+static void reg_length(int prec, int variant) {
     constexpr int P = pencils_per_cta<T, TPP>();
-    using GP = Geo<T, S, RA, RB, TPP, P, true>;
-    using GC = Geo<T, S, RA, RB, TPP, P, false>;
-    reg_one<GP, true, KIND_F1>(prec);  reg_one<GP, false, KIND_F1>(prec);
-    reg_one<GP, true, KIND_I1>(prec);  reg_one<GP, false, KIND_I1>(prec);
-    reg_one<GP, true, KIND_F2>(prec);  reg_one<GP, false, KIND_F2>(prec);
-    reg_one<GP, true, KIND_I2>(prec);  reg_one<GP, false, KIND_I2>(prec);
-    reg_one<GP, true, KIND_F3>(prec);  reg_one<GP, false, KIND_F3>(prec);
-    reg_one<GC, true, KIND_F2>(prec);  reg_one<GC, false, KIND_F2>(prec);
-    reg_one<GC, true, KIND_I2>(prec);  reg_one<GC, false, KIND_I2>(prec);
-    reg_one<GC, true, KIND_F3>(prec);  reg_one<GC, false, KIND_F3>(prec);
+    using GP = Geo<T, S, RA, RB, TPP, P, true, NBUF, TWS, MINB, PREF, KLATE>;
+    using GC = Geo<T, S, RA, RB, TPP, P, false, NBUF, TWS, MINB, PREF, KLATE>;
+    reg_one<GP, true, KIND_F1>(prec, variant);  reg_one<GP, false, KIND_F1>(prec, variant);
+    reg_one<GP, true, KIND_I1>(prec, variant);  reg_one<GP, false, KIND_I1>(prec, variant);
+    reg_one<GP, true, KIND_F2>(prec, variant);  reg_one<GP, false, KIND_F2>(prec, variant);
+    reg_one<GP, true, KIND_I2>(prec, variant);  reg_one<GP, false, KIND_I2>(prec, variant);
+    reg_one<GP, true, KIND_F3>(prec, variant);  reg_one<GP, false, KIND_F3>(prec, variant);
+    reg_one<GC, true, KIND_F2>(prec, variant);  reg_one<GC, false, KIND_F2>(prec, variant);
+    reg_one<GC, true, KIND_I2>(prec, variant);  reg_one<GC, false, KIND_I2>(prec, variant);
+    reg_one<GC, true, KIND_F3>(prec, variant);  reg_one<GC, false, KIND_F3>(prec, variant);
 }
 
 }  // namespace pfft
 
 #if defined(PF_S)
+#ifndef PF_NBUF
+#define PF_NBUF 1
+#endif
+#ifndef PF_TWS
+#define PF_TWS true
+#endif
+#ifndef PF_MINB
+#define PF_MINB 0
+#endif
+#ifndef PF_PREF
+#define PF_PREF 0
+#endif
+#ifndef PF_KLATE
+#define PF_KLATE true
+#endif
+#if defined(PF_ONLY_F64)
+#define PF_T double
+#define PF_PREC 0
+#else
+#define PF_T float
+#define PF_PREC 1
+#endif
 namespace {
 struct PfRegistrar {
     PfRegistrar() {
-#if !defined(PF_ONLY_F32)
-        pfft::reg_length<double, PF_S, PF_RA, PF_RB, PF_TPP>(0);
-#endif
-#if !defined(PF_ONLY_F64)
-        pfft::reg_length<float, PF_S, PF_RA, PF_RB, PF_TPP>(1);
+        pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, PF_NBUF, PF_TWS, PF_MINB, PF_PREF, PF_KLATE>(PF_PREC, 0);
+#if defined(PF_EXTRA_VARIANTS)
+#define PF_VARIANT(ID, NBUF, TWS, MINB, PREF, KLATE) pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, NBUF, TWS, MINB, PREF, KLATE>(PF_PREC, ID);
+        PF_EXTRA_VARIANTS
+#undef PF_VARIANT
 #endif
     }
 };

@@ -4,4 +4,6 @@
 #define PF_RB 16
 #define PF_TPP 16
 #define PF_ONLY_F64
+// tuning experiments: PF_VARIANT(id, NBUF, TWS, MINB, PREF, KLATE)
+#define PF_EXTRA_VARIANTS PF_VARIANT(1, 2, false, 1, 0, false) PF_VARIANT(3, 1, true, 5, 0, true)
 #include "inst.cuh"

@@ -4,4 +4,6 @@
 #define PF_RB 16
 #define PF_TPP 16
 #define PF_ONLY_F64
+// 32 complex fp64 values per thread: needs the full register file, 2 CTAs per SM
+#define PF_MINB 2
 #include "inst.cuh"

@@ -30,27 +30,48 @@ namespace pfft {
 
 #if defined(__CUDA_ARCH__)
 PF_HD void cta_sync() { __syncthreads(); }
+PF_HD void warp_sync() { __syncwarp(); }
 #else
 void host_cta_sync();  // provided by the development-only host harness
 PF_HD void cta_sync() { host_cta_sync(); }
+PF_HD void warp_sync() { host_cta_sync(); }
 #endif
 
 // ------------------------------------------------------------------ geometry
-template <typename T_, int S_, int RA_, int RB_, int TPP_, int P_, bool LANES_P_>
+// NBUF_   : exchange buffers (2 = one barrier per exchange, 1 = half the shared memory, one more barrier)
+// TWS_    : twiddles w_S^{n1 k2} read from a shared-memory table (true) or held in registers (false)
+// MINB_   : __launch_bounds__ minimum resident CTAs per SM (register cap); 0 = automatic
+// PREF_   : 1 = the next tile's inputs are loaded into registers while the current tile is transformed
+// KLATE_  : pass F3 loads its K^F values right before the multiply (fewer live registers) instead of
+//           at the top of the tile
+template <typename T_, int S_, int RA_, int RB_, int TPP_, int P_, bool LANES_P_, int NBUF_ = 2, bool TWS_ = true,
+          int MINB_ = 0, int PREF_ = 0, bool KLATE_ = false>
 struct Geo {
     using T = T_;
     static constexpr int S = S_, RA = RA_, RB = RB_, TPP = TPP_, P = P_;
     static constexpr bool LANES_P = LANES_P_;
+    static constexpr int NBUF = NBUF_, PREF = PREF_;
+    static constexpr bool KLATE = KLATE_;
+    // lanes along the transform: the TPP threads of a pencil sit in one warp, so the exchange is
+    // warp-private and a warp-level barrier is enough
+    static constexpr bool WARP_LOCAL = !LANES_P_ && (32 % TPP_ == 0);
+    static PF_HD void xsync() { if (WARP_LOCAL) warp_sync(); else cta_sync(); }
+    static constexpr bool TWS = TWS_ && RB_ > 1;
+    static_assert(NBUF == 1 || NBUF == 2, "one or two exchange buffers");
     static_assert(RA * RB == S, "S = RA * RB");
     static_assert(RA % TPP == 0 && RB % TPP == 0, "TPP must divide both radices");
     static constexpr int CA = RB / TPP;  // n1 columns per thread (layout A)
     static constexpr int CB = RA / TPP;  // k2 columns per thread (layout B)
     static constexpr int V = S / TPP;    // complex values per thread
     static constexpr int NT = TPP * P;   // threads per CTA
+    // MINB_ = 0: aim at 512 resident threads per SM (a 128-register budget per thread)
+    static constexpr int MINB = MINB_ > 0 ? MINB_ : (512 / NT > 0 ? 512 / NT : 1);
     static constexpr int RBP = (RB % 2 == 0 && RB > 1) ? RB + 1 : RB;  // odd pitch: conflict-free both ways
     static constexpr int XPITCH = RA * RBP;
     static constexpr int XELEMS = LANES_P ? S * P : P * XPITCH;        // one exchange buffer
-    static constexpr size_t SMEM_BYTES = 2 * (size_t)XELEMS * sizeof(cx<T_>);
+    static constexpr int TW_TABLES = !TWS ? 0 : (RA == RB ? 1 : 2);            // [k2][n1] and [n1][k2]
+    static constexpr int TW_ELEMS = TW_TABLES * S;
+    static constexpr size_t SMEM_BYTES = ((size_t)NBUF * XELEMS + TW_ELEMS) * sizeof(cx<T_>);
 
     static PF_HD void split(int tid, int &t, int &p) {
         if (LANES_P) { p = tid % P; t = tid / P; } else { t = tid % TPP; p = tid / TPP; }
@@ -76,31 +97,75 @@ struct PassParams {
     int n_tiles;       // n_g * tiles_per_g
 };
 
-// ------------------------------------------------------------------ twiddles kept in registers
+// ------------------------------------------------------------------ programmatic dependent launch
+// Every pass is launched with programmatic stream serialisation: its CTAs may become resident while
+// the previous pass drains, run their prologue (twiddle tables: constant data), and only then wait
+// for the previous pass's memory to be complete and visible.
+PF_HD void pdl_launch_dependents() {
+#if defined(__CUDA_ARCH__)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
+}
+PF_HD void pdl_wait_prior_grid() {
+#if defined(__CUDA_ARCH__)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+}
+
+// ------------------------------------------------------------------ inter-pass twiddles w_S^{n1 k2}
+// TWS: two shared-memory tables, [k2][n1] for the forward pass (thread owns n1) and [n1][k2] for the
+// inverse pass (thread owns k2), so that consecutive lanes read consecutive entries; one table when
+// RA == RB (the table is symmetric).  Otherwise: per-thread register copies.
 template <class G>
 struct Twiddles {
     using T = typename G::T;
-    static constexpr int NA = G::CA * (G::RA - 1), NB = G::CB * (G::RB - 1);
-    cx<T> a[NA > 0 ? NA : 1];  // w^{n1 k2}, n1 = t + TPP i, k2 = 1..RA-1   (forward pass 1)
-    cx<T> b[NB > 0 ? NB : 1];  // w^{n1 k2}, k2 = t + TPP i', n1 = 1..RB-1  (inverse pass 1, conjugated on use)
+    static constexpr int NA = G::TWS ? 1 : (G::CA * (G::RA - 1) > 0 ? G::CA * (G::RA - 1) : 1);
+    static constexpr int NB = G::TWS ? 1 : (G::CB * (G::RB - 1) > 0 ? G::CB * (G::RB - 1) : 1);
+    cx<T> a[NA], b[NB];
+    const cx<T> *ta, *tb;
+
+    // tab: S entries exp(-2 pi i m / S) in global memory; smem_tw: G::TW_ELEMS entries of shared memory
     template <bool NEED_A, bool NEED_B>
-    PF_HD void load(const cx<T> *tab, int t) {
-        if constexpr (NEED_A && G::RB > 1)
-            static_for<G::CA>([&](auto ic) {
-                constexpr int i = decltype(ic)::value;
-                static_for<G::RA - 1>([&](auto kc) {
-                    constexpr int k2 = decltype(kc)::value + 1;
-                    a[i * (G::RA - 1) + k2 - 1] = tab[((t + G::TPP * i) * k2) % G::S];
-                });
-            });
-        if constexpr (NEED_B && G::RB > 1)
-            static_for<G::CB>([&](auto ic) {
-                constexpr int i = decltype(ic)::value;
-                static_for<G::RB - 1>([&](auto nc) {
-                    constexpr int n1 = decltype(nc)::value + 1;
-                    b[i * (G::RB - 1) + n1 - 1] = tab[((t + G::TPP * i) * n1) % G::S];
-                });
-            });
+    PF_HD void init(const cx<T> *tab, cx<T> *smem_tw, int tid, int t) {
+        ta = smem_tw; tb = smem_tw + (G::TW_TABLES == 2 ? G::S : 0);
+        if constexpr (G::RB > 1) {
+            if constexpr (G::TWS) {
+                for (int idx = tid; idx < G::S; idx += G::NT) {
+                    const cx<T> w = tab[((idx / G::RB) * (idx % G::RB)) % G::S];     // [k2][n1]
+                    smem_tw[idx] = w;
+                    if constexpr (G::TW_TABLES == 2)
+                        smem_tw[G::S + (idx % G::RB) * G::RA + idx / G::RB] = w;       // [n1][k2]
+                }
+                cta_sync();
+            } else {
+                if constexpr (NEED_A)
+                    static_for<G::CA>([&](auto ic) {
+                        constexpr int i = decltype(ic)::value;
+                        static_for<G::RA - 1>([&](auto kc) {
+                            constexpr int k2 = decltype(kc)::value + 1;
+                            a[i * (G::RA - 1) + k2 - 1] = tab[((t + G::TPP * i) * k2) % G::S];
+                        });
+                    });
+                if constexpr (NEED_B)
+                    static_for<G::CB>([&](auto ic) {
+                        constexpr int i = decltype(ic)::value;
+                        static_for<G::RB - 1>([&](auto nc) {
+                            constexpr int n1 = decltype(nc)::value + 1;
+                            b[i * (G::RB - 1) + n1 - 1] = tab[((t + G::TPP * i) * n1) % G::S];
+                        });
+                    });
+            }
+        }
+    }
+    // forward: thread owns n1 = t + TPP*I, needs w^{n1 K2}
+    template <int I, int K2> PF_HD cx<T> fwd(int t) const {
+        if constexpr (G::TWS) return ta[K2 * G::RB + t + G::TPP * I];
+        else return a[I * (G::RA - 1) + K2 - 1];
+    }
+    // inverse: thread owns k2 = t + TPP*I, needs w^{N1 k2}
+    template <int I, int N1> PF_HD cx<T> inv(int t) const {
+        if constexpr (G::TWS) return tb[N1 * G::RA + t + G::TPP * I];
+        else return b[I * (G::RB - 1) + N1 - 1];
     }
 };
 
@@ -119,12 +184,12 @@ PF_HD void fwd_AtoB(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::
             xb[G::xidx(p, n1, 0)] = u[0];
             static_for<RA - 1>([&](auto kc) {
                 constexpr int k2 = decltype(kc)::value + 1;
-                xb[G::xidx(p, n1, k2)] = u[k2] * tw.a[i * (RA - 1) + k2 - 1];
+                xb[G::xidx(p, n1, k2)] = u[k2] * tw.template fwd<i, k2>(t);
             });
         }
     });
     if constexpr (RB > 1) {
-        cta_sync();
+        G::xsync();
         static_for<G::CB>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             const int k2 = t + G::TPP * i;
@@ -149,10 +214,10 @@ PF_HD void inv_BtoA(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::
             xb[G::xidx(p, 0, k2)] = g[0];
             static_for<RB - 1>([&](auto nc) {
                 constexpr int n1 = decltype(nc)::value + 1;
-                xb[G::xidx(p, n1, k2)] = mul_conj(g[n1], tw.b[i * (RB - 1) + n1 - 1]);
+                xb[G::xidx(p, n1, k2)] = mul_conj(g[n1], tw.template inv<i, n1>(t));
             });
         });
-        cta_sync();
+        G::xsync();
     }
     static_for<G::CA>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
@@ -164,6 +229,21 @@ PF_HD void inv_BtoA(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::
         if constexpr (PRUNED) dft_pruned_out<T, RA, true>(u); else dft<T, RA, true>(u);
     });
 }
+
+// Exchange-buffer bookkeeping.  NBUF = 2: buffers alternate, the barrier inside each transform is
+// enough.  NBUF = 1: one more barrier before the buffer is written again.
+template <class G>
+struct XBufs {
+    using T = typename G::T;
+    cx<T> *base;
+    int which;
+    bool dirty;
+    PF_HD explicit XBufs(cx<T> *b) : base(b), which(0), dirty(false) {}
+    PF_HD cx<T> *next() {
+        if constexpr (G::NBUF == 2) { cx<T> *r = base + which * G::XELEMS; which ^= 1; return r; }
+        else { if (dirty) G::xsync(); dirty = true; return base; }
+    }
+};
 
 // ------------------------------------------------------------------ global <-> register adapters
 // layout A element (i, n2) <-> n = (t + TPP i) + RB n2 ; only n2 < NA2 is touched (NA2 = RA/2 when pruned)
@@ -180,7 +260,7 @@ PF_HD void load_A(cx<typename G::T> *v, const E *src, long long ns, int t, bool 
         });
     });
 }
-template <class G, bool PRUNED>
+template <class G, bool PRUNED, bool STREAM = false>
 PF_HD void store_A(const cx<typename G::T> *v, cx<typename G::T> *dst, long long ns, int t, bool valid) {
     constexpr int NA2 = PRUNED ? G::RA / 2 : G::RA;
     if (!valid) return;
@@ -189,12 +269,12 @@ PF_HD void store_A(const cx<typename G::T> *v, cx<typename G::T> *dst, long long
         static_for<NA2>([&](auto nc) {
             constexpr int n2 = decltype(nc)::value;
             const int n = (t + G::TPP * i) + G::RB * n2;
-            dst[n * ns] = v[i * G::RA + n2];
+            st_hint<STREAM>(dst + n * ns, v[i * G::RA + n2]);
         });
     });
 }
 // layout B element (i', k1) <-> k = (t + TPP i') + RA k1
-template <class G>
+template <class G, bool STREAM = false>
 PF_HD void load_B(cx<typename G::T> *v, const cx<typename G::T> *src, long long ns, int t, bool valid) {
     using T = typename G::T;
     static_for<G::CB>([&](auto ic) {
@@ -202,7 +282,7 @@ PF_HD void load_B(cx<typename G::T> *v, const cx<typename G::T> *src, long long 
         static_for<G::RB>([&](auto kc) {
             constexpr int k1 = decltype(kc)::value;
             const int k = (t + G::TPP * i) + G::RA * k1;
-            v[i * G::RB + k1] = valid ? src[k * ns] : mk<T>((T)0, (T)0);
+            v[i * G::RB + k1] = valid ? ld_hint<STREAM>(src + k * ns) : mk<T>((T)0, (T)0);
         });
     });
 }
@@ -220,64 +300,144 @@ PF_HD void store_B(const cx<typename G::T> *v, cx<typename G::T> *dst, long long
 }
 
 // ------------------------------------------------------------------ pass bodies
+#define PF_BODY_PROLOGUE(NEED_A, NEED_B)                                                              \
+    using T = typename G::T;                                                                          \
+    int t, p; G::split(tid, t, p);                                                                    \
+    cx<T> *smem_c = reinterpret_cast<cx<T> *>(smem);                                                  \
+    XBufs<G> xbufs(smem_c);                                                                           \
+    Twiddles<G> tw;                                                                                   \
+    pdl_launch_dependents();                                                                          \
+    tw.template init<NEED_A, NEED_B>(reinterpret_cast<const cx<T> *>(prm.tw), smem_c + G::NBUF * G::XELEMS, tid, t); \
+    pdl_wait_prior_grid();
+
+// Persistent tile loop.  With G::PREF the loads of tile j+1 are issued before tile j is transformed
+// (they stay in flight across the barriers), so DRAM latency overlaps the FP64 work of the same CTA.
+template <class G, class Buf, class Issue, class Process>
+PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, Process &&process) {
+    if constexpr (G::PREF) {
+        Buf cur, nxt;
+        int tile = bid;
+        if (tile < n_tiles) issue(cur, tile);
+        for (; tile < n_tiles; tile += nb) {
+            const int tn = tile + nb;
+            if (tn < n_tiles) issue(nxt, tn);
+            process(cur, tile);
+            cur = nxt;
+        }
+    } else {
+        for (int tile = bid; tile < n_tiles; tile += nb) {
+            Buf cur;
+            issue(cur, tile);
+            process(cur, tile);
+        }
+    }
+}
+
+template <class G, bool PRUNED> struct BufA {   // inputs of a forward transform (layout A, data half only)
+    static constexpr int NA2 = PRUNED ? G::RA / 2 : G::RA;
+    cx<typename G::T> x[G::CA * NA2];
+};
+template <class G> struct BufB {                // inputs of an inverse transform (layout B)
+    cx<typename G::T> x[G::V];
+};
+template <class G, bool PRUNED> struct BufAK {  // F3: inputs + the tile's K^F values
+    static constexpr int NA2 = PRUNED ? G::RA / 2 : G::RA;
+    cx<typename G::T> x[G::CA * NA2];
+    typename G::T k[G::KLATE ? 1 : G::V];
+};
+
+template <class G, bool PRUNED, bool STREAM, class B, typename E>
+PF_HD void issue_A(B &b, const E *src, long long ns, int t, bool valid) {
+    using T = typename G::T;
+    constexpr int NA2 = PRUNED ? G::RA / 2 : G::RA;
+    static_for<G::CA>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        static_for<NA2>([&](auto nc) {
+            constexpr int n2 = decltype(nc)::value;
+            const int n = (t + G::TPP * i) + G::RB * n2;
+            b.x[i * NA2 + n2] = valid ? ld_hint<STREAM>(src + n * ns) : mk<T>((T)0, (T)0);
+        });
+    });
+}
+template <class G, bool PRUNED, class B>
+PF_HD void unpack_A(cx<typename G::T> *v, const B &b) {
+    constexpr int NA2 = PRUNED ? G::RA / 2 : G::RA;
+    static_for<G::CA>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        static_for<NA2>([&](auto nc) { constexpr int n2 = decltype(nc)::value; v[i * G::RA + n2] = b.x[i * NA2 + n2]; });
+    });
+}
+
+#define PF_TILE_COORDS                                                                   \
+    const int g = tile / prm.tiles_per_g, pp = (tile % prm.tiles_per_g) * G::P + p;      \
+    const bool valid = pp < prm.n_p;
+
 // F2: (transpose +) spread + 1D FFT along axis b
 template <class G, bool PRUNED>
 PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    using T = typename G::T;
-    int t, p; G::split(tid, t, p);
-    cx<T> *xb = reinterpret_cast<cx<T> *>(smem);
-    Twiddles<G> tw; tw.template load<true, false>(reinterpret_cast<const cx<T> *>(prm.tw), t);
-    int par = 0;
-    for (int tile = bid; tile < prm.n_tiles; tile += nb, par ^= 1) {
-        const int g = tile / prm.tiles_per_g, pp = (tile % prm.tiles_per_g) * G::P + p;
-        const bool valid = pp < prm.n_p;
-        cx<T> v[G::V];
-        load_A<G, PRUNED>(v, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
-        fwd_AtoB<G, PRUNED>(v, tw, xb + par * G::XELEMS, t, p);
-        store_B<G>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
-    }
+    PF_BODY_PROLOGUE(true, false)
+    using Buf = BufA<G, PRUNED>;
+    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            issue_A<G, PRUNED, true>(b, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+        },
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            cx<T> v[G::V];
+            unpack_A<G, PRUNED>(v, b);
+            fwd_AtoB<G, PRUNED>(v, tw, xbufs.next(), t, p);
+            store_B<G>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+        });
 }
 
 // I2: inverse 1D FFT along axis b + compactification (+ transpose)
 template <class G, bool PRUNED>
 PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    using T = typename G::T;
-    int t, p; G::split(tid, t, p);
-    cx<T> *xb = reinterpret_cast<cx<T> *>(smem);
-    Twiddles<G> tw; tw.template load<false, true>(reinterpret_cast<const cx<T> *>(prm.tw), t);
-    int par = 0;
-    for (int tile = bid; tile < prm.n_tiles; tile += nb, par ^= 1) {
-        const int g = tile / prm.tiles_per_g, pp = (tile % prm.tiles_per_g) * G::P + p;
-        const bool valid = pp < prm.n_p;
-        cx<T> v[G::V];
-        load_B<G>(v, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
-        inv_BtoA<G, PRUNED>(v, tw, xb + par * G::XELEMS, t, p);
-        store_A<G, PRUNED>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
-    }
+    PF_BODY_PROLOGUE(false, true)
+    using Buf = BufB<G>;
+    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            load_B<G, true>(b.x, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);  // last read of A2
+        },
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            inv_BtoA<G, PRUNED>(b.x, tw, xbufs.next(), t, p);
+            store_A<G, PRUNED>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+        });
 }
 
 // F3: spread + 1D FFT along axis c, K^F multiply (Eq. 3), inverse 1D FFT along c,
 // compactification; in place over the tile it read.
 template <class G, bool PRUNED>
 PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    using T = typename G::T;
-    int t, p; G::split(tid, t, p);
-    cx<T> *xb0 = reinterpret_cast<cx<T> *>(smem), *xb1 = xb0 + G::XELEMS;
-    Twiddles<G> tw; tw.template load<true, true>(reinterpret_cast<const cx<T> *>(prm.tw), t);
+    PF_BODY_PROLOGUE(true, true)
     const T *kint = reinterpret_cast<const T *>(prm.kint);
-    for (int tile = bid; tile < prm.n_tiles; tile += nb) {
-        const int g = tile / prm.tiles_per_g, pp = (tile % prm.tiles_per_g) * G::P + p;
-        const bool valid = pp < prm.n_p;
-        cx<T> v[G::V];
-        load_A<G, PRUNED>(v, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
-        T kv[G::V];
-        const T *kp = kint + (size_t)tile * G::V * G::NT + tid;
-        static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; kv[r] = kp[(size_t)r * G::NT]; });
-        fwd_AtoB<G, PRUNED>(v, tw, xb0, t, p);
-        static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], kv[r]); });
-        inv_BtoA<G, PRUNED>(v, tw, xb1, t, p);
-        store_A<G, PRUNED>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
-    }
+    using Buf = BufAK<G, PRUNED>;
+    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            issue_A<G, PRUNED, false>(b, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+            if constexpr (!G::KLATE) {
+                const T *kp = kint + (size_t)tile * G::V * G::NT + tid;
+                static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; b.k[r] = ld_stream(kp + (size_t)r * G::NT); });
+            }
+        },
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            cx<T> v[G::V];
+            unpack_A<G, PRUNED>(v, b);
+            fwd_AtoB<G, PRUNED>(v, tw, xbufs.next(), t, p);
+            if constexpr (G::KLATE) {
+                const T *kp = kint + (size_t)tile * G::V * G::NT + tid;
+                static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], ld_stream(kp + (size_t)r * G::NT)); });
+            } else {
+                static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], b.k[r]); });
+            }
+            inv_BtoA<G, PRUNED>(v, tw, xbufs.next(), t, p);
+            store_A<G, PRUNED>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+        });
 }
 
 // F1: spread + 1D FFT (R2C) along axis a
@@ -286,39 +446,42 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
 // F_{S-k} = conj(F_k) of PAPER.md:55; only k = 0..S/2 is kept.  in: pairs, out: complex.
 template <class G, bool PRUNED>
 PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    using T = typename G::T;
     static_assert(G::LANES_P, "the R2C pass runs on a strided axis");
-    int t, p; G::split(tid, t, p);
-    cx<T> *xb0 = reinterpret_cast<cx<T> *>(smem), *xb1 = xb0 + G::XELEMS;
-    Twiddles<G> tw; tw.template load<true, false>(reinterpret_cast<const cx<T> *>(prm.tw), t);
+    PF_BODY_PROLOGUE(true, false)
     constexpr int S = G::S, NK = S / 2 + 1, NM = (NK + G::TPP - 1) / G::TPP;
-    for (int tile = bid; tile < prm.n_tiles; tile += nb) {
-        const int g = tile / prm.tiles_per_g, pp = (tile % prm.tiles_per_g) * G::P + p;
-        const bool valid = pp < prm.n_p;
-        cx<T> v[G::V];
-        load_A<G, PRUNED>(v, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
-        fwd_AtoB<G, PRUNED>(v, tw, xb0, t, p);
-        static_for<G::CB>([&](auto ic) {
-            constexpr int i = decltype(ic)::value;
-            static_for<G::RB>([&](auto kc) {
-                constexpr int k1 = decltype(kc)::value;
-                xb1[G::nidx(p, (t + G::TPP * i) + G::RA * k1)] = v[i * G::RB + k1];
+    using Buf = BufA<G, PRUNED>;
+    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            issue_A<G, PRUNED, true>(b, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+        },
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            cx<T> v[G::V];
+            unpack_A<G, PRUNED>(v, b);
+            fwd_AtoB<G, PRUNED>(v, tw, xbufs.next(), t, p);
+            cx<T> *xn = xbufs.next();
+            static_for<G::CB>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                static_for<G::RB>([&](auto kc) {
+                    constexpr int k1 = decltype(kc)::value;
+                    xn[G::nidx(p, (t + G::TPP * i) + G::RA * k1)] = v[i * G::RB + k1];
+                });
+            });
+            cta_sync();
+            cx<T> *dst = reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + 2 * pp * prm.ps_out;
+            static_for<NM>([&](auto mc) {
+                constexpr int m = decltype(mc)::value;
+                const int k = t + G::TPP * m;
+                if (k < NK && valid) {
+                    const cx<T> zk = xn[G::nidx(p, k)], zp = xn[G::nidx(p, (S - k) % S)];
+                    const T hf = (T)0.5;
+                    // A = (Z_k + conj Z_{S-k})/2 ; B = -i (Z_k - conj Z_{S-k})/2
+                    dst[k * prm.ns_out] = mk<T>(hf * (zk.re + zp.re), hf * (zk.im - zp.im));
+                    dst[k * prm.ns_out + prm.ps_out] = mk<T>(hf * (zk.im + zp.im), hf * (zp.re - zk.re));
+                }
             });
         });
-        cta_sync();
-        cx<T> *dst = reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + 2 * pp * prm.ps_out;
-        static_for<NM>([&](auto mc) {
-            constexpr int m = decltype(mc)::value;
-            const int k = t + G::TPP * m;
-            if (k < NK && valid) {
-                const cx<T> zk = xb1[G::nidx(p, k)], zp = xb1[G::nidx(p, (S - k) % S)];
-                const T hf = (T)0.5;
-                // A = (Z_k + conj Z_{S-k})/2 ; B = -i (Z_k - conj Z_{S-k})/2
-                dst[k * prm.ns_out] = mk<T>(hf * (zk.re + zp.re), hf * (zk.im - zp.im));
-                dst[k * prm.ns_out + prm.ps_out] = mk<T>(hf * (zk.im + zp.im), hf * (zp.re - zk.re));
-            }
-        });
-    }
 }
 
 // I1: inverse 1D FFT (C2R) along axis a + compactification
@@ -326,33 +489,32 @@ PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
 // one complex inverse transform, real part -> pencil 2q, imaginary part -> pencil 2q+1.
 template <class G, bool PRUNED>
 PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    using T = typename G::T;
     static_assert(G::LANES_P, "the C2R pass runs on a strided axis");
-    int t, p; G::split(tid, t, p);
-    cx<T> *xb = reinterpret_cast<cx<T> *>(smem);
-    Twiddles<G> tw; tw.template load<false, true>(reinterpret_cast<const cx<T> *>(prm.tw), t);
+    PF_BODY_PROLOGUE(false, true)
     constexpr int S = G::S;
-    int par = 0;
-    for (int tile = bid; tile < prm.n_tiles; tile += nb, par ^= 1) {
-        const int g = tile / prm.tiles_per_g, pp = (tile % prm.tiles_per_g) * G::P + p;
-        const bool valid = pp < prm.n_p;
-        cx<T> v[G::V];
-        const cx<T> *src = reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + 2 * pp * prm.ps_in;
-        static_for<G::CB>([&](auto ic) {
-            constexpr int i = decltype(ic)::value;
-            static_for<G::RB>([&](auto kc) {
-                constexpr int k1 = decltype(kc)::value;
-                const int k = (t + G::TPP * i) + G::RA * k1;
-                const bool lower = k <= S / 2;
-                const int kk = lower ? k : S - k;
-                cx<T> a = mk<T>((T)0, (T)0), b = a;
-                if (valid) { a = src[kk * prm.ns_in]; b = src[kk * prm.ns_in + prm.ps_in]; }
-                v[i * G::RB + k1] = lower ? mk<T>(a.re - b.im, a.im + b.re) : mk<T>(a.re + b.im, b.re - a.im);
+    using Buf = BufB<G>;
+    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            const cx<T> *src = reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + 2 * pp * prm.ps_in;
+            static_for<G::CB>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                static_for<G::RB>([&](auto kc) {
+                    constexpr int k1 = decltype(kc)::value;
+                    const int k = (t + G::TPP * i) + G::RA * k1;
+                    const bool lower = k <= S / 2;
+                    const int kk = lower ? k : S - k;
+                    cx<T> a = mk<T>((T)0, (T)0), bb = a;
+                    if (valid) { a = src[kk * prm.ns_in]; bb = src[kk * prm.ns_in + prm.ps_in]; }
+                    b.x[i * G::RB + k1] = lower ? mk<T>(a.re - bb.im, a.im + bb.re) : mk<T>(a.re + bb.im, bb.re - a.im);
+                });
             });
+        },
+        [&](Buf &b, int tile) {
+            PF_TILE_COORDS
+            inv_BtoA<G, PRUNED>(b.x, tw, xbufs.next(), t, p);
+            store_A<G, PRUNED, true>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
         });
-        inv_BtoA<G, PRUNED>(v, tw, xb + par * G::XELEMS, t, p);
-        store_A<G, PRUNED>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
-    }
 }
 
 }  // namespace pfft

@@ -15,6 +15,8 @@ struct KernelEntry {
     int pruned;    // 1: zero-padded axis (spread / compactification fused), 0: periodic axis
     int lanes_p;   // 1: lanes along the pencil index (strided pencils), 0: lanes along the transform
     int prec;      // 0 fp64, 1 fp32
+    int variant;   // tuning variant (0 = default; others selectable with POISSON_VARIANT for experiments)
+    int nbuf, tws, minb, pref;
     int RA, RB;    // S = RA * RB: radix of the first / second register pass
     int P, TPP, V, NT;
     size_t smem_bytes;
@@ -22,7 +24,7 @@ struct KernelEntry {
 };
 
 std::vector<KernelEntry> &kernel_registry();
-const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int prec);
+const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int prec, int variant = -1);
 bool length_supported(int S);
 
 }  // namespace pfft

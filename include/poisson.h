@@ -143,6 +143,12 @@ POISSON_API int poisson_profile_read(poisson_plan *plan, double ms_sum[5] /* hos
 /* Number of kernel launches one poisson_solve enqueues (bench.py's gpu_launches). */
 POISSON_API int poisson_plan_launches_per_solve(const poisson_plan *plan);
 
+/* Measures the plain-ALU fused-multiply-add peak of the current device for the given precision
+ * (independent FMA chains in registers, no memory traffic) and returns it in TFLOP/s counting an
+ * FMA as 2 flops.  bench.py quotes the solve's nominal FLOP rate against this number; it is the
+ * ALU bound of DESIGN.md, not a tensor-core figure.  Synchronous.  Errors: EINVAL, EARCH, ECUDA. */
+POISSON_API int poisson_measure_fma_peak(int precision, double *tflops /* host, out */);
+
 POISSON_API size_t poisson_plan_workspace_bytes(const poisson_plan *plan);
 POISSON_API int poisson_plan_destroy(poisson_plan *plan);
 

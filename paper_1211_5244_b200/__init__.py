@@ -13,7 +13,7 @@ from pathlib import Path
 __all__ = [
     "FREE", "PERIODIC", "FP64", "FP32", "PoissonError", "PlanInfo", "lib_path", "load_library",
     "poisson_plan_describe", "poisson_plan_create", "poisson_set_kernel", "poisson_solve",
-    "poisson_solve_host", "poisson_plan_destroy", "PoissonPlan", "EXPORTED_SYMBOLS",
+    "poisson_solve_host", "poisson_plan_destroy", "poisson_measure_fma_peak", "PoissonPlan", "EXPORTED_SYMBOLS",
 ]
 
 FREE, PERIODIC = 0, 1
@@ -23,7 +23,7 @@ PASS_NAMES = ("F1", "F2", "F3", "I2", "I1")
 EXPORTED_SYMBOLS = (
     "poisson_plan_describe", "poisson_plan_create", "poisson_plan_kernel_dims", "poisson_plan_get_info",
     "poisson_set_kernel", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
-    "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_plan_workspace_bytes",
+    "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_measure_fma_peak", "poisson_plan_workspace_bytes",
     "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch",
 )
 
@@ -84,6 +84,7 @@ def load_library():
     lib.poisson_debug_run_passes.argtypes = [vp, vp, vp, vp, i, i]
     lib.poisson_solve_profiled.argtypes = [vp, vp, vp, vp]
     lib.poisson_profile_read.argtypes = [vp, ctypes.c_double * 5, ctypes.POINTER(i)]
+    lib.poisson_measure_fma_peak.argtypes = [i, ctypes.POINTER(ctypes.c_double)]
     lib.poisson_plan_launches_per_solve.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.restype = ctypes.c_size_t
@@ -130,6 +131,13 @@ def poisson_solve(plan: int, rho_dev_ptr: int, V_dev_ptr: int, stream: int = 0) 
 
 def poisson_solve_host(plan: int, rho_host_ptr: int, V_host_ptr: int, stream: int = 0) -> None:
     _check(load_library().poisson_solve_host(plan, rho_host_ptr, V_host_ptr, stream), "poisson_solve_host")
+
+
+def poisson_measure_fma_peak(precision: int = FP64) -> float:
+    """Plain-ALU FMA peak of the current device in TFLOP/s (FMA = 2 flops)."""
+    out = ctypes.c_double()
+    _check(load_library().poisson_measure_fma_peak(precision, ctypes.byref(out)), "poisson_measure_fma_peak")
+    return out.value
 
 
 def poisson_plan_destroy(plan: int) -> None:

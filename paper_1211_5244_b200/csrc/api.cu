@@ -57,6 +57,22 @@ __global__ void relayout_kernel(const T *__restrict__ kuser, T *__restrict__ kin
         kint[idx] = relayout_value<T>(kuser, q, idx);
 }
 
+// FMA peak probe: 16 independent chains per thread, result kept alive through a never-true store.
+template <typename T>
+__global__ void fma_peak_kernel(T *sink, int iters, T a, T b) {
+    T x[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = (T)(threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = x[i] * a + b;
+    }
+    T acc = 0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) acc += x[i];
+    if (acc == (T)123456789) sink[threadIdx.x] = acc;
+}
+
 }  // namespace pfft
 
 using namespace pfft;
@@ -211,6 +227,37 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     pl->workspace_bytes = ws;
     pl->d.info.workspace_bytes = (long long)ws;
     *out = pl;
+    return POISSON_OK;
+}
+
+int poisson_measure_fma_peak(int precision, double *tflops) {
+    if (!tflops || (precision != POISSON_FP64 && precision != POISSON_FP32)) return POISSON_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return POISSON_EARCH; }
+    int dev = 0;
+    PF_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    PF_CUDA(cudaGetDeviceProperties(&prop, dev));
+    void *sink = nullptr;
+    PF_CUDA(cudaMalloc(&sink, 1024 * sizeof(double)));
+    cudaEvent_t e0, e1;
+    PF_CUDA(cudaEventCreate(&e0));
+    PF_CUDA(cudaEventCreate(&e1));
+    const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 4096;
+    float best_ms = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {
+        PF_CUDA(cudaEventRecord(e0));
+        if (precision == POISSON_FP64) fma_peak_kernel<double><<<blocks, threads>>>(static_cast<double *>(sink), iters, 1.0000001, 1e-9);
+        else fma_peak_kernel<float><<<blocks, threads>>>(static_cast<float *>(sink), iters, 1.0000001f, 1e-9f);
+        PF_CUDA(cudaEventRecord(e1));
+        PF_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        PF_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best_ms) best_ms = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    const double flops = 2.0 * 16.0 * (double)iters * (double)blocks * (double)threads;
+    *tflops = flops / (best_ms * 1e-3) / 1e12;
     return POISSON_OK;
 }
 

@@ -340,10 +340,13 @@ def run_ours(args):
     dom = int(np.argmax(res["pass_ms"]))
     dom_gbs = info.bytes[dom] / (res["pass_ms"][dom] * 1e-3) / 1e9
     traffic = None
-    tfile = ROOT / "profiles" / "dram_traffic.json"
+    tfile = ROOT / "profiles" / "dram_traffic.csv"     # ncu dram__bytes_read.sum + dram__bytes_write.sum per launch
     if tfile.exists():
         try:
-            traffic = json.loads(tfile.read_text()).get(args.config, {}).get(pk.PASS_NAMES[dom])
+            import csv
+            for row in csv.DictReader(tfile.open()):
+                if row["config"] == args.config and row["pass"] == pk.PASS_NAMES[dom]:
+                    traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
         except Exception:
             traffic = None
     line = {

@@ -1,6 +1,6 @@
 // inst.cuh -- instantiates and registers every pass kernel for ONE transform length.
 // An inst_S<len>_<prec>.cu file defines PF_S, PF_RA, PF_RB, PF_TPP (and optionally the tuning knobs
-// PF_NBUF, PF_TWS, PF_MINB, PF_PREF, PF_EXTRA_VARIANTS) and includes this header.
+// PF_NBUF, PF_TWS, PF_MINB, PF_STG, PF_EXTRA_VARIANTS) and includes this header.
 #pragma once
 
 #include "passes.cuh"
@@ -23,9 +23,9 @@ template <class G, bool PRUNED, int KIND>
 static void reg_one(int prec, int variant) {
     KernelEntry e;
     e.kind = KIND; e.S = G::S; e.pruned = PRUNED ? 1 : 0; e.lanes_p = G::LANES_P ? 1 : 0; e.prec = prec;
-    e.variant = variant; e.nbuf = G::NBUF; e.tws = G::TWS ? 1 : 0; e.minb = G::MINB; e.pref = G::PREF;
+    e.variant = variant; e.nbuf = G::NBUF; e.tws = G::TWS ? 1 : 0; e.minb = G::MINB; e.stg = G::STG;
     e.RA = G::RA; e.RB = G::RB;
-    e.P = G::P; e.TPP = G::TPP; e.V = G::V; e.NT = G::NT; e.smem_bytes = G::SMEM_BYTES;
+    e.P = G::P; e.TPP = G::TPP; e.V = G::V; e.NT = G::NT; e.smem_bytes = pass_smem_bytes<G, PRUNED, KIND>();
     e.func = reinterpret_cast<const void *>(&pass_kernel<G, PRUNED, KIND>);
     kernel_registry().push_back(e);
 }
@@ -38,11 +38,11 @@ constexpr int pencils_per_cta() {
     return by_threads > by_line ? by_threads : by_line;
 }
 
-template <typename T, int S, int RA, int RB, int TPP, int NBUF, bool TWS, int MINB, int PREF, bool KLATE>
+template <typename T, int S, int RA, int RB, int TPP, int NBUF, bool TWS, int MINB, int STG, bool KLATE>
 static void reg_length(int prec, int variant) {
     constexpr int P = pencils_per_cta<T, TPP>();
-    using GP = Geo<T, S, RA, RB, TPP, P, true, NBUF, TWS, MINB, PREF, KLATE>;
-    using GC = Geo<T, S, RA, RB, TPP, P, false, NBUF, TWS, MINB, PREF, KLATE>;
+    using GP = Geo<T, S, RA, RB, TPP, P, true, NBUF, TWS, MINB, STG, KLATE>;
+    using GC = Geo<T, S, RA, RB, TPP, P, false, NBUF, TWS, MINB, STG, KLATE>;
     reg_one<GP, true, KIND_F1>(prec, variant);  reg_one<GP, false, KIND_F1>(prec, variant);
     reg_one<GP, true, KIND_I1>(prec, variant);  reg_one<GP, false, KIND_I1>(prec, variant);
     reg_one<GP, true, KIND_F2>(prec, variant);  reg_one<GP, false, KIND_F2>(prec, variant);
@@ -65,8 +65,8 @@ static void reg_length(int prec, int variant) {
 #ifndef PF_MINB
 #define PF_MINB 0
 #endif
-#ifndef PF_PREF
-#define PF_PREF 0
+#ifndef PF_STG
+#define PF_STG 1
 #endif
 #ifndef PF_KLATE
 #define PF_KLATE true
@@ -81,9 +81,9 @@ static void reg_length(int prec, int variant) {
 namespace {
 struct PfRegistrar {
     PfRegistrar() {
-        pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, PF_NBUF, PF_TWS, PF_MINB, PF_PREF, PF_KLATE>(PF_PREC, 0);
+        pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, PF_NBUF, PF_TWS, PF_MINB, PF_STG, PF_KLATE>(PF_PREC, 0);
 #if defined(PF_EXTRA_VARIANTS)
-#define PF_VARIANT(ID, NBUF, TWS, MINB, PREF, KLATE) pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, NBUF, TWS, MINB, PREF, KLATE>(PF_PREC, ID);
+#define PF_VARIANT(ID, NBUF, TWS, MINB, STG, KLATE) pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, NBUF, TWS, MINB, STG, KLATE>(PF_PREC, ID);
         PF_EXTRA_VARIANTS
 #undef PF_VARIANT
 #endif

@@ -41,16 +41,18 @@ PF_HD void warp_sync() { host_cta_sync(); }
 // NBUF_   : exchange buffers (2 = one barrier per exchange, 1 = half the shared memory, one more barrier)
 // TWS_    : twiddles w_S^{n1 k2} read from a shared-memory table (true) or held in registers (false)
 // MINB_   : __launch_bounds__ minimum resident CTAs per SM (register cap); 0 = automatic
-// PREF_   : 1 = the next tile's inputs are loaded into registers while the current tile is transformed
+// STG_    : asynchronous staging (cp.async, no register cost): 0 = none, tiles are loaded straight into
+//           registers; 1 = the NEXT tile's inputs land in a shared-memory stage while the current tile is
+//           transformed; 2 = as 1, and pass F3 also stages its K^F values
 // KLATE_  : pass F3 loads its K^F values right before the multiply (fewer live registers) instead of
 //           at the top of the tile
 template <typename T_, int S_, int RA_, int RB_, int TPP_, int P_, bool LANES_P_, int NBUF_ = 2, bool TWS_ = true,
-          int MINB_ = 0, int PREF_ = 0, bool KLATE_ = false>
+          int MINB_ = 0, int STG_ = 0, bool KLATE_ = false>
 struct Geo {
     using T = T_;
     static constexpr int S = S_, RA = RA_, RB = RB_, TPP = TPP_, P = P_;
     static constexpr bool LANES_P = LANES_P_;
-    static constexpr int NBUF = NBUF_, PREF = PREF_;
+    static constexpr int NBUF = NBUF_, STG = STG_;
     static constexpr bool KLATE = KLATE_;
     // lanes along the transform: the TPP threads of a pencil sit in one warp, so the exchange is
     // warp-private and a warp-level barrier is enough
@@ -299,35 +301,163 @@ PF_HD void store_B(const cx<typename G::T> *v, cx<typename G::T> *dst, long long
     });
 }
 
+// ------------------------------------------------------------------ asynchronous staging (cp.async / LDGSTS)
+// With G::STG > 0 a CTA keeps ONE tile of input in flight in shared memory while it transforms the
+// previous one: the copies are issued right after the current tile has been pulled into registers and
+// have the whole transform + store of that tile to land, at no register cost.
+enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4 };
+
+PF_HD unsigned long long evict_first_policy() {
+#if defined(__CUDA_ARCH__)
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+#else
+    return 0ull;
+#endif
+}
+// one complex element, global -> shared (16 B: L2 only; 8 B: the only size cp.async.cg does not offer)
+template <bool STREAM> PF_HD void cp_async_elem(cx<double> *sdst, const cx<double> *gsrc, unsigned long long pol) {
+#if defined(__CUDA_ARCH__)
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
+    if constexpr (STREAM) asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
+    else asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+#else
+    *sdst = *gsrc;
+#endif
+}
+template <bool STREAM> PF_HD void cp_async_elem(cx<float> *sdst, const cx<float> *gsrc, unsigned long long pol) {
+#if defined(__CUDA_ARCH__)
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
+    if constexpr (STREAM) asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
+    else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
+#else
+    *sdst = *gsrc;
+#endif
+}
+// 16 raw bytes (K^F vectors), evict-first
+PF_HD void cp_async_vec16(void *sdst, const void *gsrc, unsigned long long pol) {
+#if defined(__CUDA_ARCH__)
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
+#else
+    for (int b = 0; b < 16; ++b) static_cast<char *>(sdst)[b] = static_cast<const char *>(gsrc)[b];
+#endif
+}
+PF_HD void cp_async_commit() {
+#if defined(__CUDA_ARCH__)
+    asm volatile("cp.async.commit_group;" ::: "memory");
+#endif
+}
+template <int N> PF_HD void cp_async_wait() {   // at most N of this thread's newest groups still pending
+#if defined(__CUDA_ARCH__)
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+#endif
+}
+
+// K^F values travel in 16-byte vectors: KVEC consecutive registers r of one thread
+template <typename T> struct KVec;
+template <> struct KVec<double> { static constexpr int N = 2; using V = double2; };
+template <> struct KVec<float>  { static constexpr int N = 4; using V = float4; };
+PF_HD void kvec_get(const double2 &v, double *o) { o[0] = v.x; o[1] = v.y; }
+PF_HD void kvec_get(const float4 &v, float *o) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
+template <typename VT> PF_HD VT ld_stream_vec(const VT *p) {
+#if defined(__CUDA_ARCH__)
+    return __ldcs(p);
+#else
+    return *p;
+#endif
+}
+
+// Shape of the stage of pass KIND: NR points along the transform x W complex columns.
+template <class G, bool PRUNED, int KIND>
+struct Stage {
+    using T = typename G::T;
+    static constexpr int NR = KIND == KIND_I1 ? G::S / 2 + 1 : (KIND == KIND_I2 ? G::S : (PRUNED ? G::S / 2 : G::S));
+    static constexpr int W = KIND == KIND_I1 ? 2 * G::P : G::P;
+    // staging is dropped where it would not leave room for G::MINB resident CTAs (228 KB per SM, 1 KB
+    // reserved per CTA): the occupancy the register budget was chosen for wins
+    static constexpr size_t SM_SMEM = 233472, CTA_RESERVED = 1024;
+    static constexpr bool fits(size_t stage_bytes) { return (G::SMEM_BYTES + stage_bytes + CTA_RESERVED) * G::MINB <= SM_SMEM; }
+    static constexpr bool ON = G::STG > 0 && fits((size_t)NR * W * sizeof(cx<T>));
+    static constexpr bool KON = ON && G::STG > 1 && KIND == KIND_F3 && fits(((size_t)NR * W + G::V * G::NT / 2) * sizeof(cx<T>));
+    static constexpr int IN_ELEMS = ON ? NR * W : 0;
+    static constexpr int K_ELEMS = KON ? G::V * G::NT / 2 : 0;   // V*NT reals
+    static constexpr size_t BYTES = (size_t)(IN_ELEMS + K_ELEMS) * sizeof(cx<T>);
+    // I1: the two pencils of a pair are de-interleaved so that both reads are contiguous across lanes
+    static PF_HD int idx(int col, int n) {
+        if constexpr (KIND == KIND_I1) return n * W + (col >> 1) + (col & 1) * G::P;
+        else return G::LANES_P ? n * W + col : col * NR + n;
+    }
+};
+template <class G, bool PRUNED, int KIND>
+constexpr size_t pass_smem_bytes() { return G::SMEM_BYTES + Stage<G, PRUNED, KIND>::BYTES; }
+
+// Issue the copies of one tile.  src = element (row 0, column 0) of the tile; ncols = valid columns
+// (ragged last tile).  The threads that later share a barrier scope (CTA, or warp when the exchange
+// is warp-private) copy exactly the columns that scope reads.
+template <class G, class St, bool STREAM>
+PF_HD void stage_issue(cx<typename G::T> *stage, const cx<typename G::T> *src, long long ns, long long ps, int ncols,
+                       int tid, unsigned long long pol) {
+    if constexpr (G::LANES_P) {   // rows of W contiguous elements (ps == 1), stride ns
+        constexpr int TOT = St::NR * St::W, IT = (TOT + G::NT - 1) / G::NT;
+        static_for<IT>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            const int c = tid + G::NT * j, row = c / St::W, col = c % St::W;
+            if ((TOT % G::NT == 0 || c < TOT) && col < ncols) cp_async_elem<STREAM>(stage + St::idx(col, row), src + row * ns + col, pol);
+        });
+    } else {                      // contiguous pencils (ns == 1), stride ps
+        constexpr int GT = G::WARP_LOCAL ? 32 : G::NT, GP = GT / G::TPP;
+        constexpr int TOT = GP * St::NR, IT = (TOT + GT - 1) / GT;
+        const int grp = tid / GT, l = tid % GT;
+        static_for<IT>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            const int c = l + GT * j, pl = c / St::NR, n = c % St::NR, col = grp * GP + pl;
+            if ((TOT % GT == 0 || c < TOT) && col < ncols) cp_async_elem<false>(stage + St::idx(col, n), src + col * ps + n, pol);
+        });
+    }
+}
+
 // ------------------------------------------------------------------ pass bodies
-#define PF_BODY_PROLOGUE(NEED_A, NEED_B)                                                              \
+#define PF_BODY_PROLOGUE(NEED_A, NEED_B, KIND)                                                        \
     using T = typename G::T;                                                                          \
+    using St = Stage<G, PRUNED, KIND>;                                                                \
     int t, p; G::split(tid, t, p);                                                                    \
     cx<T> *smem_c = reinterpret_cast<cx<T> *>(smem);                                                  \
     XBufs<G> xbufs(smem_c);                                                                           \
+    cx<T> *stage = smem_c + G::NBUF * G::XELEMS + G::TW_ELEMS;                                        \
+    const unsigned long long pol = St::ON ? evict_first_policy() : 0ull;                              \
+    (void)stage; (void)pol;                                                                           \
     Twiddles<G> tw;                                                                                   \
     pdl_launch_dependents();                                                                          \
     tw.template init<NEED_A, NEED_B>(reinterpret_cast<const cx<T> *>(prm.tw), smem_c + G::NBUF * G::XELEMS, tid, t); \
     pdl_wait_prior_grid();
 
-// Persistent tile loop.  With G::PREF the loads of tile j+1 are issued before tile j is transformed
-// (they stay in flight across the barriers), so DRAM latency overlaps the FP64 work of the same CTA.
-template <class G, class Buf, class Issue, class Process>
-PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, Process &&process) {
-    if constexpr (G::PREF) {
-        Buf cur, nxt;
+// Persistent tile loop.  issue(tile): start the asynchronous copies of a tile (staged mode only);
+// after_first(): hook after the very first issue; fetch(buf, tile): tile -> registers (from the stage,
+// or straight from global memory when not staged); process(buf, tile): transform and store.
+// WAITN = copy groups that may still be pending when a tile's inputs are needed.
+template <class G, class Buf, bool STAGED, int WAITN, class Issue, class After, class Fetch, class Process>
+PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_first, Fetch &&fetch, Process &&process) {
+    if constexpr (STAGED) {
         int tile = bid;
-        if (tile < n_tiles) issue(cur, tile);
+        if (tile < n_tiles) issue(tile);
+        cp_async_commit();
+        after_first();
         for (; tile < n_tiles; tile += nb) {
-            const int tn = tile + nb;
-            if (tn < n_tiles) issue(nxt, tn);
+            Buf cur;
+            cp_async_wait<WAITN>();
+            G::xsync();                       // every copy of the scope has landed
+            fetch(cur, tile);
+            G::xsync();                       // stage free again
+            if (tile + nb < n_tiles) issue(tile + nb);
+            cp_async_commit();
             process(cur, tile);
-            cur = nxt;
         }
     } else {
         for (int tile = bid; tile < n_tiles; tile += nb) {
             Buf cur;
-            issue(cur, tile);
+            fetch(cur, tile);
             process(cur, tile);
         }
     }
@@ -340,12 +470,13 @@ template <class G, bool PRUNED> struct BufA {   // inputs of a forward transform
 template <class G> struct BufB {                // inputs of an inverse transform (layout B)
     cx<typename G::T> x[G::V];
 };
-template <class G, bool PRUNED> struct BufAK {  // F3: inputs + the tile's K^F values
+template <class G, bool PRUNED, bool WITH_K> struct BufAK {  // F3: inputs (+ the tile's K^F values)
     static constexpr int NA2 = PRUNED ? G::RA / 2 : G::RA;
     cx<typename G::T> x[G::CA * NA2];
-    typename G::T k[G::KLATE ? 1 : G::V];
+    typename G::T k[WITH_K ? G::V : 1];
 };
 
+// layout A inputs straight from global memory
 template <class G, bool PRUNED, bool STREAM, class B, typename E>
 PF_HD void issue_A(B &b, const E *src, long long ns, int t, bool valid) {
     using T = typename G::T;
@@ -359,6 +490,20 @@ PF_HD void issue_A(B &b, const E *src, long long ns, int t, bool valid) {
         });
     });
 }
+// layout A inputs from the stage
+template <class G, bool PRUNED, class St, class B>
+PF_HD void fetch_A(B &b, const cx<typename G::T> *stage, int t, int p, bool valid) {
+    using T = typename G::T;
+    constexpr int NA2 = PRUNED ? G::RA / 2 : G::RA;
+    static_for<G::CA>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        static_for<NA2>([&](auto nc) {
+            constexpr int n2 = decltype(nc)::value;
+            const int n = (t + G::TPP * i) + G::RB * n2;
+            b.x[i * NA2 + n2] = valid ? stage[St::idx(p, n)] : mk<T>((T)0, (T)0);
+        });
+    });
+}
 template <class G, bool PRUNED, class B>
 PF_HD void unpack_A(cx<typename G::T> *v, const B &b) {
     constexpr int NA2 = PRUNED ? G::RA / 2 : G::RA;
@@ -369,23 +514,32 @@ PF_HD void unpack_A(cx<typename G::T> *v, const B &b) {
 }
 
 #define PF_TILE_COORDS                                                                   \
-    const int g = tile / prm.tiles_per_g, pp = (tile % prm.tiles_per_g) * G::P + p;      \
-    const bool valid = pp < prm.n_p;
+    const int g = tile / prm.tiles_per_g, p0 = (tile % prm.tiles_per_g) * G::P, pp = p0 + p; \
+    const bool valid = pp < prm.n_p;                                                     \
+    (void)p0; (void)valid;
 
 // F2: (transpose +) spread + 1D FFT along axis b
 template <class G, bool PRUNED>
 PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    PF_BODY_PROLOGUE(true, false)
+    PF_BODY_PROLOGUE(true, false, KIND_F2)
     using Buf = BufA<G, PRUNED>;
-    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
+    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
+        [&](int tile) {
+            PF_TILE_COORDS
+            stage_issue<G, St, true>(stage, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
+        },
+        [] {},
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
-            issue_A<G, PRUNED, true>(b, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+            if constexpr (St::ON) fetch_A<G, PRUNED, St>(b, stage, t, p, valid);
+            else issue_A<G, PRUNED, true>(b, in + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
         },
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
             cx<T> v[G::V];
             unpack_A<G, PRUNED>(v, b);
+            if constexpr (St::ON) xbufs.dirty = false;   // the loop's barriers already separate the tiles
             fwd_AtoB<G, PRUNED>(v, tw, xbufs.next(), t, p);
             store_B<G>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
         });
@@ -394,15 +548,33 @@ PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
 // I2: inverse 1D FFT along axis b + compactification (+ transpose)
 template <class G, bool PRUNED>
 PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    PF_BODY_PROLOGUE(false, true)
+    PF_BODY_PROLOGUE(false, true, KIND_I2)
     using Buf = BufB<G>;
-    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
+    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
+        [&](int tile) {
+            PF_TILE_COORDS
+            stage_issue<G, St, true>(stage, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
+        },
+        [] {},
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
-            load_B<G, true>(b.x, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);  // last read of A2
+            if constexpr (St::ON) {
+                static_for<G::CB>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    static_for<G::RB>([&](auto kc) {
+                        constexpr int k1 = decltype(kc)::value;
+                        const int k = (t + G::TPP * i) + G::RA * k1;
+                        b.x[i * G::RB + k1] = valid ? stage[St::idx(p, k)] : mk<T>((T)0, (T)0);
+                    });
+                });
+            } else {
+                load_B<G, true>(b.x, in + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+            }
         },
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
+            if constexpr (St::ON) xbufs.dirty = false;
             inv_BtoA<G, PRUNED>(b.x, tw, xbufs.next(), t, p);
             store_A<G, PRUNED>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
         });
@@ -410,28 +582,62 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
 
 // F3: spread + 1D FFT along axis c, K^F multiply (Eq. 3), inverse 1D FFT along c,
 // compactification; in place over the tile it read.
+// K^F: internal order [tile][V/KVEC][NT][KVEC] (relayout.cuh), 16-byte vectors per thread.
 template <class G, bool PRUNED>
 PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    PF_BODY_PROLOGUE(true, true)
-    const T *kint = reinterpret_cast<const T *>(prm.kint);
-    using Buf = BufAK<G, PRUNED>;
-    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+    PF_BODY_PROLOGUE(true, true, KIND_F3)
+    using KV = KVec<T>;
+    constexpr int NKV = G::V / KV::N;
+    static_assert(G::V % KV::N == 0, "values per thread must fill whole K^F vectors");
+    constexpr bool K_EARLY = !St::KON && !G::KLATE;
+    using Buf = BufAK<G, PRUNED, K_EARLY>;
+    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
+    const typename KV::V *kint = reinterpret_cast<const typename KV::V *>(prm.kint);
+    typename KV::V *kstage = reinterpret_cast<typename KV::V *>(stage + St::IN_ELEMS);
+    (void)kstage;
+    auto issue_k = [&](int tile) {
+        const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
+        static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; cp_async_vec16(kstage + q * G::NT + tid, kp + (size_t)q * G::NT, pol); });
+    };
+    tile_loop<G, Buf, St::ON, (St::KON ? 1 : 0)>(bid, nb, prm.n_tiles,
+        [&](int tile) {
+            PF_TILE_COORDS
+            stage_issue<G, St, false>(stage, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
+        },
+        [&] {
+            if constexpr (St::KON) { if (bid < prm.n_tiles) issue_k(bid); cp_async_commit(); }
+        },
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
-            issue_A<G, PRUNED, false>(b, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
-            if constexpr (!G::KLATE) {
-                const T *kp = kint + (size_t)tile * G::V * G::NT + tid;
-                static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; b.k[r] = ld_stream(kp + (size_t)r * G::NT); });
+            if constexpr (St::ON) fetch_A<G, PRUNED, St>(b, stage, t, p, valid);
+            else issue_A<G, PRUNED, false>(b, in + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+            if constexpr (K_EARLY) {
+                const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
+                static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), b.k + q * KV::N); });
             }
         },
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
             cx<T> v[G::V];
             unpack_A<G, PRUNED>(v, b);
+            if constexpr (St::ON) xbufs.dirty = false;
             fwd_AtoB<G, PRUNED>(v, tw, xbufs.next(), t, p);
-            if constexpr (G::KLATE) {
-                const T *kp = kint + (size_t)tile * G::V * G::NT + tid;
-                static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], ld_stream(kp + (size_t)r * G::NT)); });
+            if constexpr (St::KON) {
+                cp_async_wait<1>();      // everything but the next tile's inputs: this tile's K^F (own copies only)
+                static_for<NKV>([&](auto qc) {
+                    constexpr int q = decltype(qc)::value;
+                    T kk[KV::N]; kvec_get(kstage[q * G::NT + tid], kk);
+                    static_for<KV::N>([&](auto jc) { constexpr int j = decltype(jc)::value; v[q * KV::N + j] = scale(v[q * KV::N + j], kk[j]); });
+                });
+                if (tile + nb < prm.n_tiles) issue_k(tile + nb);
+                cp_async_commit();
+            } else if constexpr (G::KLATE) {
+                const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
+                static_for<NKV>([&](auto qc) {
+                    constexpr int q = decltype(qc)::value;
+                    T kk[KV::N]; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), kk);
+                    static_for<KV::N>([&](auto jc) { constexpr int j = decltype(jc)::value; v[q * KV::N + j] = scale(v[q * KV::N + j], kk[j]); });
+                });
             } else {
                 static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], b.k[r]); });
             }
@@ -447,18 +653,26 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
 template <class G, bool PRUNED>
 PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     static_assert(G::LANES_P, "the R2C pass runs on a strided axis");
-    PF_BODY_PROLOGUE(true, false)
+    PF_BODY_PROLOGUE(true, false, KIND_F1)
     constexpr int S = G::S, NK = S / 2 + 1, NM = (NK + G::TPP - 1) / G::TPP;
     using Buf = BufA<G, PRUNED>;
-    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
+    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
+        [&](int tile) {
+            PF_TILE_COORDS
+            stage_issue<G, St, true>(stage, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
+        },
+        [] {},
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
-            issue_A<G, PRUNED, true>(b, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+            if constexpr (St::ON) fetch_A<G, PRUNED, St>(b, stage, t, p, valid);
+            else issue_A<G, PRUNED, true>(b, in + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
         },
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
             cx<T> v[G::V];
             unpack_A<G, PRUNED>(v, b);
+            if constexpr (St::ON) xbufs.dirty = false;
             fwd_AtoB<G, PRUNED>(v, tw, xbufs.next(), t, p);
             cx<T> *xn = xbufs.next();
             static_for<G::CB>([&](auto ic) {
@@ -490,13 +704,19 @@ PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
 template <class G, bool PRUNED>
 PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     static_assert(G::LANES_P, "the C2R pass runs on a strided axis");
-    PF_BODY_PROLOGUE(false, true)
+    PF_BODY_PROLOGUE(false, true, KIND_I1)
     constexpr int S = G::S;
     using Buf = BufB<G>;
-    tile_loop<G, Buf>(bid, nb, prm.n_tiles,
+    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
+    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
+        [&](int tile) {
+            PF_TILE_COORDS   // stage rows: kk = 0..S/2, columns: the 2 P complex pencils of the P pairs
+            stage_issue<G, St, true>(stage, in + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);
+        },
+        [] {},
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
-            const cx<T> *src = reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + 2 * pp * prm.ps_in;
+            const cx<T> *src = in + g * prm.gs_in + 2 * pp * prm.ps_in;
             static_for<G::CB>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
                 static_for<G::RB>([&](auto kc) {
@@ -505,13 +725,17 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
                     const bool lower = k <= S / 2;
                     const int kk = lower ? k : S - k;
                     cx<T> a = mk<T>((T)0, (T)0), bb = a;
-                    if (valid) { a = src[kk * prm.ns_in]; bb = src[kk * prm.ns_in + prm.ps_in]; }
+                    if (valid) {
+                        if constexpr (St::ON) { a = stage[St::idx(2 * p, kk)]; bb = stage[St::idx(2 * p + 1, kk)]; }
+                        else { a = ld_stream(src + kk * prm.ns_in); bb = ld_stream(src + kk * prm.ns_in + prm.ps_in); }
+                    }
                     b.x[i * G::RB + k1] = lower ? mk<T>(a.re - bb.im, a.im + bb.re) : mk<T>(a.re + bb.im, bb.re - a.im);
                 });
             });
         },
         [&](Buf &b, int tile) {
             PF_TILE_COORDS
+            if constexpr (St::ON) xbufs.dirty = false;
             inv_BtoA<G, PRUNED>(b.x, tw, xbufs.next(), t, p);
             store_A<G, PRUNED, true>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
         });

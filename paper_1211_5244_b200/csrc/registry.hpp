@@ -5,9 +5,9 @@
 #include <cstddef>
 #include <vector>
 
-namespace pfft {
+#include "passes.cuh"   // PassKind
 
-enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4 };
+namespace pfft {
 
 struct KernelEntry {
     int kind;      // PassKind
@@ -16,7 +16,7 @@ struct KernelEntry {
     int lanes_p;   // 1: lanes along the pencil index (strided pencils), 0: lanes along the transform
     int prec;      // 0 fp64, 1 fp32
     int variant;   // tuning variant (0 = default; others selectable with POISSON_VARIANT for experiments)
-    int nbuf, tws, minb, pref;
+    int nbuf, tws, minb, stg;
     int RA, RB;    // S = RA * RB: radix of the first / second register pass
     int P, TPP, V, NT;
     size_t smem_bytes;

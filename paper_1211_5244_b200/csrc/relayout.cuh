@@ -1,7 +1,8 @@
 // relayout.cuh -- where each slot of the internal K^F copy comes from ("a transposition
 // of the associated kernel ... carried out only once").
-// Internal order: kint[(tile*V + r)*NT + tid] -- exactly the order pass F3 reads it in, so the
-// multiply of Eq. 3 streams K^F with perfectly coalesced loads and no index arithmetic.
+// Internal order: kint[((tile*(V/KVEC) + q)*NT + tid)*KVEC + j], r = q*KVEC + j, KVEC = 16 bytes of
+// reals -- exactly the 16-byte vectors thread `tid` of pass F3 consumes for its registers r, so the
+// multiply of Eq. 3 streams K^F with perfectly coalesced 128-bit accesses and no index arithmetic.
 #pragma once
 
 #include "fft_core.cuh"
@@ -20,8 +21,9 @@ struct RelayoutParams {
 
 template <typename T>
 PF_HD T relayout_value(const T *kuser, const RelayoutParams &q, long long idx) {
-    const int tid = (int)(idx % q.NT);
-    const int r = (int)((idx / q.NT) % q.V);
+    const int kvec = 16 / (int)sizeof(T);
+    const int tid = (int)((idx / kvec) % q.NT);
+    const int r = (int)((idx / ((long long)kvec * q.NT)) % (q.V / kvec)) * kvec + (int)(idx % kvec);
     const long long tile = idx / ((long long)q.NT * q.V);
     int t, p;
     if (q.lanes_p) { p = tid % q.P; t = tid / q.P; } else { t = tid % q.TPP; p = tid / q.TPP; }

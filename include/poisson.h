@@ -109,7 +109,7 @@ POISSON_API int poisson_plan_get_info(const poisson_plan *plan, poisson_plan_inf
  * Asynchronous on `stream`; K_f_dev may be freed once that work has completed. */
 POISSON_API int poisson_set_kernel(poisson_plan *plan, const void *K_f_dev, void *stream);
 
-/* One solve (the 13 steps of PAPER.md:57-71 as 5 fused launches on `stream`).
+/* One solve (the 13 steps of PAPER.md:57-71 as 5 fused launches, or one, on `stream`; see poisson_plan_launch_mode).
  *   rho_dev: device, plan-precision reals [nz][ny][nx], 16-byte aligned, not modified
  *   V_dev  : device, same shape; may equal rho_dev (rho is consumed before V is written)
  * Asynchronous, allocates nothing, never touches host memory.  One plan = one solve in flight
@@ -140,7 +140,20 @@ POISSON_API int poisson_debug_run_passes(poisson_plan *plan, const void *rho_dev
 POISSON_API int poisson_solve_profiled(poisson_plan *plan, const void *rho_dev, void *V_dev, void *stream);
 POISSON_API int poisson_profile_read(poisson_plan *plan, double ms_sum[5] /* host, out */, int *n_solves /* host, out */);
 
-/* Number of kernel launches one poisson_solve enqueues (bench.py's gpu_launches). */
+/* How poisson_solve launches the 13 steps of PAPER.md:57-71:
+ *   FIVE      five fused passes, one launch each;
+ *   FIVE_PDL  the same five launches with programmatic dependent launch (the next pass becomes resident
+ *             while the previous one drains; pays on launch-bound grids);
+ *   FUSED     ONE persistent cooperative launch: F1 | grid barrier | F2 -> F3 -> I2 as a per-plane dataflow
+ *             through L2 | grid barrier | I1 (compiled for the combinations in csrc/fused_*.cu).
+ * poisson_plan_create times the available modes on scratch inputs and keeps the fastest (a few ms);
+ * POISSON_TUNE=0 skips that (FIVE), POISSON_PDL=0|1 and POISSON_FUSED=0|1 force a mode.
+ * poisson_plan_launch_mode reports the choice and the measured milliseconds per solve of
+ * {FIVE, FIVE_PDL, FUSED} (0 where a mode was not measured). */
+enum { POISSON_LAUNCH_FIVE = 0, POISSON_LAUNCH_FIVE_PDL = 1, POISSON_LAUNCH_FUSED = 2 };
+POISSON_API int poisson_plan_launch_mode(const poisson_plan *plan, int *mode /* host, out */, double ms_per_solve[3] /* host, out */);
+
+/* Number of kernel launches one poisson_solve enqueues (bench.py's gpu_launches): 5, or 1 in FUSED mode. */
 POISSON_API int poisson_plan_launches_per_solve(const poisson_plan *plan);
 
 /* Measures the plain-ALU fused-multiply-add peak of the current device for the given precision

@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "poisson_plan_describe", "poisson_plan_create", "poisson_plan_kernel_dims", "poisson_plan_get_info",
     "poisson_set_kernel", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
     "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_measure_fma_peak", "poisson_plan_workspace_bytes",
-    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch",
+    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode",
 )
 
 _PKG = Path(__file__).resolve().parent
@@ -86,6 +86,7 @@ def load_library():
     lib.poisson_profile_read.argtypes = [vp, ctypes.c_double * 5, ctypes.POINTER(i)]
     lib.poisson_measure_fma_peak.argtypes = [i, ctypes.POINTER(ctypes.c_double)]
     lib.poisson_plan_launches_per_solve.argtypes = [vp]
+    lib.poisson_plan_launch_mode.argtypes = [vp, ctypes.POINTER(i), ctypes.c_double * 3]
     lib.poisson_plan_workspace_bytes.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.restype = ctypes.c_size_t
     lib.poisson_plan_destroy.argtypes = [vp]
@@ -211,6 +212,14 @@ class PoissonPlan:
 
     def launches_per_solve(self) -> int:
         return load_library().poisson_plan_launches_per_solve(self._h)
+
+    def launch_mode(self):
+        """(mode name, {mode name: measured ms per solve at plan creation}) -- see poisson_plan_launch_mode."""
+        mode = ctypes.c_int()
+        ms = (ctypes.c_double * 3)()
+        _check(load_library().poisson_plan_launch_mode(self._h, ctypes.byref(mode), ms), "poisson_plan_launch_mode")
+        names = ("five", "five_pdl", "fused")
+        return names[mode.value], {names[k]: ms[k] for k in range(3) if ms[k] > 0}
 
     def workspace_bytes(self) -> int:
         return load_library().poisson_plan_workspace_bytes(self._h)

@@ -14,6 +14,7 @@
 #include "planner.hpp"
 #include "registry.hpp"
 #include "relayout.cuh"
+#include "solve_kernel.cuh"
 
 namespace pfft {
 
@@ -36,6 +37,20 @@ const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int pre
             if (e.variant == 0) fallback = &e;
         }
     return fallback;
+}
+
+std::vector<FusedEntry> &fused_registry() {
+    static std::vector<FusedEntry> reg;
+    return reg;
+}
+
+const FusedEntry *find_fused(int prec, const int S[3], const int pruned[3], const int lanes_p[3]) {
+    for (const FusedEntry &e : fused_registry()) {
+        bool same = e.prec == prec;
+        for (int q = 0; q < 3 && same; ++q) same = e.S[q] == S[q] && e.pruned[q] == pruned[q] && e.lanes_p[q] == lanes_p[q];
+        if (same) return &e;
+    }
+    return nullptr;
 }
 
 static thread_local std::string g_last_error;
@@ -88,6 +103,11 @@ struct poisson_plan {
     void *a1, *a2, *kint;
     void *tw[3];          // per axis id
     void *rho_stage, *v_stage;
+    const FusedEntry *fused;   // one-launch solve kernel compiled for this combination of axes, or NULL
+    bool use_fused;            // launch mode picked for poisson_solve: fused kernel, else 5 launches (with or without PDL)
+    float tune_ms[3];          // measured ms per solve of {5 launches, 5 launches + PDL, fused}; 0 = not measured
+    int fused_grid, fused_skew;
+    unsigned *fused_sync;      // barrier / per-plane counters of the fused kernel (zero between solves)
     size_t elem_real;     // bytes per real
     long long kint_elems;
     size_t workspace_bytes;
@@ -119,7 +139,7 @@ static void free_plan(poisson_plan *pl) {
     if (!pl) return;
     cudaFree(pl->a1); cudaFree(pl->a2); cudaFree(pl->kint);
     for (int q = 0; q < 3; ++q) cudaFree(pl->tw[q]);
-    cudaFree(pl->rho_stage); cudaFree(pl->v_stage);
+    cudaFree(pl->rho_stage); cudaFree(pl->v_stage); cudaFree(pl->fused_sync);
     if (pl->prof_events) {
         for (cudaEvent_t e : *pl->prof_events) cudaEventDestroy(e);
         delete pl->prof_events;
@@ -128,6 +148,8 @@ static void free_plan(poisson_plan *pl) {
 }
 
 extern "C" {
+
+static int tune_plan(poisson_plan *pl);
 
 const char *poisson_status_string(int st) {
     switch (st) {
@@ -188,6 +210,10 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     pl->elem_real = precision == POISSON_FP64 ? 8 : 4;
     // Programmatic dependent launch is opt-in (POISSON_PDL=1): measured on B200 it shortens back-to-back
     // launches of one pass but lengthens the 5-pass solve ("What was tried").
+    // Launch mode: five launches, five launches with programmatic dependent launch, or the one-launch fused
+    // kernel.  Which is fastest depends on the grid (PDL wins on launch-bound grids), so
+    // poisson_plan_create MEASURES the candidates once (tune_plan below) unless POISSON_TUNE=0 or the mode is
+    // forced with POISSON_PDL=0|1 / POISSON_FUSED=0|1.
     { const char *env = std::getenv("POISSON_PDL"); pl->use_pdl = env && env[0] == '1'; }
 
     for (int q = 0; q < 5; ++q) {
@@ -204,6 +230,43 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
         if (ce != cudaSuccess || occ < 1) { free_plan(pl); return cuda_fail(ce, "occupancy query"); }
         const long long resident = (long long)occ * pl->num_sms;
         pl->grid[q] = (int)(pl->n_tiles[q] < resident ? pl->n_tiles[q] : resident);  // persistent CTAs
+    }
+
+    // One-launch fused solve (solve_kernel.cuh) when this combination of axes was compiled and the per-pass
+    // tiles agree with it; POISSON_FUSED=0 keeps the 5-launch path (per-pass experiments).
+    {
+        const char *env = std::getenv("POISSON_FUSED");
+        const bool want = !(env && env[0] == '0');
+        pl->use_fused = env && env[0] == '1';
+        int S3[3], pr3[3], lp3[3];
+        const int qs[3] = {POISSON_PASS_F1, POISSON_PASS_F2, POISSON_PASS_F3};
+        for (int q = 0; q < 3; ++q) { S3[q] = d.pass[qs[q]].S; pr3[q] = d.pass[qs[q]].pruned; lp3[q] = d.pass[qs[q]].lanes_p; }
+        const FusedEntry *fe = want ? find_fused(precision, S3, pr3, lp3) : nullptr;
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        if (fe && coop && fe->P[0] == pl->k[0]->P && fe->P[1] == pl->k[1]->P && fe->P[2] == pl->k[2]->P &&
+            d.pass[1].n_g == d.H && d.pass[2].n_g == d.H) {
+            cudaError_t ce = cudaFuncSetAttribute(fe->func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fe->smem_bytes);
+            int occ = 0;
+            if (ce == cudaSuccess) ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fe->func, fe->NT, fe->smem_bytes);
+            if (ce != cudaSuccess || occ < 1) { free_plan(pl); return cuda_fail(ce, "fused kernel occupancy query"); }
+            const long long resident = (long long)occ * pl->num_sms;
+            const long long per_step = 2LL * pl->tiles_per_g[1] + pl->tiles_per_g[2];
+            long long most = (long long)d.H * per_step;
+            if (pl->n_tiles[0] > most) most = pl->n_tiles[0];
+            pl->fused = fe;
+            pl->fused_grid = (int)(most < resident ? most : resident);
+            // skew D: the first D steps hold F2 tiles only and the last D steps I2 tiles only, so D * T2 >= grid
+            // keeps every CTA busy through ramp-up and drain; it also puts a plane's F3 items several rounds
+            // behind its F2 items, so the per-plane waits are (almost) never taken
+            { const char *envd = std::getenv("POISSON_FUSED_SKEW");
+              pl->fused_skew = envd ? std::atoi(envd) : (pl->fused_grid + pl->tiles_per_g[1] - 1) / pl->tiles_per_g[1] + 1;
+              if (pl->fused_skew < 1) pl->fused_skew = 1; }
+            const size_t sync_bytes = (size_t)(2 + 2 * d.H) * sizeof(unsigned);
+            ce = cudaMalloc(reinterpret_cast<void **>(&pl->fused_sync), sync_bytes);
+            if (ce == cudaSuccess) ce = cudaMemset(pl->fused_sync, 0, sync_bytes);
+            if (ce != cudaSuccess) { free_plan(pl); return cuda_fail(ce, "fused kernel counters"); }
+        }
     }
 
     const size_t cplx = 2 * pl->elem_real;
@@ -226,6 +289,8 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     }
     pl->workspace_bytes = ws;
     pl->d.info.workspace_bytes = (long long)ws;
+    st = tune_plan(pl);
+    if (st != POISSON_OK) { free_plan(pl); return st; }
     *out = pl;
     return POISSON_OK;
 }
@@ -275,7 +340,14 @@ int poisson_plan_get_info(const poisson_plan *pl, poisson_plan_info *info) {
 
 size_t poisson_plan_workspace_bytes(const poisson_plan *pl) { return pl ? pl->workspace_bytes : 0; }
 
-int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? 5 : 0; }
+int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? (pl->fused && pl->use_fused ? 1 : 5) : 0; }
+
+int poisson_plan_launch_mode(const poisson_plan *pl, int *mode, double ms_per_solve[3]) {
+    if (!pl || !mode || !ms_per_solve) return POISSON_EINVAL;
+    *mode = pl->fused && pl->use_fused ? POISSON_LAUNCH_FUSED : (pl->use_pdl ? POISSON_LAUNCH_FIVE_PDL : POISSON_LAUNCH_FIVE);
+    for (int m = 0; m < 3; ++m) ms_per_solve[m] = (double)pl->tune_ms[m];
+    return POISSON_OK;
+}
 
 int poisson_plan_destroy(poisson_plan *pl) {
     if (!pl) return POISSON_EINVAL;
@@ -292,7 +364,6 @@ int poisson_set_kernel(poisson_plan *pl, const void *K_f_dev, void *stream) {
     q.RA = e->RA; q.RB = e->RB; q.TPP = e->TPP; q.P = e->P; q.V = e->V; q.NT = e->NT; q.lanes_p = e->lanes_p;
     q.tiles_per_g = pl->tiles_per_g[2]; q.n_p = (int)d.pass[2].n_p;
     q.a_axis = d.order[0]; q.c_axis = d.order[2];
-    q.ext2y = d.ext2[1];
     q.sx = d.s[0]; q.sy = d.s[1]; q.sz = d.s[2];
     q.total = pl->kint_elems;
     q.scale = 1.0 / ((double)d.s[0] * (double)d.s[1] * (double)d.s[2]);  // reading 2: one 1/(SxSySz)
@@ -309,26 +380,44 @@ int poisson_set_kernel(poisson_plan *pl, const void *K_f_dev, void *stream) {
     return POISSON_OK;
 }
 
+static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, void *V) {
+    const PassDesc &ps = pl->d.pass[q];
+    PassParams prm;
+    switch (q) {
+        case POISSON_PASS_F1: prm.in = rho; prm.out = pl->a1; break;
+        case POISSON_PASS_F2: prm.in = pl->a1; prm.out = pl->a2; break;
+        case POISSON_PASS_F3: prm.in = pl->a2; prm.out = pl->a2; break;
+        case POISSON_PASS_I2: prm.in = pl->a2; prm.out = pl->a1; break;
+        default: prm.in = pl->a1; prm.out = V; break;
+    }
+    prm.kint = pl->kint;
+    prm.tw = pl->tw[ps.axis];
+    prm.gs_in = ps.gs_in; prm.ns_in = ps.ns_in; prm.ps_in = ps.ps_in;
+    prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;
+    prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q];
+    return prm;
+}
+
+// The whole solve as one cooperative launch (solve_kernel.cuh).
+static int run_fused(poisson_plan *pl, const void *rho, void *V, cudaStream_t st) {
+    SolveParams sp;
+    for (int q = 0; q < 5; ++q) sp.pass[q] = pass_params(pl, q, rho, V);
+    sp.sync = pl->fused_sync;
+    sp.n_planes = pl->d.H;
+    sp.t2 = pl->tiles_per_g[1]; sp.t3 = pl->tiles_per_g[2];
+    sp.skew = pl->fused_skew;
+    void *args[] = {&sp};
+    PF_CUDA(cudaLaunchCooperativeKernel(pl->fused->func, dim3(pl->fused_grid), dim3(pl->fused->NT), args,
+                                        pl->fused->smem_bytes, st));
+    return POISSON_OK;
+}
+
 static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t st, int first, int last,
                       cudaEvent_t *ev = nullptr) {
-    const PlanDesc &d = pl->d;
     if (ev) PF_CUDA(cudaEventRecord(ev[0], st));
     for (int q = first; q <= last; ++q) {
-        const PassDesc &ps = d.pass[q];
         const KernelEntry *e = pl->k[q];
-        PassParams prm;
-        switch (q) {
-            case POISSON_PASS_F1: prm.in = rho; prm.out = pl->a1; break;
-            case POISSON_PASS_F2: prm.in = pl->a1; prm.out = pl->a2; break;
-            case POISSON_PASS_F3: prm.in = pl->a2; prm.out = pl->a2; break;
-            case POISSON_PASS_I2: prm.in = pl->a2; prm.out = pl->a1; break;
-            default: prm.in = pl->a1; prm.out = V; break;
-        }
-        prm.kint = pl->kint;
-        prm.tw = pl->tw[ps.axis];
-        prm.gs_in = ps.gs_in; prm.ns_in = ps.ns_in; prm.ps_in = ps.ps_in;
-        prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;
-        prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q];
+        PassParams prm = pass_params(pl, q, rho, V);
         void *args[] = {&prm};
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(pl->grid[q]); cfg.blockDim = dim3(e->NT);
@@ -343,11 +432,53 @@ static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t s
     return POISSON_OK;
 }
 
+static int run_solve(poisson_plan *pl, const void *rho, void *V, cudaStream_t st) {
+    if (pl->fused && pl->use_fused) return run_fused(pl, rho, V, st);
+    return run_passes(pl, rho, V, st, 0, 4);
+}
+
+// Times the launch modes on scratch inputs (timing does not depend on the values) and keeps the fastest.
+static int tune_plan(poisson_plan *pl) {
+    const char *e_tune = std::getenv("POISSON_TUNE"), *e_pdl = std::getenv("POISSON_PDL"), *e_fused = std::getenv("POISSON_FUSED");
+    if ((e_tune && e_tune[0] == '0') || e_pdl || (e_fused && e_fused[0] == '1')) return POISSON_OK;   // forced / off
+    const size_t bytes = (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * pl->elem_real;
+    void *rho = nullptr, *V = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = POISSON_OK;
+    auto cleanup = [&] { cudaFree(rho); cudaFree(V); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); };
+    if (cudaMalloc(&rho, bytes) != cudaSuccess || cudaMalloc(&V, bytes) != cudaSuccess) {   // no room to tune: keep defaults
+        cudaGetLastError(); cleanup(); return POISSON_OK;
+    }
+    cudaMemset(rho, 0, bytes);
+    cudaMemset(pl->kint, 0, (size_t)pl->kint_elems * pl->elem_real);
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { cudaGetLastError(); cleanup(); return POISSON_OK; }
+    const bool modes[3][2] = {{false, false}, {true, false}, {false, true}};   // {pdl, fused}
+    int best = 0; float best_ms = 1e30f;
+    for (int m = 0; m < 3 && rc == POISSON_OK; ++m) {
+        if (modes[m][1] && !pl->fused) continue;
+        pl->use_pdl = modes[m][0]; pl->use_fused = modes[m][1];
+        int reps = 3;
+        for (int round = 0; round < 2 && rc == POISSON_OK; ++round) {   // round 0: warm-up + pick the repeat count
+            cudaEventRecord(e0, 0);
+            for (int i = 0; i < reps && rc == POISSON_OK; ++i) rc = run_solve(pl, rho, V, 0);
+            cudaEventRecord(e1, 0);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = cuda_fail(cudaGetLastError(), "tuning solve"); break; }
+            float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+            ms /= (float)reps;
+            if (round == 0) { reps = (int)(2.0f / (ms > 1e-4f ? ms : 1e-4f)); reps = reps < 3 ? 3 : (reps > 64 ? 64 : reps); }
+            else { pl->tune_ms[m] = ms; if (ms < best_ms) { best_ms = ms; best = m; } }
+        }
+    }
+    pl->use_pdl = modes[best][0]; pl->use_fused = modes[best][1];
+    cleanup();
+    return rc;
+}
+
 int poisson_solve(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stream) {
     if (!pl || !rho_dev || !V_dev) return POISSON_EINVAL;
     if (reinterpret_cast<size_t>(rho_dev) % 16 || reinterpret_cast<size_t>(V_dev) % 16) return POISSON_EINVAL;
     if (!pl->kernel_set) return POISSON_ENOKERNEL;
-    return run_passes(pl, rho_dev, V_dev, reinterpret_cast<cudaStream_t>(stream), 0, 4);
+    return run_solve(pl, rho_dev, V_dev, reinterpret_cast<cudaStream_t>(stream));
 }
 
 int poisson_solve_profiled(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stream) {
@@ -413,7 +544,7 @@ int poisson_solve_host(poisson_plan *pl, const void *rho_host, void *V_host, voi
     }
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     PF_CUDA(cudaMemcpyAsync(pl->rho_stage, rho_host, bytes, cudaMemcpyHostToDevice, st));
-    const int rc = run_passes(pl, pl->rho_stage, pl->v_stage, st, 0, 4);
+    const int rc = run_solve(pl, pl->rho_stage, pl->v_stage, st);
     if (rc != POISSON_OK) return rc;
     PF_CUDA(cudaMemcpyAsync(V_host, pl->v_stage, bytes, cudaMemcpyDeviceToHost, st));
     PF_CUDA(cudaStreamSynchronize(st));

@@ -1,0 +1,3 @@
+// Fused solve kernels (solve_kernel.cuh): PF_FUSED(T, prec, SA, PA, SB, PB, LB, SC, PC, LC, MINB), see fused_inst.cuh.
+#define PF_FUSED_LIST PF_FUSED(float,1,8,1,8,1,1,8,1,0,0) PF_FUSED(float,1,32,1,32,1,1,32,1,0,0) PF_FUSED(float,1,64,1,64,1,1,64,1,0,0)
+#include "fused_inst.cuh"

@@ -418,21 +418,7 @@ PF_HD void stage_issue(cx<typename G::T> *stage, const cx<typename G::T> *src, l
     }
 }
 
-// ------------------------------------------------------------------ pass bodies
-#define PF_BODY_PROLOGUE(NEED_A, NEED_B, KIND)                                                        \
-    using T = typename G::T;                                                                          \
-    using St = Stage<G, PRUNED, KIND>;                                                                \
-    int t, p; G::split(tid, t, p);                                                                    \
-    cx<T> *smem_c = reinterpret_cast<cx<T> *>(smem);                                                  \
-    XBufs<G> xbufs(smem_c);                                                                           \
-    cx<T> *stage = smem_c + G::NBUF * G::XELEMS + G::TW_ELEMS;                                        \
-    const unsigned long long pol = St::ON ? evict_first_policy() : 0ull;                              \
-    (void)stage; (void)pol;                                                                           \
-    Twiddles<G> tw;                                                                                   \
-    pdl_launch_dependents();                                                                          \
-    tw.template init<NEED_A, NEED_B>(reinterpret_cast<const cx<T> *>(prm.tw), smem_c + G::NBUF * G::XELEMS, tid, t); \
-    pdl_wait_prior_grid();
-
+// ------------------------------------------------------------------ tiles
 // Persistent tile loop.  issue(tile): start the asynchronous copies of a tile (staged mode only);
 // after_first(): hook after the very first issue; fetch(buf, tile): tile -> registers (from the stage,
 // or straight from global memory when not staged); process(buf, tile): transform and store.
@@ -518,12 +504,182 @@ PF_HD void unpack_A(cx<typename G::T> *v, const B &b) {
     const bool valid = pp < prm.n_p;                                                     \
     (void)p0; (void)valid;
 
+// ---- per-tile work, shared by the one-pass kernels below and the fused solve kernel (solve_kernel.cuh).
+// fetch_*: one tile, global memory -> registers.  process_*: transform the tile and store it.
+template <class G> struct TileCtx {          // what a tile function needs besides the pass parameters
+    int tid, t, p;
+    XBufs<G> xbufs;
+    Twiddles<G> tw;
+    PF_HD TileCtx(int tid_, cx<typename G::T> *xbase) : tid(tid_), xbufs(xbase) { G::split(tid_, t, p); }
+};
+
+template <class G, bool PRUNED, bool STREAM, class Buf>
+PF_HD void fetch_fwd(Buf &b, const PassParams &prm, int tile, const TileCtx<G> &c) {   // F1 / F2 / F3 inputs (layout A)
+    using T = typename G::T;
+    const int t = c.t, p = c.p;
+    PF_TILE_COORDS
+    issue_A<G, PRUNED, STREAM>(b, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+}
+template <class G>
+PF_HD void fetch_i2(BufB<G> &b, const PassParams &prm, int tile, const TileCtx<G> &c) {
+    using T = typename G::T;
+    const int t = c.t, p = c.p;
+    PF_TILE_COORDS
+    load_B<G, true>(b.x, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);  // last read of A2
+}
+// I1 inputs: Z_k = A_k + i B_k rebuilt from the half spectra of the two packed pencils
+// (Z_{S-k} = conj A_k + i conj B_k); ld(col, kk) returns element kk of pencil 2*pp + col.
+template <class G, class Ld>
+PF_HD void fetch_i1_with(BufB<G> &b, int t, bool valid, Ld &&ld) {
+    using T = typename G::T;
+    constexpr int S = G::S;
+    static_for<G::CB>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        static_for<G::RB>([&](auto kc) {
+            constexpr int k1 = decltype(kc)::value;
+            const int k = (t + G::TPP * i) + G::RA * k1;
+            const bool lower = k <= S / 2;
+            const int kk = lower ? k : S - k;
+            cx<T> a = mk<T>((T)0, (T)0), bb = a;
+            if (valid) { a = ld(0, kk); bb = ld(1, kk); }
+            b.x[i * G::RB + k1] = lower ? mk<T>(a.re - bb.im, a.im + bb.re) : mk<T>(a.re + bb.im, bb.re - a.im);
+        });
+    });
+}
+template <class G>
+PF_HD void fetch_i1(BufB<G> &b, const PassParams &prm, int tile, const TileCtx<G> &c) {
+    using T = typename G::T;
+    const int t = c.t, p = c.p;
+    PF_TILE_COORDS
+    const cx<T> *src = reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + 2 * pp * prm.ps_in;
+    fetch_i1_with<G>(b, t, valid, [&](int col, int kk) { return ld_stream(src + kk * prm.ns_in + col * prm.ps_in); });
+}
+
 // F2: (transpose +) spread + 1D FFT along axis b
+template <class G, bool PRUNED>
+PF_HD void process_f2(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileCtx<G> &c) {
+    using T = typename G::T;
+    const int t = c.t, p = c.p;
+    PF_TILE_COORDS
+    cx<T> v[G::V];
+    unpack_A<G, PRUNED>(v, b);
+    fwd_AtoB<G, PRUNED>(v, c.tw, c.xbufs.next(), t, p);
+    store_B<G>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+}
+// I2: inverse 1D FFT along axis b + compactification (+ transpose)      (PAPER.md:68-69)
+template <class G, bool PRUNED>
+PF_HD void process_i2(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c) {
+    using T = typename G::T;
+    const int t = c.t, p = c.p;
+    PF_TILE_COORDS
+    inv_BtoA<G, PRUNED>(b.x, c.tw, c.xbufs.next(), t, p);
+    store_A<G, PRUNED>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+}
+// F3: spread + 1D FFT along axis c, K^F multiply (Eq. 3, PAPER.md:41), inverse 1D FFT along c,
+// compactification; in place over the tile it read.  kmul(v) multiplies the V
+// spectrum values of this thread by their K^F entries.
+template <class G, bool PRUNED, class Buf, class KMul>
+PF_HD void process_f3(Buf &b, const PassParams &prm, int tile, TileCtx<G> &c, KMul &&kmul) {
+    using T = typename G::T;
+    const int t = c.t, p = c.p;
+    PF_TILE_COORDS
+    cx<T> v[G::V];
+    unpack_A<G, PRUNED>(v, b);
+    fwd_AtoB<G, PRUNED>(v, c.tw, c.xbufs.next(), t, p);
+    kmul(v);
+    inv_BtoA<G, PRUNED>(v, c.tw, c.xbufs.next(), t, p);
+    store_A<G, PRUNED>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+}
+// K^F of one tile: internal order [tile][V/KVEC][NT][KVEC] (relayout.cuh), 16-byte vectors per thread
+template <class G, class VT>
+PF_HD void kmul_vectors(cx<typename G::T> *v, const VT *kp /* vector 0 of this thread */) {
+    using T = typename G::T;
+    using KV = KVec<T>;
+    static_assert(G::V % KV::N == 0, "values per thread must fill whole K^F vectors");
+    static_for<G::V / KV::N>([&](auto qc) {
+        constexpr int q = decltype(qc)::value;
+        T kk[KV::N]; kvec_get(kp[(size_t)q * G::NT], kk);
+        static_for<KV::N>([&](auto jc) { constexpr int j = decltype(jc)::value; v[q * KV::N + j] = scale(v[q * KV::N + j], kk[j]); });
+    });
+}
+template <class G>
+PF_HD void kmul_global(cx<typename G::T> *v, const void *kint, int tile, int tid) {   // streamed straight from global memory
+    using T = typename G::T;
+    using KV = KVec<T>;
+    const typename KV::V *kp = reinterpret_cast<const typename KV::V *>(kint) + (size_t)tile * (G::V / KV::N) * G::NT + tid;
+    static_for<G::V / KV::N>([&](auto qc) {
+        constexpr int q = decltype(qc)::value;
+        T kk[KV::N]; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), kk);
+        static_for<KV::N>([&](auto jc) { constexpr int j = decltype(jc)::value; v[q * KV::N + j] = scale(v[q * KV::N + j], kk[j]); });
+    });
+}
+// F1: spread + 1D FFT (R2C) along axis a                  (PAPER.md:55,59-60)
+// Two real pencils adjacent along x are transformed as ONE complex pencil z = rho(2q) + i rho(2q+1)
+// (the real array read as complex IS that packing) and separated with the Hermitian symmetry
+// F_{S-k} = conj(F_k) of PAPER.md:55; only k = 0..S/2 is kept.  in: pairs, out: complex.
+template <class G, bool PRUNED>
+PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileCtx<G> &c) {
+    static_assert(G::LANES_P, "the R2C pass runs on a strided axis");
+    using T = typename G::T;
+    constexpr int S = G::S, NK = S / 2 + 1, NM = (NK + G::TPP - 1) / G::TPP;
+    const int t = c.t, p = c.p;
+    PF_TILE_COORDS
+    cx<T> v[G::V];
+    unpack_A<G, PRUNED>(v, b);
+    fwd_AtoB<G, PRUNED>(v, c.tw, c.xbufs.next(), t, p);
+    cx<T> *xn = c.xbufs.next();
+    static_for<G::CB>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        static_for<G::RB>([&](auto kc) {
+            constexpr int k1 = decltype(kc)::value;
+            xn[G::nidx(p, (t + G::TPP * i) + G::RA * k1)] = v[i * G::RB + k1];
+        });
+    });
+    cta_sync();
+    cx<T> *dst = reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + 2 * pp * prm.ps_out;
+    static_for<NM>([&](auto mc) {
+        constexpr int m = decltype(mc)::value;
+        const int k = t + G::TPP * m;
+        if (k < NK && valid) {
+            const cx<T> zk = xn[G::nidx(p, k)], zp = xn[G::nidx(p, (S - k) % S)];
+            const T hf = (T)0.5;
+            // A = (Z_k + conj Z_{S-k})/2 ; B = -i (Z_k - conj Z_{S-k})/2
+            dst[k * prm.ns_out] = mk<T>(hf * (zk.re + zp.re), hf * (zk.im - zp.im));
+            dst[k * prm.ns_out + prm.ps_out] = mk<T>(hf * (zk.im + zp.im), hf * (zp.re - zk.re));
+        }
+    });
+}
+// I1: inverse 1D FFT (C2R) along axis a + compactification      (PAPER.md:55,70-71)
+// one complex inverse transform, real part -> pencil 2q, imaginary part -> pencil 2q+1.
+template <class G, bool PRUNED>
+PF_HD void process_i1(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c) {
+    static_assert(G::LANES_P, "the C2R pass runs on a strided axis");
+    using T = typename G::T;
+    const int t = c.t, p = c.p;
+    PF_TILE_COORDS
+    inv_BtoA<G, PRUNED>(b.x, c.tw, c.xbufs.next(), t, p);
+    store_A<G, PRUNED, true>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+}
+
+// ------------------------------------------------------------------ one pass per launch
+#define PF_BODY_PROLOGUE(NEED_A, NEED_B, KIND)                                                        \
+    using T = typename G::T;                                                                          \
+    using St = Stage<G, PRUNED, KIND>;                                                                \
+    cx<T> *smem_c = reinterpret_cast<cx<T> *>(smem);                                                  \
+    TileCtx<G> c(tid, smem_c);                                                                        \
+    const int t = c.t, p = c.p;                                                                       \
+    cx<T> *stage = smem_c + G::NBUF * G::XELEMS + G::TW_ELEMS;                                        \
+    const unsigned long long pol = St::ON ? evict_first_policy() : 0ull;                              \
+    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);                                        \
+    (void)stage; (void)pol; (void)in; (void)t; (void)p;                                               \
+    pdl_launch_dependents();                                                                          \
+    c.tw.template init<NEED_A, NEED_B>(reinterpret_cast<const cx<T> *>(prm.tw), smem_c + G::NBUF * G::XELEMS, tid, c.t); \
+    pdl_wait_prior_grid();
+
 template <class G, bool PRUNED>
 PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     PF_BODY_PROLOGUE(true, false, KIND_F2)
     using Buf = BufA<G, PRUNED>;
-    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS
@@ -531,26 +687,19 @@ PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [] {},
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
-            if constexpr (St::ON) fetch_A<G, PRUNED, St>(b, stage, t, p, valid);
-            else issue_A<G, PRUNED, true>(b, in + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+            if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
+            else fetch_fwd<G, PRUNED, true>(b, prm, tile, c);
         },
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
-            cx<T> v[G::V];
-            unpack_A<G, PRUNED>(v, b);
-            if constexpr (St::ON) xbufs.dirty = false;   // the loop's barriers already separate the tiles
-            fwd_AtoB<G, PRUNED>(v, tw, xbufs.next(), t, p);
-            store_B<G>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+            if constexpr (St::ON) c.xbufs.dirty = false;   // the loop's barriers already separate the tiles
+            process_f2<G, PRUNED>(b, prm, tile, c);
         });
 }
 
-// I2: inverse 1D FFT along axis b + compactification (+ transpose)      (PAPER.md:68-69)
 template <class G, bool PRUNED>
 PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     PF_BODY_PROLOGUE(false, true, KIND_I2)
     using Buf = BufB<G>;
-    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS
@@ -558,8 +707,8 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [] {},
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
             if constexpr (St::ON) {
+                PF_TILE_COORDS
                 static_for<G::CB>([&](auto ic) {
                     constexpr int i = decltype(ic)::value;
                     static_for<G::RB>([&](auto kc) {
@@ -569,29 +718,22 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
                     });
                 });
             } else {
-                load_B<G, true>(b.x, in + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+                fetch_i2<G>(b, prm, tile, c);
             }
         },
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
-            if constexpr (St::ON) xbufs.dirty = false;
-            inv_BtoA<G, PRUNED>(b.x, tw, xbufs.next(), t, p);
-            store_A<G, PRUNED>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+            if constexpr (St::ON) c.xbufs.dirty = false;
+            process_i2<G, PRUNED>(b, prm, tile, c);
         });
 }
 
-// F3: spread + 1D FFT along axis c, K^F multiply (Eq. 3, PAPER.md:41), inverse 1D FFT along c,
-// compactification; in place over the tile it read.
-// K^F: internal order [tile][V/KVEC][NT][KVEC] (relayout.cuh), 16-byte vectors per thread.
 template <class G, bool PRUNED>
 PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     PF_BODY_PROLOGUE(true, true, KIND_F3)
     using KV = KVec<T>;
     constexpr int NKV = G::V / KV::N;
-    static_assert(G::V % KV::N == 0, "values per thread must fill whole K^F vectors");
     constexpr bool K_EARLY = !St::KON && !G::KLATE;
     using Buf = BufAK<G, PRUNED, K_EARLY>;
-    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
     const typename KV::V *kint = reinterpret_cast<const typename KV::V *>(prm.kint);
     typename KV::V *kstage = reinterpret_cast<typename KV::V *>(stage + St::IN_ELEMS);
     (void)kstage;
@@ -608,55 +750,34 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             if constexpr (St::KON) { if (bid < prm.n_tiles) issue_k(bid); cp_async_commit(); }
         },
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
-            if constexpr (St::ON) fetch_A<G, PRUNED, St>(b, stage, t, p, valid);
-            else issue_A<G, PRUNED, false>(b, in + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+            if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
+            else fetch_fwd<G, PRUNED, false>(b, prm, tile, c);
             if constexpr (K_EARLY) {
                 const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
                 static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), b.k + q * KV::N); });
             }
         },
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
-            cx<T> v[G::V];
-            unpack_A<G, PRUNED>(v, b);
-            if constexpr (St::ON) xbufs.dirty = false;
-            fwd_AtoB<G, PRUNED>(v, tw, xbufs.next(), t, p);
-            if constexpr (St::KON) {
-                cp_async_wait<1>();      // everything but the next tile's inputs: this tile's K^F (own copies only)
-                static_for<NKV>([&](auto qc) {
-                    constexpr int q = decltype(qc)::value;
-                    T kk[KV::N]; kvec_get(kstage[q * G::NT + tid], kk);
-                    static_for<KV::N>([&](auto jc) { constexpr int j = decltype(jc)::value; v[q * KV::N + j] = scale(v[q * KV::N + j], kk[j]); });
-                });
-                if (tile + nb < prm.n_tiles) issue_k(tile + nb);
-                cp_async_commit();
-            } else if constexpr (G::KLATE) {
-                const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
-                static_for<NKV>([&](auto qc) {
-                    constexpr int q = decltype(qc)::value;
-                    T kk[KV::N]; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), kk);
-                    static_for<KV::N>([&](auto jc) { constexpr int j = decltype(jc)::value; v[q * KV::N + j] = scale(v[q * KV::N + j], kk[j]); });
-                });
-            } else {
-                static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], b.k[r]); });
-            }
-            inv_BtoA<G, PRUNED>(v, tw, xbufs.next(), t, p);
-            store_A<G, PRUNED>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+            if constexpr (St::ON) c.xbufs.dirty = false;
+            process_f3<G, PRUNED>(b, prm, tile, c, [&](cx<T> *v) {
+                if constexpr (St::KON) {
+                    cp_async_wait<1>();      // everything but the next tile's inputs: this tile's K^F (own copies only)
+                    kmul_vectors<G>(v, kstage + tid);
+                    if (tile + nb < prm.n_tiles) issue_k(tile + nb);
+                    cp_async_commit();
+                } else if constexpr (G::KLATE) {
+                    kmul_global<G>(v, prm.kint, tile, tid);
+                } else {
+                    static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], b.k[r]); });
+                }
+            });
         });
 }
 
-// F1: spread + 1D FFT (R2C) along axis a                  (PAPER.md:55,59-60)
-// Two real pencils adjacent along x are transformed as ONE complex pencil z = rho(2q) + i rho(2q+1)
-// (the real array read as complex IS that packing) and separated with the Hermitian symmetry
-// F_{S-k} = conj(F_k) of PAPER.md:55; only k = 0..S/2 is kept.  in: pairs, out: complex.
 template <class G, bool PRUNED>
 PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    static_assert(G::LANES_P, "the R2C pass runs on a strided axis");
     PF_BODY_PROLOGUE(true, false, KIND_F1)
-    constexpr int S = G::S, NK = S / 2 + 1, NM = (NK + G::TPP - 1) / G::TPP;
     using Buf = BufA<G, PRUNED>;
-    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS
@@ -664,50 +785,19 @@ PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [] {},
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
-            if constexpr (St::ON) fetch_A<G, PRUNED, St>(b, stage, t, p, valid);
-            else issue_A<G, PRUNED, true>(b, in + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+            if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
+            else fetch_fwd<G, PRUNED, true>(b, prm, tile, c);
         },
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
-            cx<T> v[G::V];
-            unpack_A<G, PRUNED>(v, b);
-            if constexpr (St::ON) xbufs.dirty = false;
-            fwd_AtoB<G, PRUNED>(v, tw, xbufs.next(), t, p);
-            cx<T> *xn = xbufs.next();
-            static_for<G::CB>([&](auto ic) {
-                constexpr int i = decltype(ic)::value;
-                static_for<G::RB>([&](auto kc) {
-                    constexpr int k1 = decltype(kc)::value;
-                    xn[G::nidx(p, (t + G::TPP * i) + G::RA * k1)] = v[i * G::RB + k1];
-                });
-            });
-            cta_sync();
-            cx<T> *dst = reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + 2 * pp * prm.ps_out;
-            static_for<NM>([&](auto mc) {
-                constexpr int m = decltype(mc)::value;
-                const int k = t + G::TPP * m;
-                if (k < NK && valid) {
-                    const cx<T> zk = xn[G::nidx(p, k)], zp = xn[G::nidx(p, (S - k) % S)];
-                    const T hf = (T)0.5;
-                    // A = (Z_k + conj Z_{S-k})/2 ; B = -i (Z_k - conj Z_{S-k})/2
-                    dst[k * prm.ns_out] = mk<T>(hf * (zk.re + zp.re), hf * (zk.im - zp.im));
-                    dst[k * prm.ns_out + prm.ps_out] = mk<T>(hf * (zk.im + zp.im), hf * (zp.re - zk.re));
-                }
-            });
+            if constexpr (St::ON) c.xbufs.dirty = false;
+            process_f1<G, PRUNED>(b, prm, tile, c);
         });
 }
 
-// I1: inverse 1D FFT (C2R) along axis a + compactification      (PAPER.md:55,70-71)
-// Z_k = A_k + i B_k rebuilt from the half spectra of the two packed pencils (Z_{S-k} = conj A_k + i conj B_k),
-// one complex inverse transform, real part -> pencil 2q, imaginary part -> pencil 2q+1.
 template <class G, bool PRUNED>
 PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) {
-    static_assert(G::LANES_P, "the C2R pass runs on a strided axis");
     PF_BODY_PROLOGUE(false, true, KIND_I1)
-    constexpr int S = G::S;
     using Buf = BufB<G>;
-    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS   // stage rows: kk = 0..S/2, columns: the 2 P complex pencils of the P pairs
@@ -715,29 +805,16 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [] {},
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
-            const cx<T> *src = in + g * prm.gs_in + 2 * pp * prm.ps_in;
-            static_for<G::CB>([&](auto ic) {
-                constexpr int i = decltype(ic)::value;
-                static_for<G::RB>([&](auto kc) {
-                    constexpr int k1 = decltype(kc)::value;
-                    const int k = (t + G::TPP * i) + G::RA * k1;
-                    const bool lower = k <= S / 2;
-                    const int kk = lower ? k : S - k;
-                    cx<T> a = mk<T>((T)0, (T)0), bb = a;
-                    if (valid) {
-                        if constexpr (St::ON) { a = stage[St::idx(2 * p, kk)]; bb = stage[St::idx(2 * p + 1, kk)]; }
-                        else { a = ld_stream(src + kk * prm.ns_in); bb = ld_stream(src + kk * prm.ns_in + prm.ps_in); }
-                    }
-                    b.x[i * G::RB + k1] = lower ? mk<T>(a.re - bb.im, a.im + bb.re) : mk<T>(a.re + bb.im, bb.re - a.im);
-                });
-            });
+            if constexpr (St::ON) {
+                PF_TILE_COORDS
+                fetch_i1_with<G>(b, t, valid, [&](int col, int kk) { return stage[St::idx(2 * p + col, kk)]; });
+            } else {
+                fetch_i1<G>(b, prm, tile, c);
+            }
         },
         [&](Buf &b, int tile) {
-            PF_TILE_COORDS
-            if constexpr (St::ON) xbufs.dirty = false;
-            inv_BtoA<G, PRUNED>(b.x, tw, xbufs.next(), t, p);
-            store_A<G, PRUNED, true>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+            if constexpr (St::ON) c.xbufs.dirty = false;
+            process_i1<G, PRUNED>(b, prm, tile, c);
         });
 }
 

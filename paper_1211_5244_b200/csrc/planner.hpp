@@ -90,10 +90,11 @@ inline int plan_build(int nx, int ny, int nz, const int bc_in[3], int prec, Plan
 
     // F2 / I2: axis b
     PassDesc f2{}; f2.kind = POISSON_PASS_F2; f2.axis = b; f2.S = d.s[b]; f2.pruned = !per(b);
-    if (b == 0) {
-        f2.lanes_p = 0; f2.n_g = 1; f2.n_p = d.ext1[1] * d.ext1[2];
-        f2.gs_in = 0; f2.ns_in = 1; f2.ps_in = d.ext1[0];
-        f2.gs_out = 0; f2.ns_out = 1; f2.ps_out = d.ext2[0];
+    // every middle pass works plane by plane: g = k_a (n_g = H), so that F3 / I2 of a plane depend on that plane only
+    if (b == 0) {   // contiguous pencils along x, one per point of the remaining axis c
+        f2.lanes_p = 0; f2.n_g = d.H; f2.n_p = d.ext1[c];
+        f2.gs_in = stride(d.ext1, a); f2.ns_in = 1; f2.ps_in = stride(d.ext1, c);
+        f2.gs_out = stride(d.ext2, a); f2.ns_out = 1; f2.ps_out = stride(d.ext2, c);
     } else {
         f2.lanes_p = 1; f2.n_g = d.H; f2.n_p = d.ext1[0];
         f2.gs_in = stride(d.ext1, a); f2.ns_in = stride(d.ext1, b); f2.ps_in = 1;
@@ -105,9 +106,9 @@ inline int plan_build(int nx, int ny, int nz, const int bc_in[3], int prec, Plan
 
     // F3: axis c, in place on A2
     PassDesc f3{}; f3.kind = POISSON_PASS_F3; f3.axis = c; f3.S = d.s[c]; f3.pruned = !per(c);
-    if (c == 0) {
-        f3.lanes_p = 0; f3.n_g = 1; f3.n_p = d.ext2[1] * d.ext2[2];
-        f3.gs_in = 0; f3.ns_in = 1; f3.ps_in = d.ext2[0];
+    if (c == 0) {   // contiguous pencils along x, one per point of axis b (already at its padded length S_b)
+        f3.lanes_p = 0; f3.n_g = d.H; f3.n_p = d.ext2[b];
+        f3.gs_in = stride(d.ext2, a); f3.ns_in = 1; f3.ps_in = stride(d.ext2, b);
     } else {
         f3.lanes_p = 1; f3.n_g = d.H; f3.n_p = d.ext2[0];
         f3.gs_in = stride(d.ext2, a); f3.ns_in = stride(d.ext2, c); f3.ps_in = 1;

@@ -23,7 +23,19 @@ struct KernelEntry {
     const void *func;  // __global__ void (*)(PassParams)
 };
 
+// A fused solve kernel (solve_kernel.cuh): all five passes of one (axis a, axis b, axis c) combination.
+struct FusedEntry {
+    int prec;
+    int S[3], pruned[3], lanes_p[3];   // per processed axis a, b, c
+    int P[3];                          // pencils per tile of F1/I1, F2/I2, F3
+    int NT, minb;
+    size_t smem_bytes;
+    const void *func;                  // __global__ void (*)(SolveParams)
+};
+
 std::vector<KernelEntry> &kernel_registry();
+std::vector<FusedEntry> &fused_registry();
+const FusedEntry *find_fused(int prec, const int S[3], const int pruned[3], const int lanes_p[3]);
 const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int prec, int variant = -1);
 bool length_supported(int S);
 

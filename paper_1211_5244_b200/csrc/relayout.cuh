@@ -12,8 +12,7 @@ namespace pfft {
 struct RelayoutParams {
     int RA, RB, TPP, P, V, NT, lanes_p;
     int tiles_per_g, n_p;
-    int a_axis, c_axis;
-    long long ext2y;
+    int a_axis, c_axis;   // the pencil index pp runs along the remaining axis
     int sx, sy, sz;
     long long total;
     double scale;  // 1/(S_x S_y S_z)
@@ -33,8 +32,7 @@ PF_HD T relayout_value(const T *kuser, const RelayoutParams &q, long long idx) {
     const int i = r / q.RB, k1 = r % q.RB;
     const int kc = (t + q.TPP * i) + q.RA * k1;  // layout B of passes.cuh: k = k2 + RA*k1
     long long f[3];
-    if (!q.lanes_p) { f[0] = kc; f[1] = pp % q.ext2y; f[2] = pp / q.ext2y; }
-    else { f[0] = pp; f[q.c_axis] = kc; f[q.a_axis] = g; }
+    f[3 - q.a_axis - q.c_axis] = pp; f[q.c_axis] = kc; f[q.a_axis] = g;
     long long kx = f[0], ky = f[1], kz = f[2];
     const int hx = q.sx / 2 + 1;
     if (kx > q.sx / 2) {  // K^F(-k) = K^F(k): the half the caller did not pass

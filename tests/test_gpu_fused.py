@@ -1,0 +1,104 @@
+"""The one-launch fused solve kernel (csrc/solve_kernel.cuh: F1 | F2 -> F3 -> I2 per plane | I1 in one
+cooperative launch) against the CPU oracle, and against the 5-launch path on the same inputs."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import generators as gen
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pk():
+    import torch
+    import paper_1211_5244_b200 as pk
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; the solve has no fallback")
+    pk.load_library()
+    torch.cuda.set_device(0)
+    return pk
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def _even_kernel(rng, s):
+    sx, sy, sz = s
+    K = rng.standard_normal((sz, sy, sx))
+    for ax in range(3):
+        K = 0.5 * (K + np.roll(np.flip(K, axis=ax), 1, axis=ax))
+    return K
+
+
+def _solve(pk, rho, Kf, n, bc, prec, fused, repeats=1):
+    import torch
+    dt = np.float64 if prec == "fp64" else np.float32
+    old = os.environ.get("POISSON_FUSED")
+    os.environ["POISSON_FUSED"] = "1" if fused else "0"
+    try:
+        plan = pk.PoissonPlan(n, bc, 0.25, pk.FP64 if prec == "fp64" else pk.FP32)
+    finally:
+        if old is None:
+            del os.environ["POISSON_FUSED"]
+        else:
+            os.environ["POISSON_FUSED"] = old
+    try:
+        assert plan.launches_per_solve() == (1 if fused else 5)
+        plan.set_kernel(torch.from_numpy(np.ascontiguousarray(Kf.astype(dt))).cuda())
+        r = torch.from_numpy(np.ascontiguousarray(rho.astype(dt))).cuda()
+        outs = []
+        for _ in range(repeats):   # back-to-back solves: the kernel must re-arm its own counters
+            outs.append(plan.solve(r))
+        torch.cuda.synchronize()
+        return [o.cpu().numpy().astype(np.float64) for o in outs]
+    finally:
+        plan.close()
+
+
+# (n, bc, precisions): combinations with a compiled fused kernel (csrc/fused_*.cu)
+FUSED_CASES = [
+    ((4, 4, 4), (0, 0, 0), ("fp64", "fp32")),
+    ((8, 8, 8), (0, 0, 0), ("fp64",)),
+    ((16, 16, 16), (1, 1, 1), ("fp64",)),
+    ((16, 16, 16), (0, 0, 0), ("fp64", "fp32")),
+    ((6, 24, 12), (0, 0, 0), ("fp64",)),          # three different lengths 12 / 48 / 24, ragged tiles
+    ((32, 32, 32), (0, 0, 0), ("fp64", "fp32")),
+]
+
+
+@pytest.mark.parametrize("n,bc,precs", FUSED_CASES, ids=lambda v: "x".join(map(str, v)) if isinstance(v, tuple) and isinstance(v[0], int) else None)
+def test_fused_kernel_vs_oracle_and_vs_five_launches(pk, n, bc, precs):
+    rng = np.random.default_rng(77 + sum(n))
+    s = gen.padded_shape(n, bc)
+    rho = rng.standard_normal((n[2], n[1], n[0]))
+    Kf = oracle.kernel_spectrum(_even_kernel(rng, s))
+    for prec in precs:
+        tol = 1e-12 if prec == "fp64" else 1e-5
+        if prec == "fp32":
+            r_in, k_in = rho.astype(np.float32).astype(np.float64), Kf.astype(np.float32).astype(np.float64)
+        else:
+            r_in, k_in = rho, Kf
+        ref = oracle.solve(r_in, k_in, bc)
+        outs = _solve(pk, rho, Kf, n, bc, prec, fused=True, repeats=3)
+        for V in outs:
+            assert rel_l2(V, ref) <= tol, (n, bc, prec)
+        assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])   # bitwise repeatable
+        five = _solve(pk, rho, Kf, n, bc, prec, fused=False)[0]
+        # same butterflies, but two separately compiled kernels may contract multiply-adds differently
+        assert rel_l2(outs[0], five) <= (1e-14 if prec == "fp64" else 1e-6)
+
+
+@pytest.mark.parametrize("key", ["c0", "c1", "c2", "c3"])
+def test_named_configs_run_fused(pk, key):
+    """configs[0..3] take the one-launch path, and it matches the oracle."""
+    cfg = gen.get_config(key)
+    rho = gen.gaussian_density(cfg)
+    K = gen.green_kernel_realspace(cfg.n, cfg.bc, cfg.h, cfg.images)
+    Kf = oracle.kernel_spectrum(K)
+    V = _solve(pk, rho, Kf, cfg.n, cfg.bc, "fp64", fused=True, repeats=2)
+    ref = oracle.solve(rho, Kf, cfg.bc)
+    assert rel_l2(V[0], ref) <= 1e-12 and np.array_equal(V[0], V[1])

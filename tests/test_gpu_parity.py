@@ -212,7 +212,7 @@ def test_in_place_determinism_linearity_and_host_entry(pk):
     vh = torch.empty_like(rh).pin_memory()
     plan.solve_host(rh, vh)
     assert np.array_equal(vh.numpy(), V1)
-    assert plan.launches_per_solve() == 5
+    assert plan.launches_per_solve() in (1, 5)                       # 1: the fused one-launch kernel
     plan.close()
 
 

@@ -122,6 +122,30 @@ POISSON_API int poisson_solve(poisson_plan *plan, const void *rho_dev, void *V_d
  * The plan owns the two device staging buffers (allocated on first use). */
 POISSON_API int poisson_solve_host(poisson_plan *plan, const void *rho_host, void *V_host, void *stream);
 
+/* Batched solves: `count` densities with the one K^F of the plan -- the paper's repeated-solve setting and its
+ * stated remedy for the transfer cost, "overlap the transfer of one density with the computation of the
+ * previous one".  The solves are dealt round-robin to up to 3 lanes (1 for device batches whose
+ * intermediates exceed 256 MB per lane; POISSON_LANES=1..8 overrides),
+ * each with its own A1 / A2 intermediates and its own internal stream, so that the tail of one solve overlaps
+ * the head of the next (and, in the host variant, H2D of solve i+1 and D2H of solve i-1 overlap the passes of
+ * solve i on the two copy engines).  Lanes are allocated on first use and kept by the plan (its
+ * workspace_bytes grows accordingly).  Always five launches per solve (the cooperative fused kernel cannot
+ * overlap with itself).
+ *   rho / V : host arrays of `count` pointers; poisson_solve_batch: device buffers as in poisson_solve
+ *             (rho[i] == V[i] allowed; the V[i] must not overlap each other or any other rho[j]);
+ *             poisson_solve_batch_host: host buffers (pinned for overlap), [nz][ny][nx] reals each.
+ * poisson_solve_batch is asynchronous: the lanes start after the work already queued on `stream`, and work
+ * queued on `stream` afterwards starts after every solve of the batch.  poisson_solve_batch_host returns
+ * after the last V has arrived on the host.  A plan runs ONE call at a time.
+ * Errors: EINVAL (null / misaligned pointer, count < 0), ENOKERNEL, ENOMEM, ECUDA. */
+POISSON_API int poisson_solve_batch(poisson_plan *plan, const void *const *rho_dev /* host array of device ptrs */,
+                        void *const *V_dev /* host array of device ptrs */, int count, void *stream);
+POISSON_API int poisson_solve_batch_host(poisson_plan *plan, const void *const *rho_host /* host array of host ptrs */,
+                             void *const *V_host /* host array of host ptrs */, int count, void *stream);
+/* Lanes a batch of `count` solves would use (host != 0: the host variant); 0 on a null plan or count <= 0.
+ * With one lane a device batch is poisson_solve in a loop (same launch mode). */
+POISSON_API int poisson_plan_batch_lanes(const poisson_plan *plan, int count, int host);
+
 /* Debug/test access to the plan's intermediates (per-pass parity).  which = 0: A1,
  * complex [.][.][.] after F1 (or after I2); which = 1: A2 after F2 / F3.  dims are the array
  * extents in memory order (z-extent, y-extent, x-extent), each axis holding N_i, S_i or H. */

@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "poisson_plan_describe", "poisson_plan_create", "poisson_plan_kernel_dims", "poisson_plan_get_info",
     "poisson_set_kernel", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
     "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_measure_fma_peak", "poisson_plan_workspace_bytes",
-    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode",
+    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes",
 )
 
 _PKG = Path(__file__).resolve().parent
@@ -86,6 +86,9 @@ def load_library():
     lib.poisson_profile_read.argtypes = [vp, ctypes.c_double * 5, ctypes.POINTER(i)]
     lib.poisson_measure_fma_peak.argtypes = [i, ctypes.POINTER(ctypes.c_double)]
     lib.poisson_plan_launches_per_solve.argtypes = [vp]
+    lib.poisson_plan_batch_lanes.argtypes = [vp, i, i]
+    lib.poisson_solve_batch.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), i, vp]
+    lib.poisson_solve_batch_host.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), i, vp]
     lib.poisson_plan_launch_mode.argtypes = [vp, ctypes.POINTER(i), ctypes.c_double * 3]
     lib.poisson_plan_workspace_bytes.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.restype = ctypes.c_size_t
@@ -212,6 +215,34 @@ class PoissonPlan:
 
     def launches_per_solve(self) -> int:
         return load_library().poisson_plan_launches_per_solve(self._h)
+
+    def solve_batch(self, rhos, Vs=None, stream=None):
+        """poisson_solve_batch on lists of device tensors (asynchronous; returns the list of V tensors)."""
+        import torch
+        if Vs is None:
+            Vs = [torch.empty_like(r) for r in rhos]
+        for r, v in zip(rhos, Vs):
+            assert r.is_cuda and r.is_contiguous() and r.dtype == self._dtype() and tuple(r.shape) == (self.n[2], self.n[1], self.n[0])
+            assert v.is_cuda and v.is_contiguous() and v.dtype == r.dtype and v.shape == r.shape
+        n = len(rhos)
+        rp = (ctypes.c_void_p * n)(*[r.data_ptr() for r in rhos])
+        vp_ = (ctypes.c_void_p * n)(*[v.data_ptr() for v in Vs])
+        _check(load_library().poisson_solve_batch(self._h, rp, vp_, n, self._stream(stream)), "poisson_solve_batch")
+        return Vs
+
+    def solve_batch_host(self, rhos, Vs, stream=None):
+        """poisson_solve_batch_host on lists of (pinned) host tensors; returns when every V is on the host."""
+        for r, v in zip(rhos, Vs):
+            assert (not r.is_cuda) and r.is_contiguous() and r.dtype == self._dtype()
+            assert (not v.is_cuda) and v.is_contiguous() and v.dtype == r.dtype and v.shape == r.shape
+        n = len(rhos)
+        rp = (ctypes.c_void_p * n)(*[r.data_ptr() for r in rhos])
+        vp_ = (ctypes.c_void_p * n)(*[v.data_ptr() for v in Vs])
+        _check(load_library().poisson_solve_batch_host(self._h, rp, vp_, n, self._stream(stream)), "poisson_solve_batch_host")
+        return Vs
+
+    def batch_lanes(self, count: int, host: bool = False) -> int:
+        return load_library().poisson_plan_batch_lanes(self._h, count, 1 if host else 0)
 
     def launch_mode(self):
         """(mode name, {mode name: measured ms per solve at plan creation}) -- see poisson_plan_launch_mode."""

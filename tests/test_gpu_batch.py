@@ -1,0 +1,90 @@
+"""poisson_solve_batch / poisson_solve_batch_host (several densities, one K^F, solves dealt to lanes with
+their own intermediates and streams -- PAPER.md:53,89) against the oracle and against one-by-one solves."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import generators as gen
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pk():
+    import torch
+    import paper_1211_5244_b200 as pk
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; the solve has no fallback")
+    pk.load_library()
+    torch.cuda.set_device(0)
+    return pk
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def _even_kernel(rng, s):
+    sx, sy, sz = s
+    K = rng.standard_normal((sz, sy, sx))
+    for ax in range(3):
+        K = 0.5 * (K + np.roll(np.flip(K, axis=ax), 1, axis=ax))
+    return K
+
+
+@pytest.mark.parametrize("n,bc,prec", [((32, 32, 32), (0, 0, 0), "fp64"), ((24, 16, 32), (1, 0, 0), "fp64"),
+                                       ((16, 8, 4), (0, 1, 0), "fp32")])
+def test_batch_matches_oracle_and_single_solves(pk, n, bc, prec):
+    import torch
+    rng = np.random.default_rng(4242 + n[0])
+    dt = np.float64 if prec == "fp64" else np.float32
+    tol = 1e-12 if prec == "fp64" else 1e-5
+    s = gen.padded_shape(n, bc)
+    Kf = oracle.kernel_spectrum(_even_kernel(rng, s)).astype(dt)
+    count = 7                                                      # more solves than lanes, not a multiple of them
+    rhos_np = [rng.standard_normal((n[2], n[1], n[0])).astype(dt) for _ in range(count)]
+    plan = pk.PoissonPlan(n, bc, 0.25, pk.FP64 if prec == "fp64" else pk.FP32)
+    try:
+        plan.set_kernel(torch.from_numpy(Kf).cuda())
+        rhos = [torch.from_numpy(r).cuda() for r in rhos_np]
+        Vs = plan.solve_batch(rhos)
+        torch.cuda.synchronize()
+        single = [plan.solve(r) for r in rhos]
+        torch.cuda.synchronize()
+        for i in range(count):
+            ref = oracle.solve(rhos_np[i].astype(np.float64), Kf.astype(np.float64), bc)
+            assert rel_l2(Vs[i].cpu().numpy().astype(np.float64), ref) <= tol, (i, n, bc, prec)
+            assert rel_l2(Vs[i].cpu().numpy().astype(np.float64), single[i].cpu().numpy().astype(np.float64)) <= tol * 1e-2
+        # in place (rho[i] == V[i]) and a second batch on the same lanes
+        work = [r.clone() for r in rhos]
+        plan.solve_batch(work, work)
+        torch.cuda.synchronize()
+        for i in range(count):
+            assert torch.equal(work[i], Vs[i])                     # same kernels, same order: bitwise
+        # host variant: H2D + passes + D2H per lane, returns with every V on the host
+        hr = [torch.from_numpy(r).pin_memory() for r in rhos_np]
+        hv = [torch.empty_like(h).pin_memory() for h in hr]
+        plan.solve_batch_host(hr, hv)
+        for i in range(count):
+            assert torch.equal(hv[i], Vs[i].cpu())
+        plan.solve_batch([], [])                                   # empty batch is a no-op
+    finally:
+        plan.close()
+
+
+def test_batch_error_codes(pk):
+    import ctypes
+    import torch
+    plan = pk.PoissonPlan((8, 8, 8), (0, 0, 0), 0.1, pk.FP64)
+    rho = torch.zeros(8, 8, 8, dtype=torch.float64, device="cuda")
+    lib = pk.load_library()
+    arr = (ctypes.c_void_p * 1)(rho.data_ptr())
+    assert lib.poisson_solve_batch(plan.handle, arr, arr, 1, None) == 4          # ENOKERNEL
+    plan.set_kernel(torch.ones(16, 16, 9, dtype=torch.float64, device="cuda"))
+    assert lib.poisson_solve_batch(plan.handle, arr, arr, -1, None) == 1         # EINVAL
+    bad = (ctypes.c_void_p * 1)(rho.data_ptr() + 8)
+    assert lib.poisson_solve_batch(plan.handle, bad, arr, 1, None) == 1          # misaligned
+    assert lib.poisson_solve_batch(plan.handle, None, arr, 1, None) == 1         # null
+    assert lib.poisson_solve_batch(plan.handle, arr, arr, 1, None) == 0          # K^F == 1: V = rho
+    torch.cuda.synchronize()
+    plan.close()

@@ -66,7 +66,7 @@ static void reg_length(int prec, int variant) {
 #define PF_MINB 0
 #endif
 #ifndef PF_STG
-#define PF_STG 1
+#define PF_STG 0
 #endif
 #ifndef PF_KLATE
 #define PF_KLATE true

@@ -1,6 +1,6 @@
 // inst.cuh -- instantiates and registers every pass kernel for ONE transform length.
 // An inst_S<len>_<prec>.cu file defines PF_S, PF_RA, PF_RB, PF_TPP (and optionally the tuning knobs
-// PF_NBUF, PF_TWS, PF_MINB, PF_STG, PF_EXTRA_VARIANTS) and includes this header.
+// PF_NBUF, PF_TWS, PF_MINB, PF_STG, PF_KLATE, PF_PCMUL, PF_EXTRA_VARIANTS) and includes this header.
 #pragma once
 
 #include "passes.cuh"
@@ -38,11 +38,15 @@ constexpr int pencils_per_cta() {
     return by_threads > by_line ? by_threads : by_line;
 }
 
-template <typename T, int S, int RA, int RB, int TPP, int NBUF, bool TWS, int MINB, int STG, bool KLATE>
+// PCMUL: the contiguous-axis kernels (lanes along the transform, warp-private exchange) may take PCMUL times
+// more pencils per CTA, with MINB / PCMUL resident CTAs: same warps per SM, but ONE copy of the twiddle
+// tables per SM, which is what leaves room for the asynchronous stage at S = 512 in fp64.
+template <typename T, int S, int RA, int RB, int TPP, int NBUF, bool TWS, int MINB, int STG, bool KLATE, int PCMUL = 1>
 static void reg_length(int prec, int variant) {
     constexpr int P = pencils_per_cta<T, TPP>();
+    constexpr int MINBC = MINB > 0 ? (MINB / PCMUL > 0 ? MINB / PCMUL : 1) : 0;
     using GP = Geo<T, S, RA, RB, TPP, P, true, NBUF, TWS, MINB, STG, KLATE>;
-    using GC = Geo<T, S, RA, RB, TPP, P, false, NBUF, TWS, MINB, STG, KLATE>;
+    using GC = Geo<T, S, RA, RB, TPP, P * PCMUL, false, NBUF, TWS, MINBC, STG, KLATE>;
     reg_one<GP, true, KIND_F1>(prec, variant);  reg_one<GP, false, KIND_F1>(prec, variant);
     reg_one<GP, true, KIND_I1>(prec, variant);  reg_one<GP, false, KIND_I1>(prec, variant);
     reg_one<GP, true, KIND_F2>(prec, variant);  reg_one<GP, false, KIND_F2>(prec, variant);
@@ -71,6 +75,9 @@ static void reg_length(int prec, int variant) {
 #ifndef PF_KLATE
 #define PF_KLATE true
 #endif
+#ifndef PF_PCMUL
+#define PF_PCMUL 1
+#endif
 #if defined(PF_ONLY_F64)
 #define PF_T double
 #define PF_PREC 0
@@ -81,10 +88,12 @@ static void reg_length(int prec, int variant) {
 namespace {
 struct PfRegistrar {
     PfRegistrar() {
-        pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, PF_NBUF, PF_TWS, PF_MINB, PF_STG, PF_KLATE>(PF_PREC, 0);
+        pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, PF_NBUF, PF_TWS, PF_MINB, PF_STG, PF_KLATE, PF_PCMUL>(PF_PREC, 0);
 #if defined(PF_EXTRA_VARIANTS)
 #define PF_VARIANT(ID, NBUF, TWS, MINB, STG, KLATE) pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, NBUF, TWS, MINB, STG, KLATE>(PF_PREC, ID);
+#define PF_VARIANT_PC(ID, NBUF, TWS, MINB, STG, KLATE, PCMUL) pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, NBUF, TWS, MINB, STG, KLATE, PCMUL>(PF_PREC, ID);
         PF_EXTRA_VARIANTS
+#undef PF_VARIANT_PC
 #undef PF_VARIANT
 #endif
     }

@@ -4,4 +4,7 @@
 #define PF_RB 16
 #define PF_TPP 16
 #define PF_ONLY_F32
+// tuning experiments: PF_VARIANT(id, NBUF, TWS, MINB, STG, KLATE) / PF_VARIANT_PC(..., PCMUL)
+#define PF_EXTRA_VARIANTS PF_VARIANT(1, 1, true, 2, 1, true) PF_VARIANT_PC(2, 1, true, 2, 1, true, 2) PF_VARIANT(3, 1, true, 3, 0, true) \
+    PF_VARIANT_PC(4, 1, true, 2, 2, true, 2)
 #include "inst.cuh"

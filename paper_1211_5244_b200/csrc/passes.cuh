@@ -37,6 +37,8 @@ PF_HD void cta_sync() { host_cta_sync(); }
 PF_HD void warp_sync() { host_cta_sync(); }
 #endif
 
+enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4 };
+
 // ------------------------------------------------------------------ geometry
 // NBUF_   : exchange buffers (2 = one barrier per exchange, 1 = half the shared memory, one more barrier)
 // TWS_    : twiddles w_S^{n1 k2} read from a shared-memory table (true) or held in registers (false)
@@ -74,6 +76,9 @@ struct Geo {
     static constexpr int TW_TABLES = !TWS ? 0 : (RA == RB ? 1 : 2);            // [k2][n1] and [n1][k2]
     static constexpr int TW_ELEMS = TW_TABLES * S;
     static constexpr size_t SMEM_BYTES = ((size_t)NBUF * XELEMS + TW_ELEMS) * sizeof(cx<T_>);
+    // a one-pass kernel only keeps the table(s) its direction reads: F1/F2 [k2][n1], I2/I1 [n1][k2], F3 both
+    static constexpr int tw_elems(int kind) { return (kind == KIND_F3 ? TW_TABLES : (TW_TABLES > 0 ? 1 : 0)) * S; }
+    static constexpr size_t smem_bytes(int kind) { return ((size_t)NBUF * XELEMS + tw_elems(kind)) * sizeof(cx<T_>); }
 
     static PF_HD void split(int tid, int &t, int &p) {
         if (LANES_P) { p = tid % P; t = tid / P; } else { t = tid % TPP; p = tid / TPP; }
@@ -129,14 +134,15 @@ struct Twiddles {
     // tab: S entries exp(-2 pi i m / S) in global memory; smem_tw: G::TW_ELEMS entries of shared memory
     template <bool NEED_A, bool NEED_B>
     PF_HD void init(const cx<T> *tab, cx<T> *smem_tw, int tid, int t) {
-        ta = smem_tw; tb = smem_tw + (G::TW_TABLES == 2 ? G::S : 0);
+        constexpr bool ONE = G::TW_TABLES == 1;                       // RA == RB: the table is symmetric
+        constexpr bool FILL_A = ONE || NEED_A, FILL_B = !ONE && NEED_B;
+        ta = smem_tw; tb = smem_tw + (FILL_A && FILL_B ? G::S : 0);
         if constexpr (G::RB > 1) {
             if constexpr (G::TWS) {
                 for (int idx = tid; idx < G::S; idx += G::NT) {
-                    const cx<T> w = tab[((idx / G::RB) * (idx % G::RB)) % G::S];     // [k2][n1]
-                    smem_tw[idx] = w;
-                    if constexpr (G::TW_TABLES == 2)
-                        smem_tw[G::S + (idx % G::RB) * G::RA + idx / G::RB] = w;       // [n1][k2]
+                    const cx<T> w = tab[((idx / G::RB) * (idx % G::RB)) % G::S];
+                    if constexpr (FILL_A) smem_tw[idx] = w;                                                        // [k2][n1]
+                    if constexpr (FILL_B) smem_tw[(FILL_A ? G::S : 0) + (idx % G::RB) * G::RA + idx / G::RB] = w;  // [n1][k2]
                 }
                 cta_sync();
             } else {
@@ -305,7 +311,6 @@ PF_HD void store_B(const cx<typename G::T> *v, cx<typename G::T> *dst, long long
 // With G::STG > 0 a CTA keeps ONE tile of input in flight in shared memory while it transforms the
 // previous one: the copies are issued right after the current tile has been pulled into registers and
 // have the whole transform + store of that tile to land, at no register cost.
-enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4 };
 
 PF_HD unsigned long long evict_first_policy() {
 #if defined(__CUDA_ARCH__)
@@ -378,7 +383,7 @@ struct Stage {
     // staging is dropped where it would not leave room for G::MINB resident CTAs (228 KB per SM, 1 KB
     // reserved per CTA): the occupancy the register budget was chosen for wins
     static constexpr size_t SM_SMEM = 233472, CTA_RESERVED = 1024;
-    static constexpr bool fits(size_t stage_bytes) { return (G::SMEM_BYTES + stage_bytes + CTA_RESERVED) * G::MINB <= SM_SMEM; }
+    static constexpr bool fits(size_t stage_bytes) { return (G::smem_bytes(KIND) + stage_bytes + CTA_RESERVED) * G::MINB <= SM_SMEM; }
     static constexpr bool ON = G::STG > 0 && fits((size_t)NR * W * sizeof(cx<T>));
     static constexpr bool KON = ON && G::STG > 1 && KIND == KIND_F3 && fits(((size_t)NR * W + G::V * G::NT / 2) * sizeof(cx<T>));
     static constexpr int IN_ELEMS = ON ? NR * W : 0;
@@ -391,7 +396,7 @@ struct Stage {
     }
 };
 template <class G, bool PRUNED, int KIND>
-constexpr size_t pass_smem_bytes() { return G::SMEM_BYTES + Stage<G, PRUNED, KIND>::BYTES; }
+constexpr size_t pass_smem_bytes() { return G::smem_bytes(KIND) + Stage<G, PRUNED, KIND>::BYTES; }
 
 // Issue the copies of one tile.  src = element (row 0, column 0) of the tile; ncols = valid columns
 // (ragged last tile).  The threads that later share a barrier scope (CTA, or warp when the exchange
@@ -668,7 +673,7 @@ PF_HD void process_i1(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c
     cx<T> *smem_c = reinterpret_cast<cx<T> *>(smem);                                                  \
     TileCtx<G> c(tid, smem_c);                                                                        \
     const int t = c.t, p = c.p;                                                                       \
-    cx<T> *stage = smem_c + G::NBUF * G::XELEMS + G::TW_ELEMS;                                        \
+    cx<T> *stage = smem_c + G::NBUF * G::XELEMS + G::tw_elems(KIND);                                       \
     const unsigned long long pol = St::ON ? evict_first_policy() : 0ull;                              \
     const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);                                        \
     (void)stage; (void)pol; (void)in; (void)t; (void)p;                                               \

@@ -92,6 +92,37 @@ PF_HD void st_stream(cx<float> *p, cx<float> v) {
     *p = v;
 #endif
 }
+// Two complex values adjacent in memory as ONE access: 256-bit LDG/STG in fp64 (new on sm_100), 128-bit in fp32.
+// p must be aligned to the size of the pair.
+PF_HD void st_pair(cx<double> *p, cx<double> a, cx<double> b) {
+#if defined(__CUDA_ARCH__)
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a.re), "d"(a.im), "d"(b.re), "d"(b.im) : "memory");
+#else
+    p[0] = a; p[1] = b;
+#endif
+}
+PF_HD void st_pair(cx<float> *p, cx<float> a, cx<float> b) {
+#if defined(__CUDA_ARCH__)
+    *reinterpret_cast<float4 *>(p) = make_float4(a.re, a.im, b.re, b.im);
+#else
+    p[0] = a; p[1] = b;
+#endif
+}
+PF_HD void ld_pair_stream(const cx<double> *p, cx<double> &a, cx<double> &b) {
+#if defined(__CUDA_ARCH__)
+    asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a.re), "=d"(a.im), "=d"(b.re), "=d"(b.im) : "l"(p));
+#else
+    a = p[0]; b = p[1];
+#endif
+}
+PF_HD void ld_pair_stream(const cx<float> *p, cx<float> &a, cx<float> &b) {
+#if defined(__CUDA_ARCH__)
+    const float4 v = __ldcs(reinterpret_cast<const float4 *>(p));
+    a = mk<float>(v.x, v.y); b = mk<float>(v.z, v.w);
+#else
+    a = p[0]; b = p[1];
+#endif
+}
 template <bool STREAM, typename E> PF_HD E ld_hint(const E *p) {
     if constexpr (STREAM) return ld_stream(p); else return *p;
 }

@@ -30,12 +30,13 @@ static void reg_one(int prec, int variant) {
     kernel_registry().push_back(e);
 }
 
-// pencils per CTA: >= 128 threads per CTA and tile rows of >= 128 bytes
+// pencils per CTA: whole 128-byte tile rows, >= 128 threads per CTA, whole warps
 template <typename T, int TPP>
 constexpr int pencils_per_cta() {
-    constexpr int by_threads = 128 / TPP > 0 ? 128 / TPP : 1;
     constexpr int by_line = 128 / (int)sizeof(cx<T>);
-    return by_threads > by_line ? by_threads : by_line;
+    int P = by_line;
+    while (P * TPP < 128 || (P * TPP) % 32 != 0) P += by_line;
+    return P;
 }
 
 // PCMUL: the contiguous-axis kernels (lanes along the transform, warp-private exchange) may take PCMUL times

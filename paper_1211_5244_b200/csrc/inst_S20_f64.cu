@@ -1,0 +1,7 @@
+// Pass kernels for transform length 20 = 20 x 1, 1 thread(s) per pencil, f64 (see sizes.def).
+#define PF_S 20
+#define PF_RA 20
+#define PF_RB 1
+#define PF_TPP 1
+#define PF_ONLY_F64
+#include "inst.cuh"

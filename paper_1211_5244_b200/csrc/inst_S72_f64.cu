@@ -1,0 +1,7 @@
+// Pass kernels for transform length 72 = 12 x 6, 6 thread(s) per pencil, f64 (see sizes.def).
+#define PF_S 72
+#define PF_RA 12
+#define PF_RB 6
+#define PF_TPP 6
+#define PF_ONLY_F64
+#include "inst.cuh"

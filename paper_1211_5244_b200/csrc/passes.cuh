@@ -533,7 +533,7 @@ PF_HD void fetch_i2(BufB<G> &b, const PassParams &prm, int tile, const TileCtx<G
     load_B<G, true>(b.x, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);  // last read of A2
 }
 // I1 inputs: Z_k = A_k + i B_k rebuilt from the half spectra of the two packed pencils
-// (Z_{S-k} = conj A_k + i conj B_k); ld(col, kk) returns element kk of pencil 2*pp + col.
+// (Z_{S-k} = conj A_k + i conj B_k); ld(kk, a, b) fetches element kk of pencils 2*pp and 2*pp + 1.
 template <class G, class Ld>
 PF_HD void fetch_i1_with(BufB<G> &b, int t, bool valid, Ld &&ld) {
     using T = typename G::T;
@@ -546,7 +546,7 @@ PF_HD void fetch_i1_with(BufB<G> &b, int t, bool valid, Ld &&ld) {
             const bool lower = k <= S / 2;
             const int kk = lower ? k : S - k;
             cx<T> a = mk<T>((T)0, (T)0), bb = a;
-            if (valid) { a = ld(0, kk); bb = ld(1, kk); }
+            if (valid) ld(kk, a, bb);
             b.x[i * G::RB + k1] = lower ? mk<T>(a.re - bb.im, a.im + bb.re) : mk<T>(a.re + bb.im, bb.re - a.im);
         });
     });
@@ -557,7 +557,12 @@ PF_HD void fetch_i1(BufB<G> &b, const PassParams &prm, int tile, const TileCtx<G
     const int t = c.t, p = c.p;
     PF_TILE_COORDS
     const cx<T> *src = reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + 2 * pp * prm.ps_in;
-    fetch_i1_with<G>(b, t, valid, [&](int col, int kk) { return ld_stream(src + kk * prm.ns_in + col * prm.ps_in); });
+    if (prm.ps_in == 1)   // the two pencils of a pair are adjacent: one access (256-bit in fp64)
+        fetch_i1_with<G>(b, t, valid, [&](int kk, cx<T> &a, cx<T> &bb) { ld_pair_stream(src + kk * prm.ns_in, a, bb); });
+    else
+        fetch_i1_with<G>(b, t, valid, [&](int kk, cx<T> &a, cx<T> &bb) {
+            a = ld_stream(src + kk * prm.ns_in); bb = ld_stream(src + kk * prm.ns_in + prm.ps_in);
+        });
 }
 
 // F2: (transpose +) spread + 1D FFT along axis b
@@ -642,6 +647,7 @@ PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
     });
     cta_sync();
     cx<T> *dst = reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + 2 * pp * prm.ps_out;
+    const bool pair_store = prm.ps_out == 1;
     static_for<NM>([&](auto mc) {
         constexpr int m = decltype(mc)::value;
         const int k = t + G::TPP * m;
@@ -649,8 +655,9 @@ PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
             const cx<T> zk = xn[G::nidx(p, k)], zp = xn[G::nidx(p, (S - k) % S)];
             const T hf = (T)0.5;
             // A = (Z_k + conj Z_{S-k})/2 ; B = -i (Z_k - conj Z_{S-k})/2
-            dst[k * prm.ns_out] = mk<T>(hf * (zk.re + zp.re), hf * (zk.im - zp.im));
-            dst[k * prm.ns_out + prm.ps_out] = mk<T>(hf * (zk.im + zp.im), hf * (zp.re - zk.re));
+            const cx<T> fa = mk<T>(hf * (zk.re + zp.re), hf * (zk.im - zp.im)), fb = mk<T>(hf * (zk.im + zp.im), hf * (zp.re - zk.re));
+            if (pair_store) st_pair(dst + k * prm.ns_out, fa, fb);   // adjacent pencils: one access (256-bit in fp64)
+            else { dst[k * prm.ns_out] = fa; dst[k * prm.ns_out + prm.ps_out] = fb; }
         }
     });
 }
@@ -812,7 +819,7 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         [&](Buf &b, int tile) {
             if constexpr (St::ON) {
                 PF_TILE_COORDS
-                fetch_i1_with<G>(b, t, valid, [&](int col, int kk) { return stage[St::idx(2 * p + col, kk)]; });
+                fetch_i1_with<G>(b, t, valid, [&](int kk, cx<T> &a, cx<T> &bb) { a = stage[St::idx(2 * p, kk)]; bb = stage[St::idx(2 * p + 1, kk)]; });
             } else {
                 fetch_i1<G>(b, prm, tile, c);
             }

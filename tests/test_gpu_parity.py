@@ -61,13 +61,16 @@ def oracle_inputs(rho, Kf, prec):
 
 # --------------------------------------------------------------------------- small sweep: every BC combo
 SWEEP_SIZES = [(4, 4, 4), (8, 4, 16), (16, 8, 4), (12, 24, 6), (32, 6, 8), (6, 48, 2), (24, 16, 32), (48, 12, 24),
-               (64, 32, 16), (96, 8, 4), (4, 128, 8)]
+               (64, 32, 16), (96, 8, 4), (4, 128, 8),
+               # lengths with factors 5 and 9, and 1024 (sizes.def, second block)
+               (20, 40, 36), (72, 20, 40), (100, 36, 20), (144, 8, 20), (200, 4, 8), (4, 288, 8), (8, 4, 512)]
 
 
 @pytest.mark.parametrize("prec", ["fp64", "fp32"])
 @pytest.mark.parametrize("n", SWEEP_SIZES, ids=lambda n: "x".join(map(str, n)))
 def test_sweep_all_bc_vs_oracle(pk, n, prec):
-    """Lengths 2^a and 3*2^a, several tiles and ragged tails, all 8 BC combinations per size."""
+    """Lengths 2^a, 3*2^a and the 5- and 9-smooth ones of sizes.def, several tiles and ragged tails, all 8 BC
+    combinations per size."""
     rng = np.random.default_rng(1000 + sum(n))
     ran = 0
     for bc in itertools.product((0, 1), repeat=3):

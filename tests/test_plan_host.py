@@ -96,7 +96,7 @@ def test_argument_validation(lib):
     assert lib.poisson_plan_describe(8, 8, 8, (ctypes.c_int * 3)(0, 2, 0), 0, ctypes.byref(info)) == 1
     assert lib.poisson_plan_describe(8, 8, 8, bc, 0, None) == 1                          # EINVAL: null
     assert lib.poisson_plan_describe(7, 8, 8, bc, 0, ctypes.byref(info)) == 2           # EUNSUPPORTED: odd N
-    assert lib.poisson_plan_describe(8, 8, 10, bc, 0, ctypes.byref(info)) == 2          # EUNSUPPORTED: S = 20
+    assert lib.poisson_plan_describe(8, 8, 14, bc, 0, ctypes.byref(info)) == 2          # EUNSUPPORTED: S = 28
     assert lib.poisson_plan_describe(8, 8, 8, bc, 0, ctypes.byref(info)) == 0
     handle = ctypes.c_void_p(123)
     assert lib.poisson_plan_create(ctypes.byref(handle), 8, 8, 8, bc, -1.0, 0) == 1     # EINVAL: h <= 0

@@ -1,0 +1,7 @@
+// Pass kernels for transform length 240 = 20 x 12, 12 thread(s) per pencil, f64 (see sizes.def).
+#define PF_S 240
+#define PF_RA 20
+#define PF_RB 12
+#define PF_TPP 12
+#define PF_ONLY_F64
+#include "inst.cuh"

@@ -1,0 +1,7 @@
+// Pass kernels for transform length 320 = 20 x 16, 16 thread(s) per pencil, f32 (see sizes.def).
+#define PF_S 320
+#define PF_RA 20
+#define PF_RB 16
+#define PF_TPP 16
+#define PF_ONLY_F32
+#include "inst.cuh"

@@ -1,0 +1,7 @@
+// Pass kernels for transform length 384 = 24 x 16, 16 thread(s) per pencil, f32 (see sizes.def).
+#define PF_S 384
+#define PF_RA 24
+#define PF_RB 16
+#define PF_TPP 16
+#define PF_ONLY_F32
+#include "inst.cuh"

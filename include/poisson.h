@@ -131,6 +131,10 @@ POISSON_API int poisson_solve_host(poisson_plan *plan, const void *rho_host, voi
  * solve i on the two copy engines).  Lanes are allocated on first use and kept by the plan (its
  * workspace_bytes grows accordingly).  Always five launches per solve (the cooperative fused kernel cannot
  * overlap with itself).
+ * Small grids (intermediates of one density <= 16 MB, i.e. up to 64^3 -> 128^3, where one solve has far fewer tiles than the
+ * GPU has resident CTAs) take a different route in poisson_solve_batch: up to 32 densities per LAUNCH -- each of the
+ * five launches covers the tiles of all of them, density i using slot i of a wide A1 / A2 allocation (<= 96 MB, so it
+ * stays in L2) -- on the caller's stream, no lanes (POISSON_WIDE=0 disables, =n forces n per launch).
  *   rho / V : host arrays of `count` pointers; poisson_solve_batch: device buffers as in poisson_solve
  *             (rho[i] == V[i] allowed; the V[i] must not overlap each other or any other rho[j]);
  *             poisson_solve_batch_host: host buffers (pinned for overlap), [nz][ny][nx] reals each.
@@ -142,6 +146,8 @@ POISSON_API int poisson_solve_batch(poisson_plan *plan, const void *const *rho_d
                         void *const *V_dev /* host array of device ptrs */, int count, void *stream);
 POISSON_API int poisson_solve_batch_host(poisson_plan *plan, const void *const *rho_host /* host array of host ptrs */,
                              void *const *V_host /* host array of host ptrs */, int count, void *stream);
+/* Densities per launch a DEVICE batch of `count` solves would use (the small-grid route above); 0 = the lane route. */
+POISSON_API int poisson_plan_batch_width(const poisson_plan *plan, int count);
 /* Lanes a batch of `count` solves would use (host != 0: the host variant); 0 on a null plan or count <= 0.
  * With one lane a device batch is poisson_solve in a loop (same launch mode). */
 POISSON_API int poisson_plan_batch_lanes(const poisson_plan *plan, int count, int host);

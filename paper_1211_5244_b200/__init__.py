@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "poisson_plan_describe", "poisson_plan_create", "poisson_plan_kernel_dims", "poisson_plan_get_info",
     "poisson_set_kernel", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
     "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_measure_fma_peak", "poisson_plan_workspace_bytes",
-    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes",
+    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes", "poisson_plan_batch_width",
 )
 
 _PKG = Path(__file__).resolve().parent
@@ -87,6 +87,8 @@ def load_library():
     lib.poisson_measure_fma_peak.argtypes = [i, ctypes.POINTER(ctypes.c_double)]
     lib.poisson_plan_launches_per_solve.argtypes = [vp]
     lib.poisson_plan_batch_lanes.argtypes = [vp, i, i]
+    lib.poisson_plan_batch_width.argtypes = [vp, i]
+    lib.poisson_plan_batch_width.restype = i
     lib.poisson_solve_batch.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), i, vp]
     lib.poisson_solve_batch_host.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), i, vp]
     lib.poisson_plan_launch_mode.argtypes = [vp, ctypes.POINTER(i), ctypes.c_double * 3]
@@ -230,6 +232,21 @@ class PoissonPlan:
         _check(load_library().poisson_solve_batch(self._h, rp, vp_, n, self._stream(stream)), "poisson_solve_batch")
         return Vs
 
+    def pointer_batch(self, rhos, Vs):
+        """Marshal a batch ONCE: validates the device tensors and returns the two pointer arrays poisson_solve_batch
+        takes (what a C caller holds anyway), for repeated solve_pointer_batch calls on the same buffers."""
+        for r, v in zip(rhos, Vs):
+            assert r.is_cuda and r.is_contiguous() and r.dtype == self._dtype() and tuple(r.shape) == (self.n[2], self.n[1], self.n[0])
+            assert v.is_cuda and v.is_contiguous() and v.dtype == r.dtype and v.shape == r.shape
+        n = len(rhos)
+        rp = (ctypes.c_void_p * n)(*[r.data_ptr() for r in rhos])
+        vp_ = (ctypes.c_void_p * n)(*[v.data_ptr() for v in Vs])
+        return (rp, vp_, n, list(rhos), list(Vs))     # the tensor lists keep the buffers alive
+
+    def solve_pointer_batch(self, batch, stream=None):
+        rp, vp_, n = batch[0], batch[1], batch[2]
+        _check(load_library().poisson_solve_batch(self._h, rp, vp_, n, self._stream(stream)), "poisson_solve_batch")
+
     def solve_batch_host(self, rhos, Vs, stream=None):
         """poisson_solve_batch_host on lists of (pinned) host tensors; returns when every V is on the host."""
         for r, v in zip(rhos, Vs):
@@ -243,6 +260,10 @@ class PoissonPlan:
 
     def batch_lanes(self, count: int, host: bool = False) -> int:
         return load_library().poisson_plan_batch_lanes(self._h, count, 1 if host else 0)
+
+    def batch_width(self, count: int) -> int:
+        """Densities per launch of a device batch of `count` solves (small grids), 0 = the lane route."""
+        return load_library().poisson_plan_batch_width(self._h, count)
 
     def launch_mode(self):
         """(mode name, {mode name: measured ms per solve at plan creation}) -- see poisson_plan_launch_mode."""

@@ -109,7 +109,10 @@ struct poisson_plan {
     int num_sms;
     const KernelEntry *k[5];
     int grid[5];
+    int resident[5];      // co-resident CTAs of each pass kernel on this device
     int n_tiles[5], tiles_per_g[5];
+    void *wide_a1, *wide_a2;   // intermediates of wide_w densities (several small solves per launch), allocated on first use
+    int wide_w;
     void *a1, *a2, *kint;
     void *tw[3];          // per axis id
     void *rho_stage, *v_stage;
@@ -152,6 +155,7 @@ static void free_plan(poisson_plan *pl) {
     cudaFree(pl->a1); cudaFree(pl->a2); cudaFree(pl->kint);
     for (int q = 0; q < 3; ++q) cudaFree(pl->tw[q]);
     cudaFree(pl->rho_stage); cudaFree(pl->v_stage); cudaFree(pl->fused_sync);
+    cudaFree(pl->wide_a1); cudaFree(pl->wide_a2);
     if (pl->lanes) {
         for (Lane &ln : *pl->lanes) {
             if (ln.owns_ws) { cudaFree(ln.a1); cudaFree(ln.a2); }
@@ -251,6 +255,7 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
         ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, e->func, e->NT, e->smem_bytes);
         if (ce != cudaSuccess || occ < 1) { free_plan(pl); return cuda_fail(ce, "occupancy query"); }
         const long long resident = (long long)occ * pl->num_sms;
+        pl->resident[q] = (int)resident;
         pl->grid[q] = (int)(pl->n_tiles[q] < resident ? pl->n_tiles[q] : resident);  // persistent CTAs
     }
 
@@ -405,7 +410,7 @@ int poisson_set_kernel(poisson_plan *pl, const void *K_f_dev, void *stream) {
 static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, void *V, const Lane *ln = nullptr) {
     const PassDesc &ps = pl->d.pass[q];
     void *a1 = ln ? ln->a1 : pl->a1, *a2 = ln ? ln->a2 : pl->a2;
-    PassParams prm;
+    PassParams prm{};
     switch (q) {
         case POISSON_PASS_F1: prm.in = rho; prm.out = a1; break;
         case POISSON_PASS_F2: prm.in = a1; prm.out = a2; break;
@@ -418,6 +423,7 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
     prm.gs_in = ps.gs_in; prm.ns_in = ps.ns_in; prm.ps_in = ps.ps_in;
     prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;
     prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q];
+    prm.n_tiles1 = pl->n_tiles[q];   // one density per launch
     // L2 prefetch of the next tile only where the pass's input cannot be sitting in L2 already (measured: a few
     // per cent faster on the 512^3 grids, slightly slower on 256^3 where A1 / A2 are L2 hits anyway)
     {
@@ -467,6 +473,52 @@ static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t s
 static int run_solve(poisson_plan *pl, const void *rho, void *V, cudaStream_t st) {
     if (pl->fused && pl->use_fused) return run_fused(pl, rho, V, st);
     return run_passes(pl, rho, V, st, 0, 4);
+}
+
+// Several small solves per launch (poisson_solve_batch on small grids): each of the five launches covers the
+// tiles of nbw densities; density bi uses slot bi of the wide intermediates, reads rho[bi] and writes V[bi].
+static int run_passes_wide(poisson_plan *pl, const void *const *rho, void *const *V, int nbw, cudaStream_t st) {
+    const size_t cplx = 2 * pl->elem_real;
+    for (int q = 0; q < 5; ++q) {
+        const KernelEntry *e = pl->k[q];
+        PassParams prm = pass_params(pl, q, nullptr, nullptr);
+        prm.n_tiles = nbw * pl->n_tiles[q];
+        const long long s1 = pl->d.a1_elems, s2 = pl->d.a2_elems;
+        switch (q) {
+            case POISSON_PASS_F1: prm.in = nullptr; prm.out = pl->wide_a1; prm.use_list = 1; prm.bs_out = s1; break;
+            case POISSON_PASS_F2: prm.in = pl->wide_a1; prm.out = pl->wide_a2; prm.bs_in = s1; prm.bs_out = s2; break;
+            case POISSON_PASS_F3: prm.in = pl->wide_a2; prm.out = pl->wide_a2; prm.bs_in = s2; prm.bs_out = s2; break;
+            case POISSON_PASS_I2: prm.in = pl->wide_a2; prm.out = pl->wide_a1; prm.bs_in = s2; prm.bs_out = s1; break;
+            default: prm.in = pl->wide_a1; prm.out = nullptr; prm.use_list = 2; prm.bs_in = s1; break;
+        }
+        if (q == POISSON_PASS_F1) for (int i = 0; i < nbw; ++i) prm.blist[i] = rho[i];
+        if (q == POISSON_PASS_I1) for (int i = 0; i < nbw; ++i) prm.blist[i] = V[i];
+        prm.prefetch = 0;
+        (void)cplx;
+        void *args[] = {&prm};
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(prm.n_tiles < pl->resident[q] ? prm.n_tiles : pl->resident[q]); cfg.blockDim = dim3(e->NT);
+        cfg.dynamicSmemBytes = e->smem_bytes; cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = pl->use_pdl ? 1 : 0;
+        PF_CUDA(cudaLaunchKernelExC(&cfg, e->func, args));
+    }
+    return POISSON_OK;
+}
+
+// Densities per launch for device batches: small grids only (one density leaves most of the GPU idle: 32^3 -> 64^3
+// has 64 .. 264 tiles per pass for 592 resident CTAs), as many as keep the wide intermediates within ~96 MB of L2.
+static int wide_width(const poisson_plan *pl, int count) {
+    const char *env = std::getenv("POISSON_WIDE");
+    const size_t lane_bytes = (size_t)(pl->d.a1_elems + pl->d.a2_elems) * 2 * pl->elem_real;
+    int w = 0;
+    if (env) w = std::atoi(env);
+    else if (lane_bytes <= ((size_t)16 << 20)) w = (int)(((size_t)96 << 20) / lane_bytes);   // measured: 64^3 (12.8 MB) gains 18 % over 3 lanes, 96^3 (43 MB) loses
+    if (w > PF_MAX_WIDE) w = PF_MAX_WIDE;
+    if (w > count) w = count;
+    return w >= 2 ? w : 0;
 }
 
 // Times the launch modes on scratch inputs (timing does not depend on the values) and keeps the fastest.
@@ -625,6 +677,27 @@ static int solve_batch_impl(poisson_plan *pl, const void *const *rho, void *cons
         if (!host && (reinterpret_cast<size_t>(rho[i]) % 16 || reinterpret_cast<size_t>(V[i]) % 16)) return POISSON_EINVAL;
     }
     if (!pl->kernel_set) return POISSON_ENOKERNEL;
+    if (!host) {
+        const int W = wide_width(pl, count);
+        if (W) {
+            if (pl->wide_w < W) {   // allocated once, for the widest launch this grid will ever take
+                const int cap = wide_width(pl, PF_MAX_WIDE) > W ? wide_width(pl, PF_MAX_WIDE) : W;
+                cudaFree(pl->wide_a1); cudaFree(pl->wide_a2); pl->wide_a1 = pl->wide_a2 = nullptr;
+                if (pl->wide_w) pl->workspace_bytes -= (size_t)pl->wide_w * (pl->d.a1_elems + pl->d.a2_elems) * 2 * pl->elem_real;
+                pl->wide_w = 0;
+                cudaError_t ce = cudaMalloc(&pl->wide_a1, (size_t)cap * pl->d.a1_elems * 2 * pl->elem_real);
+                if (ce == cudaSuccess) ce = cudaMalloc(&pl->wide_a2, (size_t)cap * pl->d.a2_elems * 2 * pl->elem_real);
+                if (ce != cudaSuccess) { cudaGetLastError(); return ce == cudaErrorMemoryAllocation ? POISSON_ENOMEM : cuda_fail(ce, "wide batch allocation"); }
+                pl->wide_w = cap;
+                pl->workspace_bytes += (size_t)cap * (pl->d.a1_elems + pl->d.a2_elems) * 2 * pl->elem_real;
+            }
+            for (int i = 0; i < count; i += W) {
+                const int rc1 = run_passes_wide(pl, rho + i, V + i, count - i < W ? count - i : W, user);
+                if (rc1 != POISSON_OK) return rc1;
+            }
+            return POISSON_OK;
+        }
+    }
     const int L = batch_lanes(pl, count, host);
     if (L == 1 && !host) {   // one lane: the plan's own intermediates on the caller's stream, in the plan's tuned launch mode
         for (int i = 0; i < count; ++i) {
@@ -660,6 +733,10 @@ static int solve_batch_impl(poisson_plan *pl, const void *const *rho, void *cons
 
 int poisson_plan_batch_lanes(const poisson_plan *pl, int count, int host) {
     return pl && count > 0 ? batch_lanes(pl, count, host != 0) : 0;
+}
+
+int poisson_plan_batch_width(const poisson_plan *pl, int count) {
+    return pl && count > 0 ? wide_width(pl, count) : 0;
 }
 
 int poisson_solve_batch(poisson_plan *pl, const void *const *rho_dev, void *const *V_dev, int count, void *stream) {

@@ -99,6 +99,7 @@ struct Geo {
     static PF_HD int nidx(int p, int k) { return LANES_P ? k * P + p : p * XPITCH + k; }
 };
 
+#define PF_MAX_WIDE 32
 // Per-launch parameters.  Strides are in elements of the accessed type.
 struct PassParams {
     const void *in;
@@ -111,7 +112,19 @@ struct PassParams {
     int tiles_per_g;   // ceil(n_p / P)
     int n_tiles;       // n_g * tiles_per_g
     int prefetch;      // 1: prefetch the next tile's inputs into L2 (unstaged tile loops)
+    // several densities per launch (small grids, poisson_solve_batch): tile = bi * n_tiles1 + tile of density bi
+    int n_tiles1;      // tiles of ONE density (n_tiles = nb * n_tiles1; nb = 1 for a single solve)
+    int use_list;      // 0: in/out + bi * bs_in/bs_out; 1: inputs are blist[bi] (F1: rho); 2: outputs are blist[bi] (I1: V)
+    long long bs_in, bs_out;   // elements between the intermediates of consecutive densities
+    const void *blist[PF_MAX_WIDE];
 };
+
+template <typename T> PF_HD const cx<T> *pass_in(const PassParams &prm, int bi) {
+    return prm.use_list == 1 ? reinterpret_cast<const cx<T> *>(prm.blist[bi]) : reinterpret_cast<const cx<T> *>(prm.in) + bi * prm.bs_in;
+}
+template <typename T> PF_HD cx<T> *pass_out(const PassParams &prm, int bi) {
+    return prm.use_list == 2 ? reinterpret_cast<cx<T> *>(const_cast<void *>(prm.blist[bi])) : reinterpret_cast<cx<T> *>(prm.out) + bi * prm.bs_out;
+}
 
 // ------------------------------------------------------------------ programmatic dependent launch
 // Every pass is launched with programmatic stream serialisation: its CTAs may become resident while
@@ -591,9 +604,10 @@ PF_HD void unpack_A(cx<typename G::T> *v, const B &b) {
 #define PF_TPREF 1   // L2 prefetch of the next tile's inputs in the unstaged tile loops
 #endif
 #define PF_TILE_COORDS                                                                   \
-    const int g = tile / prm.tiles_per_g, p0 = (tile % prm.tiles_per_g) * G::P, pp = p0 + p; \
+    const int bi = tile / prm.n_tiles1, tl = tile - bi * prm.n_tiles1;                   \
+    const int g = tl / prm.tiles_per_g, p0 = (tl % prm.tiles_per_g) * G::P, pp = p0 + p; \
     const bool valid = pp < prm.n_p;                                                     \
-    (void)p0; (void)valid;
+    (void)p0; (void)valid; (void)bi;
 
 // ---- per-tile work, shared by the one-pass kernels below and the fused solve kernel (solve_kernel.cuh).
 // fetch_*: one tile, global memory -> registers.  process_*: transform the tile and store it.
@@ -609,14 +623,14 @@ PF_HD void fetch_fwd(Buf &b, const PassParams &prm, int tile, const TileCtx<G> &
     using T = typename G::T;
     const int t = c.t, p = c.p;
     PF_TILE_COORDS
-    issue_A<G, PRUNED, STREAM>(b, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
+    issue_A<G, PRUNED, STREAM>(b, pass_in<T>(prm, bi) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);
 }
 template <class G>
 PF_HD void fetch_i2(BufB<G> &b, const PassParams &prm, int tile, const TileCtx<G> &c) {
     using T = typename G::T;
     const int t = c.t, p = c.p;
     PF_TILE_COORDS
-    load_B<G, true>(b.x, reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);  // last read of A2
+    load_B<G, true>(b.x, pass_in<T>(prm, bi) + g * prm.gs_in + pp * prm.ps_in, prm.ns_in, t, valid);  // last read of A2
 }
 // I1 inputs: Z_k = A_k + i B_k rebuilt from the half spectra of the two packed pencils
 // (Z_{S-k} = conj A_k + i conj B_k); ld(kk, a, b) fetches element kk of pencils 2*pp and 2*pp + 1.
@@ -642,7 +656,7 @@ PF_HD void fetch_i1(BufB<G> &b, const PassParams &prm, int tile, const TileCtx<G
     using T = typename G::T;
     const int t = c.t, p = c.p;
     PF_TILE_COORDS
-    const cx<T> *src = reinterpret_cast<const cx<T> *>(prm.in) + g * prm.gs_in + 2 * pp * prm.ps_in;
+    const cx<T> *src = pass_in<T>(prm, bi) + g * prm.gs_in + 2 * pp * prm.ps_in;
     if (prm.ps_in == 1)   // the two pencils of a pair are adjacent: one access (256-bit in fp64)
         fetch_i1_with<G>(b, t, valid, [&](int kk, cx<T> &a, cx<T> &bb) { ld_pair_stream(src + kk * prm.ns_in, a, bb); });
     else
@@ -660,7 +674,7 @@ PF_HD void process_f2(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
     cx<T> v[G::V];
     unpack_A<G, PRUNED>(v, b);
     fwd_AtoB<G, PRUNED>(v, c.tw, c.xbufs.next(), t, p);
-    store_B<G>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+    store_B<G>(v, pass_out<T>(prm, bi) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
 }
 // I2: inverse 1D FFT along axis b + compactification (+ transpose)
 template <class G, bool PRUNED, class Hook = NoHook>
@@ -669,7 +683,7 @@ PF_HD void process_i2(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c
     const int t = c.t, p = c.p;
     PF_TILE_COORDS
     inv_BtoA<G, PRUNED>(b.x, c.tw, c.xbufs.next(), t, p, after_read);
-    store_A<G, PRUNED>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+    store_A<G, PRUNED>(b.x, pass_out<T>(prm, bi) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
 }
 // F3: spread + 1D FFT along axis c, K^F multiply (Eq. 3), inverse 1D FFT along c,
 // compactification; in place over the tile it read.  kmul(v) multiplies the V
@@ -684,7 +698,7 @@ PF_HD void process_f3(Buf &b, const PassParams &prm, int tile, TileCtx<G> &c, KM
     fwd_AtoB<G, PRUNED>(v, c.tw, c.xbufs.next(), t, p);
     kmul(v);
     inv_BtoA<G, PRUNED>(v, c.tw, c.xbufs.next(), t, p);
-    store_A<G, PRUNED>(v, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+    store_A<G, PRUNED>(v, pass_out<T>(prm, bi) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
 }
 // K^F of one tile: internal order [tile][V/KVEC][NT][KVEC] (relayout.cuh), 16-byte vectors per thread
 template <class G, class VT>
@@ -702,7 +716,7 @@ template <class G>
 PF_HD void kmul_global(cx<typename G::T> *v, const void *kint, int tile, int tid) {   // streamed straight from global memory
     using T = typename G::T;
     using KV = KVec<T>;
-    const typename KV::V *kp = reinterpret_cast<const typename KV::V *>(kint) + (size_t)tile * (G::V / KV::N) * G::NT + tid;
+    const typename KV::V *kp = reinterpret_cast<const typename KV::V *>(kint) + (size_t)tile * (G::V / KV::N) * G::NT + tid;   // tile: within one density
     static_for<G::V / KV::N>([&](auto qc) {
         constexpr int q = decltype(qc)::value;
         T kk[KV::N]; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), kk);
@@ -732,7 +746,7 @@ PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
         });
     });
     cta_sync();
-    cx<T> *dst = reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + 2 * pp * prm.ps_out;
+    cx<T> *dst = pass_out<T>(prm, bi) + g * prm.gs_out + 2 * pp * prm.ps_out;
     const bool pair_store = prm.ps_out == 1;
     static_for<NM>([&](auto mc) {
         constexpr int m = decltype(mc)::value;
@@ -756,7 +770,7 @@ PF_HD void process_i1(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c
     const int t = c.t, p = c.p;
     PF_TILE_COORDS
     inv_BtoA<G, PRUNED>(b.x, c.tw, c.xbufs.next(), t, p, after_read);
-    store_A<G, PRUNED, true>(b.x, reinterpret_cast<cx<T> *>(prm.out) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+    store_A<G, PRUNED, true>(b.x, pass_out<T>(prm, bi) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
 }
 
 // ------------------------------------------------------------------ one pass per launch
@@ -768,8 +782,7 @@ PF_HD void process_i1(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c
     const int t = c.t, p = c.p;                                                                       \
     cx<T> *stage = smem_c + G::NBUF * G::XELEMS + G::tw_elems(KIND);                                       \
     const unsigned long long pol = (St::ON || St::XON) ? evict_first_policy() : 0ull;                              \
-    const cx<T> *in = reinterpret_cast<const cx<T> *>(prm.in);                                        \
-    (void)stage; (void)pol; (void)in; (void)t; (void)p;                                               \
+    (void)stage; (void)pol; (void)t; (void)p;                                               \
     pdl_launch_dependents();                                                                          \
     c.tw.template init<NEED_A, NEED_B>(reinterpret_cast<const cx<T> *>(prm.tw), smem_c + G::NBUF * G::XELEMS, tid, c.t); \
     pdl_wait_prior_grid();
@@ -781,7 +794,7 @@ PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS
-            stage_issue<G, St, true>(stage, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
+            stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
         },
         [] {},
         [&](Buf &b, int tile) {
@@ -794,7 +807,7 @@ PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](int tile) {
             PF_TILE_COORDS
-            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
+            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
         });
 }
 
@@ -806,7 +819,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         tile_loop_x<G, Buf>(bid, nb, prm.n_tiles,
             [&](int tile) {
                 PF_TILE_COORDS
-                stage_issue<G, St, true, true>(smem_c, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
+                stage_issue<G, St, true, true>(smem_c, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
             },
             [&](Buf &b, int tile) {
                 PF_TILE_COORDS
@@ -828,7 +841,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS
-            stage_issue<G, St, true>(stage, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
+            stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
         },
         [] {},
         [&](Buf &b, int tile) {
@@ -852,7 +865,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](int tile) {
             PF_TILE_COORDS
-            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
+            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
         });
 }
 
@@ -871,13 +884,13 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     typename KV::V *kstage = reinterpret_cast<typename KV::V *>(stage + St::IN_ELEMS);
     (void)kstage;
     auto issue_k = [&](int tile) {
-        const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
+        const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1) * NKV * G::NT + tid;
         static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; cp_async_vec16(kstage + q * G::NT + tid, kp + (size_t)q * G::NT, pol); });
     };
     tile_loop<G, Buf, St::ON, (St::KON ? 1 : 0)>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS
-            stage_issue<G, St, false>(stage, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
+            stage_issue<G, St, false>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
         },
         [&] {
             if constexpr (St::KON) { if (bid < prm.n_tiles) issue_k(bid); cp_async_commit(); }
@@ -886,11 +899,11 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
             else fetch_fwd<G, PRUNED, false>(b, prm, tile, c);
             if constexpr (G::KLATE && !St::KON && KPREF) {   // start this tile's K^F on its way DRAM -> L2 now
-                const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
+                const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1) * NKV * G::NT + tid;
                 static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; prefetch_l2(kp + (size_t)q * G::NT); });
             }
             if constexpr (K_EARLY) {
-                const typename KV::V *kp = kint + (size_t)tile * NKV * G::NT + tid;
+                const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1) * NKV * G::NT + tid;
                 static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), b.k + q * KV::N); });
             }
         },
@@ -903,7 +916,7 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
                     if (tile + nb < prm.n_tiles) issue_k(tile + nb);
                     cp_async_commit();
                 } else if constexpr (G::KLATE) {
-                    kmul_global<G>(v, prm.kint, tile, tid);
+                    kmul_global<G>(v, prm.kint, tile % prm.n_tiles1, tid);
                 } else {
                     static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], b.k[r]); });
                 }
@@ -918,7 +931,7 @@ PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS
-            stage_issue<G, St, true>(stage, in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
+            stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
         },
         [] {},
         [&](Buf &b, int tile) {
@@ -931,7 +944,7 @@ PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](int tile) {
             PF_TILE_COORDS
-            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(in + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
+            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
         });
 }
 
@@ -943,7 +956,7 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         tile_loop_x<G, Buf>(bid, nb, prm.n_tiles,
             [&](int tile) {
                 PF_TILE_COORDS
-                stage_issue<G, St, true, true>(smem_c, in + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);
+                stage_issue<G, St, true, true>(smem_c, pass_in<T>(prm, bi) + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);
             },
             [&](Buf &b, int tile) {
                 PF_TILE_COORDS
@@ -958,7 +971,7 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
         [&](int tile) {
             PF_TILE_COORDS   // stage rows: kk = 0..S/2, columns: the 2 P complex pencils of the P pairs
-            stage_issue<G, St, true>(stage, in + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);
+            stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);
         },
         [] {},
         [&](Buf &b, int tile) {
@@ -975,7 +988,7 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](int tile) {
             PF_TILE_COORDS
-            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(in + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid);
+            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid);
         });
 }
 

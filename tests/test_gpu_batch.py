@@ -34,8 +34,12 @@ def _even_kernel(rng, s):
 
 @pytest.mark.parametrize("n,bc,prec", [((32, 32, 32), (0, 0, 0), "fp64"), ((24, 16, 32), (1, 0, 0), "fp64"),
                                        ((16, 8, 4), (0, 1, 0), "fp32")])
-def test_batch_matches_oracle_and_single_solves(pk, n, bc, prec):
+@pytest.mark.parametrize("wide", ["auto", "0", "3"])
+def test_batch_matches_oracle_and_single_solves(pk, n, bc, prec, wide, monkeypatch):
+    """wide = auto: small grids go several densities per launch; 0: the lane path; 3: chunks of 3 (7 = 3 + 3 + 1)."""
     import torch
+    if wide != "auto":
+        monkeypatch.setenv("POISSON_WIDE", wide)
     rng = np.random.default_rng(4242 + n[0])
     dt = np.float64 if prec == "fp64" else np.float32
     tol = 1e-12 if prec == "fp64" else 1e-5
@@ -88,3 +92,26 @@ def test_batch_error_codes(pk):
     assert lib.poisson_solve_batch(plan.handle, arr, arr, 1, None) == 0          # K^F == 1: V = rho
     torch.cuda.synchronize()
     plan.close()
+
+
+def test_wide_batch_more_densities_than_one_launch_takes(pk):
+    """40 densities on a 16x8x12 grid: two launches' worth (32 + 8) through the several-densities-per-launch route,
+    compared with one-by-one solves of the same plan."""
+    import torch
+    rng = np.random.default_rng(99)
+    n, bc = (16, 8, 12), (0, 1, 0)
+    s = gen.padded_shape(n, bc)
+    Kf = oracle.kernel_spectrum(_even_kernel(rng, s))
+    plan = pk.PoissonPlan(n, bc, 0.25, pk.FP64)
+    try:
+        plan.set_kernel(torch.from_numpy(Kf).cuda())
+        rhos = [torch.from_numpy(rng.standard_normal((n[2], n[1], n[0]))).cuda() for _ in range(40)]
+        Vs = plan.solve_batch(rhos)
+        torch.cuda.synchronize()
+        for i in (0, 1, 31, 32, 39):
+            ref = oracle.solve(rhos[i].cpu().numpy(), Kf, bc)
+            assert rel_l2(Vs[i].cpu().numpy(), ref) <= 1e-12
+        for i in range(40):
+            assert torch.equal(plan.solve(rhos[i]), Vs[i])     # same kernels, same arithmetic per tile: bitwise
+    finally:
+        plan.close()

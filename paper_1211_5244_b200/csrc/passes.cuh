@@ -820,6 +820,12 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             [&](int tile) {
                 PF_TILE_COORDS
                 stage_issue<G, St, true, true>(smem_c, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
+                if (PF_TPREF && prm.prefetch && tile + nb < prm.n_tiles) {   // and the tile after it starts its way DRAM -> L2
+                    const int tile2 = tile + nb;
+                    const int bi2 = tile2 / prm.n_tiles1, tl2 = tile2 - bi2 * prm.n_tiles1;
+                    const int g2 = tl2 / prm.tiles_per_g, q0 = (tl2 % prm.tiles_per_g) * G::P;
+                    prefetch_tile_l2<G, St>(pass_in<T>(prm, bi2) + g2 * prm.gs_in + q0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - q0, tid);
+                }
             },
             [&](Buf &b, int tile) {
                 PF_TILE_COORDS

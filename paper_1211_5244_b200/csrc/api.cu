@@ -111,6 +111,8 @@ struct poisson_plan {
     int grid[5];
     int resident[5];      // co-resident CTAs of each pass kernel on this device
     int n_tiles[5], tiles_per_g[5];
+    size_t pf_min_bytes;  // L2 prefetch (PassParams::prefetch) for arrays at least this large
+    int pf_force;         // POISSON_PREFETCH=0..3 forces the prefetch bits (experiments), -1 = by size
     void *wide_a1, *wide_a2;   // intermediates of wide_w densities (several small solves per launch), allocated on first use
     int wide_w;
     void *a1, *a2, *kint;
@@ -241,6 +243,7 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     // poisson_plan_create MEASURES the candidates once (tune_plan below) unless POISSON_TUNE=0 or the mode is
     // forced with POISSON_PDL=0|1 / POISSON_FUSED=0|1.
     { const char *env = std::getenv("POISSON_PDL"); pl->use_pdl = env && env[0] == '1'; }
+    { const char *env = std::getenv("POISSON_PREFETCH"); pl->pf_force = env ? std::atoi(env) : -1; pl->pf_min_bytes = (size_t)96 << 20; }
 
     for (int q = 0; q < 5; ++q) {
         const PassDesc &ps = d.pass[q];
@@ -431,7 +434,9 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
         const size_t in_bytes = q == POISSON_PASS_F1 ? (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * r
                               : (q == POISSON_PASS_F2 || q == POISSON_PASS_I1) ? (size_t)pl->d.a1_elems * 2 * r
                               : (size_t)pl->d.a2_elems * 2 * r;
-        prm.prefetch = in_bytes >= ((size_t)48 << 20) ? 1 : 0;
+        const size_t k_bytes = (size_t)pl->kint_elems * r;
+        prm.prefetch = (in_bytes >= pl->pf_min_bytes ? 1 : 0) | (q == POISSON_PASS_F3 && k_bytes >= pl->pf_min_bytes ? 2 : 0);
+        if (pl->pf_force >= 0) prm.prefetch = pl->pf_force;
     }
     return prm;
 }

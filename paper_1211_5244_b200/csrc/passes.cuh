@@ -111,7 +111,7 @@ struct PassParams {
     int n_p;           // pencils per g
     int tiles_per_g;   // ceil(n_p / P)
     int n_tiles;       // n_g * tiles_per_g
-    int prefetch;      // 1: prefetch the next tile's inputs into L2 (unstaged tile loops)
+    int prefetch;      // bit 0: prefetch the next tile's inputs into L2 (unstaged tile loops); bit 1: F3 prefetches its K^F lines
     // several densities per launch (small grids, poisson_solve_batch): tile = bi * n_tiles1 + tile of density bi
     int n_tiles1;      // tiles of ONE density (n_tiles = nb * n_tiles1; nb = 1 for a single solve)
     int use_list;      // 0: in/out + bi * bs_in/bs_out; 1: inputs are blist[bi] (F1: rho); 2: outputs are blist[bi] (I1: V)
@@ -807,7 +807,7 @@ PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](int tile) {
             PF_TILE_COORDS
-            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
+            if (PF_TPREF && (prm.prefetch & 1)) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
         });
 }
 
@@ -820,7 +820,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             [&](int tile) {
                 PF_TILE_COORDS
                 stage_issue<G, St, true, true>(smem_c, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
-                if (PF_TPREF && prm.prefetch && tile + nb < prm.n_tiles) {   // and the tile after it starts its way DRAM -> L2
+                if (PF_TPREF && (prm.prefetch & 1) && tile + nb < prm.n_tiles) {   // and the tile after it starts its way DRAM -> L2
                     const int tile2 = tile + nb;
                     const int bi2 = tile2 / prm.n_tiles1, tl2 = tile2 - bi2 * prm.n_tiles1;
                     const int g2 = tl2 / prm.tiles_per_g, q0 = (tl2 % prm.tiles_per_g) * G::P;
@@ -871,7 +871,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](int tile) {
             PF_TILE_COORDS
-            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
+            if (PF_TPREF && (prm.prefetch & 1)) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
         });
 }
 
@@ -904,7 +904,7 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         [&](Buf &b, int tile) {
             if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
             else fetch_fwd<G, PRUNED, false>(b, prm, tile, c);
-            if constexpr (G::KLATE && !St::KON && KPREF) {   // start this tile's K^F on its way DRAM -> L2 now
+            if (G::KLATE && !St::KON && KPREF && (prm.prefetch & 2)) {   // start this tile's K^F on its way DRAM -> L2 now
                 const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1) * NKV * G::NT + tid;
                 static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; prefetch_l2(kp + (size_t)q * G::NT); });
             }
@@ -950,7 +950,7 @@ PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](int tile) {
             PF_TILE_COORDS
-            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
+            if (PF_TPREF && (prm.prefetch & 1)) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid);
         });
 }
 
@@ -994,7 +994,7 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](int tile) {
             PF_TILE_COORDS
-            if (PF_TPREF && prm.prefetch) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid);
+            if (PF_TPREF && (prm.prefetch & 1)) prefetch_tile_l2<G, St>(pass_in<T>(prm, bi) + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid);
         });
 }
 

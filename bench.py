@@ -175,34 +175,45 @@ def barrier():
 
 
 # ------------------------------------------------------------------ CPU oracle timing (cpu_baseline / --impl reference)
-def oracle_sample_seconds(cfg, rho, budget_s: float):
-    """Time the oracle (as it stands) on a bounded sample of the workload and scale to one solve.
-    The oracle's solve is six naive-DFT sweeps over the padded grid (oracle/poisson_oracle.c); the
-    sample runs each sweep's routine (oracle.dft_axis) on a slab holding m of the S planes, i.e. the
-    fraction f = m/S of that sweep's lines.  Returns (seconds per full solve, description, threads)."""
-    import oracle
-    sx, sy, sz = cfg.s
-    nx, ny, nz = cfg.n
-    pad = np.zeros((sz, sy, sx), dtype=np.complex128)
-    pad[:nz, :ny, :nx] = rho
+class OracleSampler:
+    """Times the oracle (as it stands) on a bounded sample of the workload and scales to one solve.
+    The oracle's solve is six naive-DFT sweeps over the padded grid (oracle/poisson_oracle.c); a sample runs each
+    sweep's routine (oracle.dft_axis) on a slab holding m of the S planes, i.e. the fraction f = m/S of that sweep's
+    lines.  The padded array and the per-plane calibration are made once, outside every timed sample."""
 
-    def sweeps(m):
+    def __init__(self, cfg, rho):
+        import oracle
+        self.oracle = oracle
+        self.s, self.n = cfg.s, cfg.n
+        sx, sy, sz = cfg.s
+        nx, ny, nz = cfg.n
+        self.pad = np.zeros((sz, sy, sx), dtype=np.complex128)
+        self.pad[:nz, :ny, :nx] = rho
+        self.per_plane = sum(self.sweeps(1))          # calibration (also warms the library)
+
+    def sweeps(self, m):
+        pad, dft = self.pad, self.oracle.dft_axis
         tx = ty = tz = 0.0
         for sign in (-1, +1):
-            t0 = time.perf_counter(); oracle.dft_axis(pad[:m], 2, sign); tx += time.perf_counter() - t0   # x sweep, m z-planes
-            t0 = time.perf_counter(); oracle.dft_axis(pad[:m], 1, sign); ty += time.perf_counter() - t0   # y sweep, m z-planes
-            t0 = time.perf_counter(); oracle.dft_axis(pad[:, :m], 0, sign); tz += time.perf_counter() - t0  # z sweep, m y-planes
+            t0 = time.perf_counter(); dft(pad[:m], 2, sign); tx += time.perf_counter() - t0      # x sweep, m z-planes
+            t0 = time.perf_counter(); dft(pad[:m], 1, sign); ty += time.perf_counter() - t0      # y sweep, m z-planes
+            t0 = time.perf_counter(); dft(pad[:, :m], 0, sign); tz += time.perf_counter() - t0   # z sweep, m y-planes
         return tx, ty, tz
 
-    t2 = sum(sweeps(2))                                      # calibration (also warms the library)
-    per_plane = t2 / 2.0
-    m = int(max(2, min(min(sy, sz), budget_s / max(per_plane, 1e-9))))
-    tx, ty, tz = sweeps(m)
-    f = m / float(min(sy, sz))
-    full = tx * sz / m + ty * sz / m + tz * sy / m
-    desc = (f"oracle naive-DFT sweeps on {m} of {min(sy, sz)} planes per sweep (f={f:.4f}) of the padded "
-            f"{sx}x{sy}x{sz} grid, 6 sweeps, scaled by 1/f; K_f multiply and padding copy not included")
-    return full, desc, oracle.n_threads()
+    def sample(self, budget_s: float):
+        """(seconds per full solve, description, threads) from one sample of about budget_s seconds."""
+        sx, sy, sz = self.s
+        m = int(max(1, min(min(sy, sz), budget_s / max(self.per_plane, 1e-9))))
+        tx, ty, tz = self.sweeps(m)
+        f = m / float(min(sy, sz))
+        full = tx * sz / m + ty * sz / m + tz * sy / m
+        desc = (f"oracle naive-DFT sweeps on {m} of {min(sy, sz)} planes per sweep (f={f:.4f}) of the padded "
+                f"{sx}x{sy}x{sz} grid, 6 sweeps, scaled by 1/f; K_f multiply and padding copy not included")
+        return full, desc, self.oracle.n_threads()
+
+
+def oracle_sample_seconds(cfg, rho, budget_s: float):
+    return OracleSampler(cfg, rho).sample(budget_s)
 
 
 def run_reference(args):
@@ -213,11 +224,12 @@ def run_reference(args):
     cfg = gen.get_config(args.config)
     rho = gen.gaussian_density(cfg)
     steps, warmup = max(1, args.steps), max(0, args.warmup)
-    budget = min(20.0, 150.0 / (steps + warmup + 1))
+    budget = min(20.0, 150.0 / (steps + warmup + 1))     # the whole run ends within a few minutes
+    sampler = OracleSampler(cfg, rho)
     times = []
     desc, threads = "", 1
     for i in range(warmup + steps):
-        sec, desc, threads = oracle_sample_seconds(cfg, rho, budget)
+        sec, desc, threads = sampler.sample(budget)
         if i >= warmup:
             times.append(sec)
     sec = float(np.mean(times))

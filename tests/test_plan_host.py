@@ -116,3 +116,25 @@ def test_plan_create_fails_loudly_without_a_b200(lib):
     assert st == 6 and handle.value is None        # POISSON_EARCH, no fallback
     with pytest.raises(pk.PoissonError):
         pk.PoissonPlan((8, 8, 8), (0, 0, 0), 0.1)
+
+
+SUPPORTED_LENGTHS = [4, 8, 12, 16, 20, 24, 32, 36, 40, 48, 60, 64, 72, 80, 96, 100, 120, 128, 144, 160, 192, 200, 240,
+                     256, 288, 320, 384, 400, 480, 512, 576, 640, 768, 1024]
+
+
+def test_supported_lengths_match_design_reading_12():
+    """DESIGN.md reading 12 ('various grid sizes'): exactly the lengths of csrc/sizes.def are planned, every
+    other even length is refused with EUNSUPPORTED; a periodic axis uses S = N, a free axis S = 2N."""
+    for s in range(4, 1100, 2):
+        ok_p = s in SUPPORTED_LENGTHS
+        try:
+            info = pk.poisson_plan_describe(8, s, 8, (0, 1, 0), pk.FP64)     # periodic y: S_y = N_y
+            assert ok_p and list(info.s) == [16, s, 16]
+        except pk.PoissonError as e:
+            assert e.status == 2 and not ok_p
+        if s % 4 == 0:                                                       # free y with N_y = s/2 (even)
+            try:
+                info = pk.poisson_plan_describe(8, s // 2, 8, (0, 0, 0), pk.FP32)
+                assert ok_p and list(info.s) == [16, s, 16]
+            except pk.PoissonError as e:
+                assert e.status == 2 and not ok_p

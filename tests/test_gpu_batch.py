@@ -115,3 +115,39 @@ def test_wide_batch_more_densities_than_one_launch_takes(pk):
             assert torch.equal(plan.solve(rhos[i]), Vs[i])     # same kernels, same arithmetic per tile: bitwise
     finally:
         plan.close()
+
+
+def test_config1_batch_in_the_bench_configuration(pk):
+    """configs[1] (128^3 -> 256^3 fp64) through poisson_solve_batch the way bench.py times it (device batch, 3 lanes,
+    marshalled once): every V equals the single-stream solve of the same density bitwise (that solve is checked against the
+    oracle in test_named_config_vs_oracle), and the shift property V = rho displaced holds for a delta kernel."""
+    import torch
+    cfg = gen.get_config("c1")
+    rng = np.random.default_rng(7)
+    n = cfg.n
+    s = gen.padded_shape(n, cfg.bc)
+    # K = delta at displacement d (and at -d, the kernel is inversion symmetric): K_f = 2 cos(2 pi k.d / S), analytic
+    d = (3, 5, 7)
+    kz = np.arange(s[2])[:, None, None] * d[2] / s[2]
+    ky = np.arange(s[1])[None, :, None] * d[1] / s[1]
+    kx = np.arange(s[0] // 2 + 1)[None, None, :] * d[0] / s[0]
+    Kf = 2.0 * np.cos(2 * np.pi * (kx + ky + kz))
+    plan = pk.PoissonPlan(n, cfg.bc, cfg.h, pk.FP64)
+    try:
+        plan.set_kernel(torch.from_numpy(Kf).cuda())
+        assert plan.batch_width(8) == 0 and plan.batch_lanes(8) == 3
+        rhos = [torch.from_numpy(rng.standard_normal((n[2], n[1], n[0]))).cuda() for _ in range(8)]
+        Vs = [torch.empty_like(r) for r in rhos]
+        pb = plan.pointer_batch(rhos, Vs)
+        plan.solve_pointer_batch(pb)
+        plan.solve_pointer_batch(pb)
+        torch.cuda.synchronize()
+        for i in range(8):
+            assert torch.equal(plan.solve(rhos[i]), Vs[i])
+        r = rhos[3].cpu().numpy()
+        exp = np.zeros_like(r)
+        exp[d[2]:, d[1]:, d[0]:] += r[:-d[2], :-d[1], :-d[0]]          # zero fill on free axes: nothing wraps around
+        exp[:-d[2], :-d[1], :-d[0]] += r[d[2]:, d[1]:, d[0]:]
+        assert rel_l2(Vs[3].cpu().numpy(), exp) <= 1e-12
+    finally:
+        plan.close()

@@ -331,7 +331,8 @@ def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, wi
     if with_e2e:
         # end to end through the C ABI with HOST buffers: poisson_solve_batch_host copies every rho H2D, runs the
         # passes and copies every V D2H inside the call (pinned host memory), overlapping neighbouring solves
-        nh = 4 if rho_bytes > 64e6 else 12
+        # (batch size: the pipeline's fill and drain -- first H2D, last D2H -- are paid once per call)
+        nh = 8 if rho_bytes > 64e6 else 32
         hr = [torch.from_numpy(np.ascontiguousarray(rho_np.astype(np_dt))).pin_memory() for _ in range(nh)]
         hv = [torch.empty_like(hr[0]).pin_memory() for _ in range(nh)]
         ne2e = max(nh, min(steps, 96) // nh * nh)

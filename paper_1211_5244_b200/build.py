@@ -32,7 +32,7 @@ def _headers_mtime() -> float:
     return max(h.stat().st_mtime for h in hs)
 
 
-def build(force: bool = False, jobs: int | None = None, verbose: bool = False) -> Path:
+def build(force: bool = False, jobs: int | None = None, verbose: bool = False, experiments: bool = False) -> Path:
     nvcc = os.environ.get("NVCC", "nvcc")
     OBJ.mkdir(exist_ok=True)
     srcs = sorted(CSRC.glob("*.cu"))
@@ -46,6 +46,8 @@ def build(force: bool = False, jobs: int | None = None, verbose: bool = False) -
     def compile_one(so):
         s, o = so
         cmd = [nvcc, *NVCC_FLAGS, "-c", str(s), "-o", str(o)]
+        if experiments:
+            cmd.insert(1, "-DPF_EXPERIMENTS")   # also compile the tuning variants (POISSON_VARIANT=n selects one)
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         r = subprocess.run(cmd, capture_output=True, text=True)
@@ -76,5 +78,6 @@ if __name__ == "__main__":
     ap.add_argument("--force", action="store_true")
     ap.add_argument("--jobs", type=int, default=None)
     ap.add_argument("--verbose", action="store_true")
+    ap.add_argument("--experiments", action="store_true", help="also compile the tuning variants of inst_S*.cu")
     a = ap.parse_args()
-    print(build(a.force, a.jobs, a.verbose))
+    print(build(a.force or a.experiments, a.jobs, a.verbose, a.experiments))

@@ -12,5 +12,8 @@
 #define PF_STG 1
 #define PF_PCMUL 2
 // tuning experiments: PF_VARIANT(id, NBUF, TWS, MINB, STG, KLATE) / PF_VARIANT_PC(..., PCMUL)
+// (instantiated only when the library is built with -DPF_EXPERIMENTS: python -m paper_1211_5244_b200.build --experiments)
+#if defined(PF_EXPERIMENTS)
 #define PF_EXTRA_VARIANTS PF_VARIANT(1, 1, true, 2, 0, true) PF_VARIANT_PC(3, 1, true, 3, 0, true, 3)
+#endif
 #include "inst.cuh"

@@ -100,6 +100,18 @@ struct Lane {
     cudaStream_t st;
     cudaEvent_t done;
     bool owns_ws;
+    struct GraphSolve *gs;       // this lane's five launches as a CUDA graph (graph launch mode), or NULL
+};
+
+// The five launches of one solve as an instantiated CUDA graph (kernel nodes F1 -> F2 -> F3 -> I2 -> I1): one graph
+// launch per solve; rho / V of the call are patched into the F1 / I1 nodes when they differ from the previous call.
+struct GraphSolve {
+    cudaGraph_t graph;
+    cudaGraphExec_t exec;
+    cudaGraphNode_t node[5];
+    PassParams prm[5];
+    const void *rho;
+    void *V;
 };
 
 struct poisson_plan {
@@ -120,7 +132,9 @@ struct poisson_plan {
     void *rho_stage, *v_stage;
     const FusedEntry *fused;   // one-launch solve kernel compiled for this combination of axes, or NULL
     bool use_fused;            // launch mode picked for poisson_solve: fused kernel, else 5 launches (with or without PDL)
-    float tune_ms[3];          // measured ms per solve of {5 launches, 5 launches + PDL, fused}; 0 = not measured
+    bool use_graph;            // ... or the five launches as one CUDA graph launch
+    GraphSolve gs;
+    float tune_ms[4];          // measured ms per solve of {5 launches, 5 launches + PDL, fused, graph}; 0 = not measured
     int fused_grid, fused_skew;
     unsigned *fused_sync;      // barrier / per-plane counters of the fused kernel (zero between solves)
     size_t elem_real;     // bytes per real
@@ -158,9 +172,12 @@ static void free_plan(poisson_plan *pl) {
     for (int q = 0; q < 3; ++q) cudaFree(pl->tw[q]);
     cudaFree(pl->rho_stage); cudaFree(pl->v_stage); cudaFree(pl->fused_sync);
     cudaFree(pl->wide_a1); cudaFree(pl->wide_a2);
+    if (pl->gs.exec) cudaGraphExecDestroy(pl->gs.exec);
+    if (pl->gs.graph) cudaGraphDestroy(pl->gs.graph);
     if (pl->lanes) {
         for (Lane &ln : *pl->lanes) {
             if (ln.owns_ws) { cudaFree(ln.a1); cudaFree(ln.a2); }
+            if (ln.gs) { if (ln.gs->exec) cudaGraphExecDestroy(ln.gs->exec); if (ln.gs->graph) cudaGraphDestroy(ln.gs->graph); delete ln.gs; }
             cudaFree(ln.rho_stage); cudaFree(ln.v_stage);
             if (ln.st) cudaStreamDestroy(ln.st);
             if (ln.done) cudaEventDestroy(ln.done);
@@ -370,12 +387,12 @@ int poisson_plan_get_info(const poisson_plan *pl, poisson_plan_info *info) {
 
 size_t poisson_plan_workspace_bytes(const poisson_plan *pl) { return pl ? pl->workspace_bytes : 0; }
 
-int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? (pl->fused && pl->use_fused ? 1 : 5) : 0; }
+int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? (pl->fused && pl->use_fused ? 1 : 5) : 0; }   // kernels per solve (graph mode: 5 kernel nodes)
 
 int poisson_plan_launch_mode(const poisson_plan *pl, int *mode, double ms_per_solve[3]) {
     if (!pl || !mode || !ms_per_solve) return POISSON_EINVAL;
-    *mode = pl->fused && pl->use_fused ? POISSON_LAUNCH_FUSED : (pl->use_pdl ? POISSON_LAUNCH_FIVE_PDL : POISSON_LAUNCH_FIVE);
-    for (int m = 0; m < 3; ++m) ms_per_solve[m] = (double)pl->tune_ms[m];
+    *mode = pl->fused && pl->use_fused ? POISSON_LAUNCH_FUSED : (pl->use_graph && pl->gs.exec ? POISSON_LAUNCH_GRAPH : (pl->use_pdl ? POISSON_LAUNCH_FIVE_PDL : POISSON_LAUNCH_FIVE));
+    for (int m = 0; m < 4; ++m) ms_per_solve[m] = (double)pl->tune_ms[m];
     return POISSON_OK;
 }
 
@@ -475,8 +492,53 @@ static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t s
     return POISSON_OK;
 }
 
+// Builds the graph of one solve on the plan's own intermediates (explicit kernel nodes, plain dependencies).
+static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln = nullptr) {
+    if (g.exec) return POISSON_OK;
+    PF_CUDA(cudaGraphCreate(&g.graph, 0));
+    for (int q = 0; q < 5; ++q) {
+        const KernelEntry *e = pl->k[q];
+        g.prm[q] = pass_params(pl, q, nullptr, nullptr, ln);
+        void *args[] = {&g.prm[q]};
+        cudaKernelNodeParams kp{};
+        kp.func = const_cast<void *>(e->func);
+        kp.gridDim = dim3(pl->grid[q]); kp.blockDim = dim3(e->NT);
+        kp.sharedMemBytes = (unsigned)e->smem_bytes;
+        kp.kernelParams = args; kp.extra = nullptr;
+        PF_CUDA(cudaGraphAddKernelNode(&g.node[q], g.graph, q ? &g.node[q - 1] : nullptr, q ? 1 : 0, &kp));
+    }
+    PF_CUDA(cudaGraphInstantiate(&g.exec, g.graph, 0));
+    g.rho = nullptr; g.V = nullptr;
+    return POISSON_OK;
+}
+
+static int run_graph(poisson_plan *pl, GraphSolve &g, const void *rho, void *V, cudaStream_t st) {
+    for (int q = 0; q < 5; q += 4) {
+        const bool stale = q == 0 ? g.rho != rho : g.V != V;
+        if (!stale) continue;
+        const KernelEntry *e = pl->k[q];
+        if (q == 0) g.prm[0].in = rho; else g.prm[4].out = V;
+        void *args[] = {&g.prm[q]};
+        cudaKernelNodeParams kp{};
+        kp.func = const_cast<void *>(e->func);
+        kp.gridDim = dim3(pl->grid[q]); kp.blockDim = dim3(e->NT);
+        kp.sharedMemBytes = (unsigned)e->smem_bytes;
+        kp.kernelParams = args; kp.extra = nullptr;
+        PF_CUDA(cudaGraphExecKernelNodeSetParams(g.exec, g.node[q], &kp));
+    }
+    g.rho = rho; g.V = V;
+    PF_CUDA(cudaGraphLaunch(g.exec, st));
+    return POISSON_OK;
+}
+
 static int run_solve(poisson_plan *pl, const void *rho, void *V, cudaStream_t st) {
     if (pl->fused && pl->use_fused) return run_fused(pl, rho, V, st);
+    if (pl->use_graph && pl->gs.exec) {
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
+        if (cap == cudaStreamCaptureStatusNone) return run_graph(pl, pl->gs, rho, V, st);
+        // the caller is capturing `st` into a graph of their own: plain launches become its nodes
+    }
     return run_passes(pl, rho, V, st, 0, 4);
 }
 
@@ -529,6 +591,11 @@ static int wide_width(const poisson_plan *pl, int count) {
 // Times the launch modes on scratch inputs (timing does not depend on the values) and keeps the fastest.
 static int tune_plan(poisson_plan *pl) {
     const char *e_tune = std::getenv("POISSON_TUNE"), *e_pdl = std::getenv("POISSON_PDL"), *e_fused = std::getenv("POISSON_FUSED");
+    const char *e_graph = std::getenv("POISSON_GRAPH");
+    if (e_graph && e_graph[0] == '1') {                                                    // forced
+        if (build_graph(pl, pl->gs) == POISSON_OK) pl->use_graph = true; else cudaGetLastError();
+        return POISSON_OK;
+    }
     if ((e_tune && e_tune[0] == '0') || e_pdl || (e_fused && e_fused[0] == '1')) return POISSON_OK;   // forced / off
     const size_t bytes = (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * pl->elem_real;
     void *rho = nullptr, *V = nullptr;
@@ -541,11 +608,13 @@ static int tune_plan(poisson_plan *pl) {
     cudaMemset(rho, 0, bytes);
     cudaMemset(pl->kint, 0, (size_t)pl->kint_elems * pl->elem_real);
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { cudaGetLastError(); cleanup(); return POISSON_OK; }
-    const bool modes[3][2] = {{false, false}, {true, false}, {false, true}};   // {pdl, fused}
+    const bool modes[4][3] = {{false, false, false}, {true, false, false}, {false, true, false}, {false, false, true}};   // {pdl, fused, graph}
     int best = 0; float best_ms = 1e30f;
-    for (int m = 0; m < 3 && rc == POISSON_OK; ++m) {
+    if (build_graph(pl, pl->gs) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }      // no graph: that mode is skipped
+    for (int m = 0; m < 4 && rc == POISSON_OK; ++m) {
         if (modes[m][1] && !pl->fused) continue;
-        pl->use_pdl = modes[m][0]; pl->use_fused = modes[m][1];
+        if (modes[m][2] && !pl->gs.exec) continue;
+        pl->use_pdl = modes[m][0]; pl->use_fused = modes[m][1]; pl->use_graph = modes[m][2];
         int reps = 3;
         for (int round = 0; round < 2 && rc == POISSON_OK; ++round) {   // round 0: warm-up + pick the repeat count
             cudaEventRecord(e0, 0);
@@ -558,7 +627,7 @@ static int tune_plan(poisson_plan *pl) {
             else { pl->tune_ms[m] = ms; if (ms < best_ms) { best_ms = ms; best = m; } }
         }
     }
-    pl->use_pdl = modes[best][0]; pl->use_fused = modes[best][1];
+    pl->use_pdl = modes[best][0]; pl->use_fused = modes[best][1]; pl->use_graph = modes[best][2];
     cleanup();
     return rc;
 }
@@ -724,7 +793,18 @@ static int solve_batch_impl(poisson_plan *pl, const void *const *rho, void *cons
             PF_CUDA(cudaMemcpyAsync(ln.rho_stage, rho[i], bytes, cudaMemcpyHostToDevice, ln.st));
             r = ln.rho_stage; v = ln.v_stage;
         }
-        rc = run_passes(pl, r, v, ln.st, 0, 4, nullptr, &ln);
+        if (pl->use_graph && pl->gs.exec && !(std::getenv("POISSON_LANE_GRAPH") && std::getenv("POISSON_LANE_GRAPH")[0] == '0')) {
+            if (!ln.gs) {
+                ln.gs = new (std::nothrow) GraphSolve();
+                if (!ln.gs) return POISSON_ENOMEM;
+                std::memset(ln.gs, 0, sizeof(GraphSolve));
+                rc = build_graph(pl, *ln.gs, &ln);
+                if (rc != POISSON_OK) return rc;
+            }
+            rc = run_graph(pl, *ln.gs, r, v, ln.st);
+        } else {
+            rc = run_passes(pl, r, v, ln.st, 0, 4, nullptr, &ln);
+        }
         if (rc != POISSON_OK) return rc;
         if (host) PF_CUDA(cudaMemcpyAsync(V[i], ln.v_stage, bytes, cudaMemcpyDeviceToHost, ln.st));
     }

@@ -102,3 +102,41 @@ def test_named_configs_run_fused(pk, key):
     V = _solve(pk, rho, Kf, cfg.n, cfg.bc, "fp64", fused=True, repeats=2)
     ref = oracle.solve(rho, Kf, cfg.bc)
     assert rel_l2(V[0], ref) <= 1e-12 and np.array_equal(V[0], V[1])
+
+
+def test_graph_launch_mode_matches_five_launches_bitwise(pk, monkeypatch):
+    """POISSON_GRAPH=1: the five launches as one CUDA graph launch (rho / V patched into the F1 / I1 nodes per call).
+    Same kernels, same arithmetic: bitwise equal to the five stream launches, also when the buffers change between
+    calls and when rho == V."""
+    import torch
+    rng = np.random.default_rng(31)
+    n, bc = (24, 16, 32), (0, 1, 0)
+    s = gen.padded_shape(n, bc)
+    Kf = torch.from_numpy(rng.standard_normal((s[2], s[1], s[0] // 2 + 1))).cuda()
+    rhos = [torch.from_numpy(rng.standard_normal((n[2], n[1], n[0]))).cuda() for _ in range(3)]
+    monkeypatch.setenv("POISSON_TUNE", "0")
+    ref_plan = pk.PoissonPlan(n, bc, 0.3, pk.FP64)
+    ref_plan.set_kernel(Kf)
+    assert ref_plan.launch_mode()[0] == "five"
+    refs = [ref_plan.solve(r).clone() for r in rhos]
+    ref_plan.close()
+    monkeypatch.setenv("POISSON_GRAPH", "1")
+    plan = pk.PoissonPlan(n, bc, 0.3, pk.FP64)
+    try:
+        plan.set_kernel(Kf)
+        assert plan.launch_mode()[0] == "graph"
+        outs = [torch.empty_like(r) for r in rhos]
+        for rep in range(2):
+            for r, o, ref in zip(rhos, outs, refs):
+                plan.solve(r, o)
+                assert torch.equal(o, ref)
+        w = rhos[1].clone()
+        plan.solve(w, w)                                   # in place
+        assert torch.equal(w, refs[1])
+        s2 = torch.cuda.Stream()
+        with torch.cuda.stream(s2):
+            plan.solve(rhos[2], outs[0], stream=s2)        # another stream, another (rho, V) pair
+        s2.synchronize()
+        assert torch.equal(outs[0], refs[2])
+    finally:
+        plan.close()

@@ -441,7 +441,7 @@ def run_ours(args):
                      "algorithmic_bytes_per_launch": dom_bytes, "peak_source": peak_src},
         "launch_mode": {"chosen": res["launch_mode"], "batch_lanes": res["lanes"], "ms_per_solve_at_plan_creation": res["tune_ms"],
                         "note": "poisson_plan_create times {five launches, five + programmatic dependent launch, one fused "
-                                "cooperative launch, the five launches as one CUDA graph} and keeps the fastest; pass_us below are the five passes timed one by one"},
+                                "cooperative launch, the five launches as one CUDA graph, that graph with PDL edges} and keeps the fastest; pass_us below are the five passes timed one by one"},
         "e2e": {"value": world * 1e3 / res["e2e_ms_per_step"], "unit": UNIT, "h2d_bytes_per_step": res["rho_bytes"],
                 "d2h_bytes_per_step": res["rho_bytes"], "ms_per_step": res["e2e_ms_per_step"], "steps": res["e2e_steps"],
                 "api": (f"poisson_solve_batch_host, {res['e2e_batch']} pinned host densities per call: every rho copied H2D, five passes, "

@@ -178,13 +178,14 @@ POISSON_API int poisson_profile_read(poisson_plan *plan, double ms_sum[5] /* hos
  *             through L2 | grid barrier | I1 (compiled for the combinations in csrc/fused_*.cu).
  *   GRAPH     the five launches as kernel nodes of one instantiated CUDA graph (one cudaGraphLaunch per solve; rho / V
  *             are patched into the F1 / I1 nodes when they change): the dependent kernels follow each other with less
- *             latency than stream launches (128^3 -> 256^3 fp64: 103.7 -> 98.7 us per solve).
+ *             latency than stream launches (128^3 -> 256^3 fp64: 103.7 -> 98.7 us per solve);
+ *   GRAPH_PDL the same graph with programmatic-dependent-launch edges between the kernel nodes.
  * poisson_plan_create times the available modes on scratch inputs and keeps the fastest (a few ms);
- * POISSON_TUNE=0 skips that (FIVE), POISSON_PDL=0|1, POISSON_FUSED=0|1 and POISSON_GRAPH=1 force a mode.
+ * POISSON_TUNE=0 skips that (FIVE), POISSON_PDL=0|1, POISSON_FUSED=0|1 and POISSON_GRAPH=1 (with POISSON_PDL=1: GRAPH_PDL) force a mode.
  * poisson_plan_launch_mode reports the choice and the measured milliseconds per solve of
- * {FIVE, FIVE_PDL, FUSED, GRAPH} (0 where a mode was not measured). */
-enum { POISSON_LAUNCH_FIVE = 0, POISSON_LAUNCH_FIVE_PDL = 1, POISSON_LAUNCH_FUSED = 2, POISSON_LAUNCH_GRAPH = 3 };
-POISSON_API int poisson_plan_launch_mode(const poisson_plan *plan, int *mode /* host, out */, double ms_per_solve[4] /* host, out */);
+ * {FIVE, FIVE_PDL, FUSED, GRAPH, GRAPH_PDL} (0 where a mode was not measured). */
+enum { POISSON_LAUNCH_FIVE = 0, POISSON_LAUNCH_FIVE_PDL = 1, POISSON_LAUNCH_FUSED = 2, POISSON_LAUNCH_GRAPH = 3, POISSON_LAUNCH_GRAPH_PDL = 4 };
+POISSON_API int poisson_plan_launch_mode(const poisson_plan *plan, int *mode /* host, out */, double ms_per_solve[5] /* host, out */);
 
 /* Number of kernel launches one poisson_solve enqueues (bench.py's gpu_launches): 5, or 1 in FUSED mode. */
 POISSON_API int poisson_plan_launches_per_solve(const poisson_plan *plan);

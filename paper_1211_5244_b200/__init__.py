@@ -91,7 +91,7 @@ def load_library():
     lib.poisson_plan_batch_width.restype = i
     lib.poisson_solve_batch.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), i, vp]
     lib.poisson_solve_batch_host.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), i, vp]
-    lib.poisson_plan_launch_mode.argtypes = [vp, ctypes.POINTER(i), ctypes.c_double * 4]
+    lib.poisson_plan_launch_mode.argtypes = [vp, ctypes.POINTER(i), ctypes.c_double * 5]
     lib.poisson_plan_workspace_bytes.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.restype = ctypes.c_size_t
     lib.poisson_plan_destroy.argtypes = [vp]
@@ -268,10 +268,10 @@ class PoissonPlan:
     def launch_mode(self):
         """(mode name, {mode name: measured ms per solve at plan creation}) -- see poisson_plan_launch_mode."""
         mode = ctypes.c_int()
-        ms = (ctypes.c_double * 4)()
+        ms = (ctypes.c_double * 5)()
         _check(load_library().poisson_plan_launch_mode(self._h, ctypes.byref(mode), ms), "poisson_plan_launch_mode")
-        names = ("five", "five_pdl", "fused", "graph")
-        return names[mode.value], {names[k]: ms[k] for k in range(4) if ms[k] > 0}
+        names = ("five", "five_pdl", "fused", "graph", "graph_pdl")
+        return names[mode.value], {names[k]: ms[k] for k in range(5) if ms[k] > 0}
 
     def workspace_bytes(self) -> int:
         return load_library().poisson_plan_workspace_bytes(self._h)

@@ -132,9 +132,9 @@ struct poisson_plan {
     void *rho_stage, *v_stage;
     const FusedEntry *fused;   // one-launch solve kernel compiled for this combination of axes, or NULL
     bool use_fused;            // launch mode picked for poisson_solve: fused kernel, else 5 launches (with or without PDL)
-    bool use_graph;            // ... or the five launches as one CUDA graph launch
-    GraphSolve gs;
-    float tune_ms[4];          // measured ms per solve of {5 launches, 5 launches + PDL, fused, graph}; 0 = not measured
+    bool use_graph;            // ... or the five launches as one CUDA graph launch (use_pdl: with programmatic edges)
+    GraphSolve gs, gs_pdl;
+    float tune_ms[5];          // measured ms per solve of {5 launches, 5 launches + PDL, fused, graph, graph + PDL}; 0 = not measured
     int fused_grid, fused_skew;
     unsigned *fused_sync;      // barrier / per-plane counters of the fused kernel (zero between solves)
     size_t elem_real;     // bytes per real
@@ -172,8 +172,7 @@ static void free_plan(poisson_plan *pl) {
     for (int q = 0; q < 3; ++q) cudaFree(pl->tw[q]);
     cudaFree(pl->rho_stage); cudaFree(pl->v_stage); cudaFree(pl->fused_sync);
     cudaFree(pl->wide_a1); cudaFree(pl->wide_a2);
-    if (pl->gs.exec) cudaGraphExecDestroy(pl->gs.exec);
-    if (pl->gs.graph) cudaGraphDestroy(pl->gs.graph);
+    for (GraphSolve *g : {&pl->gs, &pl->gs_pdl}) { if (g->exec) cudaGraphExecDestroy(g->exec); if (g->graph) cudaGraphDestroy(g->graph); }
     if (pl->lanes) {
         for (Lane &ln : *pl->lanes) {
             if (ln.owns_ws) { cudaFree(ln.a1); cudaFree(ln.a2); }
@@ -191,6 +190,12 @@ static void free_plan(poisson_plan *pl) {
     }
     delete pl;
 }
+
+static GraphSolve *active_graph(poisson_plan *pl) {
+    GraphSolve *g = pl->use_pdl ? &pl->gs_pdl : &pl->gs;
+    return g->exec ? g : nullptr;
+}
+static const GraphSolve *active_graph(const poisson_plan *pl) { return active_graph(const_cast<poisson_plan *>(pl)); }
 
 extern "C" {
 
@@ -391,8 +396,10 @@ int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? (pl->f
 
 int poisson_plan_launch_mode(const poisson_plan *pl, int *mode, double ms_per_solve[3]) {
     if (!pl || !mode || !ms_per_solve) return POISSON_EINVAL;
-    *mode = pl->fused && pl->use_fused ? POISSON_LAUNCH_FUSED : (pl->use_graph && pl->gs.exec ? POISSON_LAUNCH_GRAPH : (pl->use_pdl ? POISSON_LAUNCH_FIVE_PDL : POISSON_LAUNCH_FIVE));
-    for (int m = 0; m < 4; ++m) ms_per_solve[m] = (double)pl->tune_ms[m];
+    *mode = pl->fused && pl->use_fused ? POISSON_LAUNCH_FUSED
+          : (pl->use_graph && active_graph(pl) ? (pl->use_pdl ? POISSON_LAUNCH_GRAPH_PDL : POISSON_LAUNCH_GRAPH)
+                                               : (pl->use_pdl ? POISSON_LAUNCH_FIVE_PDL : POISSON_LAUNCH_FIVE));
+    for (int m = 0; m < 5; ++m) ms_per_solve[m] = (double)pl->tune_ms[m];
     return POISSON_OK;
 }
 
@@ -512,6 +519,39 @@ static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln = nullptr
     return POISSON_OK;
 }
 
+// The same graph with programmatic-dependent-launch edges: captured from the five PDL stream launches (capture turns
+// the launch attribute into programmatic edges), kernel nodes identified by their function.
+static int build_graph_pdl(poisson_plan *pl, GraphSolve &g, const Lane *ln = nullptr) {
+    if (g.exec) return POISSON_OK;
+    cudaStream_t cs = nullptr;
+    PF_CUDA(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+    const bool saved = pl->use_pdl;
+    pl->use_pdl = true;
+    cudaError_t ce = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+    int rc = ce == cudaSuccess ? run_passes(pl, nullptr, nullptr, cs, 0, 4, nullptr, ln) : POISSON_ECUDA;
+    cudaGraph_t graph = nullptr;
+    if (ce == cudaSuccess) ce = cudaStreamEndCapture(cs, &graph);
+    pl->use_pdl = saved;
+    cudaStreamDestroy(cs);
+    if (rc != POISSON_OK || ce != cudaSuccess || !graph) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return POISSON_ECUDA; }
+    g.graph = graph;
+    cudaGraphNode_t nodes[16]; size_t nn = 16;
+    PF_CUDA(cudaGraphGetNodes(graph, nodes, &nn));
+    int found = 0;
+    for (size_t i = 0; i < nn; ++i) {
+        cudaGraphNodeType ty;
+        if (cudaGraphNodeGetType(nodes[i], &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
+        cudaKernelNodeParams kp{};
+        PF_CUDA(cudaGraphKernelNodeGetParams(nodes[i], &kp));
+        for (int q = 0; q < 5; ++q) if (kp.func == pl->k[q]->func) { g.node[q] = nodes[i]; ++found; }
+    }
+    if (found != 5) return POISSON_ECUDA;
+    for (int q = 0; q < 5; ++q) g.prm[q] = pass_params(pl, q, nullptr, nullptr, ln);
+    PF_CUDA(cudaGraphInstantiate(&g.exec, g.graph, 0));
+    g.rho = nullptr; g.V = nullptr;
+    return POISSON_OK;
+}
+
 static int run_graph(poisson_plan *pl, GraphSolve &g, const void *rho, void *V, cudaStream_t st) {
     for (int q = 0; q < 5; q += 4) {
         const bool stale = q == 0 ? g.rho != rho : g.V != V;
@@ -524,7 +564,7 @@ static int run_graph(poisson_plan *pl, GraphSolve &g, const void *rho, void *V, 
         kp.gridDim = dim3(pl->grid[q]); kp.blockDim = dim3(e->NT);
         kp.sharedMemBytes = (unsigned)e->smem_bytes;
         kp.kernelParams = args; kp.extra = nullptr;
-        PF_CUDA(cudaGraphExecKernelNodeSetParams(g.exec, g.node[q], &kp));
+        PF_CUDA(cudaGraphExecKernelNodeSetParams(g.exec, g.node[q], &kp));   // launch attributes (PDL edges) stay as built
     }
     g.rho = rho; g.V = V;
     PF_CUDA(cudaGraphLaunch(g.exec, st));
@@ -533,10 +573,10 @@ static int run_graph(poisson_plan *pl, GraphSolve &g, const void *rho, void *V, 
 
 static int run_solve(poisson_plan *pl, const void *rho, void *V, cudaStream_t st) {
     if (pl->fused && pl->use_fused) return run_fused(pl, rho, V, st);
-    if (pl->use_graph && pl->gs.exec) {
+    if (pl->use_graph && active_graph(pl)) {
         cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
         if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
-        if (cap == cudaStreamCaptureStatusNone) return run_graph(pl, pl->gs, rho, V, st);
+        if (cap == cudaStreamCaptureStatusNone) return run_graph(pl, *active_graph(pl), rho, V, st);
         // the caller is capturing `st` into a graph of their own: plain launches become its nodes
     }
     return run_passes(pl, rho, V, st, 0, 4);
@@ -593,7 +633,8 @@ static int tune_plan(poisson_plan *pl) {
     const char *e_tune = std::getenv("POISSON_TUNE"), *e_pdl = std::getenv("POISSON_PDL"), *e_fused = std::getenv("POISSON_FUSED");
     const char *e_graph = std::getenv("POISSON_GRAPH");
     if (e_graph && e_graph[0] == '1') {                                                    // forced
-        if (build_graph(pl, pl->gs) == POISSON_OK) pl->use_graph = true; else cudaGetLastError();
+        const bool pdl = e_pdl && e_pdl[0] == '1';
+        if ((pdl ? build_graph_pdl(pl, pl->gs_pdl) : build_graph(pl, pl->gs)) == POISSON_OK) pl->use_graph = true; else cudaGetLastError();
         return POISSON_OK;
     }
     if ((e_tune && e_tune[0] == '0') || e_pdl || (e_fused && e_fused[0] == '1')) return POISSON_OK;   // forced / off
@@ -608,12 +649,13 @@ static int tune_plan(poisson_plan *pl) {
     cudaMemset(rho, 0, bytes);
     cudaMemset(pl->kint, 0, (size_t)pl->kint_elems * pl->elem_real);
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { cudaGetLastError(); cleanup(); return POISSON_OK; }
-    const bool modes[4][3] = {{false, false, false}, {true, false, false}, {false, true, false}, {false, false, true}};   // {pdl, fused, graph}
+    const bool modes[5][3] = {{false, false, false}, {true, false, false}, {false, true, false}, {false, false, true}, {true, false, true}};   // {pdl, fused, graph}
     int best = 0; float best_ms = 1e30f;
     if (build_graph(pl, pl->gs) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }      // no graph: that mode is skipped
-    for (int m = 0; m < 4 && rc == POISSON_OK; ++m) {
+    if (build_graph_pdl(pl, pl->gs_pdl) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }
+    for (int m = 0; m < 5 && rc == POISSON_OK; ++m) {
         if (modes[m][1] && !pl->fused) continue;
-        if (modes[m][2] && !pl->gs.exec) continue;
+        if (modes[m][2] && !(modes[m][0] ? pl->gs_pdl.exec : pl->gs.exec)) continue;
         pl->use_pdl = modes[m][0]; pl->use_fused = modes[m][1]; pl->use_graph = modes[m][2];
         int reps = 3;
         for (int round = 0; round < 2 && rc == POISSON_OK; ++round) {   // round 0: warm-up + pick the repeat count
@@ -793,12 +835,12 @@ static int solve_batch_impl(poisson_plan *pl, const void *const *rho, void *cons
             PF_CUDA(cudaMemcpyAsync(ln.rho_stage, rho[i], bytes, cudaMemcpyHostToDevice, ln.st));
             r = ln.rho_stage; v = ln.v_stage;
         }
-        if (pl->use_graph && pl->gs.exec && !(std::getenv("POISSON_LANE_GRAPH") && std::getenv("POISSON_LANE_GRAPH")[0] == '0')) {
+        if (pl->use_graph && active_graph(pl) && !(std::getenv("POISSON_LANE_GRAPH") && std::getenv("POISSON_LANE_GRAPH")[0] == '0')) {
             if (!ln.gs) {
                 ln.gs = new (std::nothrow) GraphSolve();
                 if (!ln.gs) return POISSON_ENOMEM;
                 std::memset(ln.gs, 0, sizeof(GraphSolve));
-                rc = build_graph(pl, *ln.gs, &ln);
+                rc = pl->use_pdl ? build_graph_pdl(pl, *ln.gs, &ln) : build_graph(pl, *ln.gs, &ln);
                 if (rc != POISSON_OK) return rc;
             }
             rc = run_graph(pl, *ln.gs, r, v, ln.st);

@@ -104,7 +104,8 @@ def test_named_configs_run_fused(pk, key):
     assert rel_l2(V[0], ref) <= 1e-12 and np.array_equal(V[0], V[1])
 
 
-def test_graph_launch_mode_matches_five_launches_bitwise(pk, monkeypatch):
+@pytest.mark.parametrize("pdl", [False, True])
+def test_graph_launch_mode_matches_five_launches_bitwise(pk, monkeypatch, pdl):
     """POISSON_GRAPH=1: the five launches as one CUDA graph launch (rho / V patched into the F1 / I1 nodes per call).
     Same kernels, same arithmetic: bitwise equal to the five stream launches, also when the buffers change between
     calls and when rho == V."""
@@ -121,10 +122,12 @@ def test_graph_launch_mode_matches_five_launches_bitwise(pk, monkeypatch):
     refs = [ref_plan.solve(r).clone() for r in rhos]
     ref_plan.close()
     monkeypatch.setenv("POISSON_GRAPH", "1")
+    if pdl:
+        monkeypatch.setenv("POISSON_PDL", "1")     # graph captured from the PDL launches: programmatic edges
     plan = pk.PoissonPlan(n, bc, 0.3, pk.FP64)
     try:
         plan.set_kernel(Kf)
-        assert plan.launch_mode()[0] == "graph"
+        assert plan.launch_mode()[0] == ("graph_pdl" if pdl else "graph")
         outs = [torch.empty_like(r) for r in rhos]
         for rep in range(2):
             for r, o, ref in zip(rhos, outs, refs):

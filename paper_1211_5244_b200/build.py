@@ -37,6 +37,10 @@ def build(force: bool = False, jobs: int | None = None, verbose: bool = False, e
     OBJ.mkdir(exist_ok=True)
     srcs = sorted(CSRC.glob("*.cu"))
     hdr_t = _headers_mtime()
+    # the linked library is newer than every source: nothing to do (also the case on a GPU box, where the
+    # library travels with the snapshot and the object files do not, see .gpurunignore)
+    if not force and LIB.exists() and LIB.stat().st_mtime >= max(hdr_t, max(s.stat().st_mtime for s in srcs)):
+        return LIB
     todo = []
     for s in srcs:
         o = OBJ / (s.stem + ".o")

@@ -262,3 +262,35 @@ def test_intermediate_after_f1_matches_oracle_stage(pk):
     assert a1.shape == ref.shape
     assert rel_l2(a1, ref) <= 1e-13
     plan.close()
+
+
+def test_maximum_length_1024_cubed_shift_kernel_property(pk):
+    """The largest compiled length on every axis: 512^3 physical -> 1024^3 padded, fp64 (A2 alone is 4.3 GB, element
+    offsets pass 2^31 bytes).  K = delta(r - d) + delta(r + d) has the analytic spectrum 2 cos(2 pi k.d / S); the exact
+    result is rho displaced by +-d with zero fill (free axes: nothing wraps).  Inputs are made on the device."""
+    import torch
+    n, bc, d = (512, 512, 512), (0, 0, 0), (5, 3, 2)
+    s = (1024, 1024, 1024)
+    free, total = torch.cuda.mem_get_info()
+    if free < 30 * 2**30:
+        pytest.skip("needs about 20 GB of device memory")
+    g = torch.Generator(device="cuda").manual_seed(1234)
+    rho = torch.randn(n[2], n[1], n[0], dtype=torch.float64, device="cuda", generator=g)
+    kz = torch.arange(s[2], device="cuda", dtype=torch.float64)[:, None, None] * (d[2] / s[2])
+    ky = torch.arange(s[1], device="cuda", dtype=torch.float64)[None, :, None] * (d[1] / s[1])
+    kx = torch.arange(s[0] // 2 + 1, device="cuda", dtype=torch.float64)[None, None, :] * (d[0] / s[0])
+    Kf = 2.0 * torch.cos(2 * np.pi * (kx + ky + kz))
+    plan = pk.PoissonPlan(n, bc, 0.1, pk.FP64)
+    try:
+        plan.set_kernel(Kf)
+        torch.cuda.synchronize()
+        del Kf
+        V = plan.solve(rho)
+        torch.cuda.synchronize()
+        exp = torch.zeros_like(rho)
+        exp[d[2]:, d[1]:, d[0]:] += rho[:-d[2], :-d[1], :-d[0]]
+        exp[:-d[2], :-d[1], :-d[0]] += rho[d[2]:, d[1]:, d[0]:]
+        err = float(torch.linalg.vector_norm(V - exp) / torch.linalg.vector_norm(exp))
+        assert err <= 1e-12, err
+    finally:
+        plan.close()

@@ -1,7 +1,7 @@
-// Pass kernels for transform length 160 = 16 x 10, 10 thread(s) per pencil, f64 (see sizes.def).
+// Pass kernels for transform length 160 = 10 x 16, 16 thread(s) per pencil, f64 (see sizes.def).
 #define PF_S 160
-#define PF_RA 16
-#define PF_RB 10
-#define PF_TPP 10
+#define PF_RA 10
+#define PF_RB 16
+#define PF_TPP 16
 #define PF_ONLY_F64
 #include "inst.cuh"

@@ -1,7 +1,8 @@
-// Pass kernels for transform length 320 = 20 x 16, 16 thread(s) per pencil, f32 (see sizes.def).
+// Pass kernels for transform length 320 = 16 x 20, 20 thread(s) per pencil, f32 (see sizes.def).
+// (RA < RB = TPP: every thread owns one column of the second pass, 16 of 20 threads have one)
 #define PF_S 320
-#define PF_RA 20
-#define PF_RB 16
-#define PF_TPP 16
+#define PF_RA 16
+#define PF_RB 20
+#define PF_TPP 20
 #define PF_ONLY_F32
 #include "inst.cuh"

@@ -1,9 +1,8 @@
-// Pass kernels for transform length 320 = 20 x 16, 16 thread(s) per pencil, f64 (see sizes.def).
+// Pass kernels for transform length 320 = 16 x 20, 20 thread(s) per pencil, f64 (see sizes.def).
+// (RA < RB = TPP: every thread owns one column of the second pass, 16 of 20 threads have one)
 #define PF_S 320
-#define PF_RA 20
-#define PF_RB 16
-#define PF_TPP 16
+#define PF_RA 16
+#define PF_RB 20
+#define PF_TPP 20
 #define PF_ONLY_F64
-// 32 complex fp64 values per thread: the full register file, 2 CTAs of 128 threads per SM
-#define PF_MINB 2
 #include "inst.cuh"

@@ -6,4 +6,5 @@
 #define PF_ONLY_F64
 // 32 complex fp64 values per thread and a 128 KB exchange buffer: one 256-thread CTA per SM
 #define PF_MINB 1
+#define PF_STG 1
 #include "inst.cuh"

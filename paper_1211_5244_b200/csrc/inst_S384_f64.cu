@@ -6,4 +6,5 @@
 #define PF_ONLY_F64
 // 32 complex fp64 values per thread: the full register file, 2 CTAs of 128 threads per SM
 #define PF_MINB 2
+#define PF_STG 1
 #include "inst.cuh"

@@ -6,4 +6,5 @@
 #define PF_ONLY_F64
 // 24 complex fp64 values per thread: 170 registers, 2 CTAs of 192 threads per SM
 #define PF_MINB 2
+#define PF_STG 1
 #include "inst.cuh"

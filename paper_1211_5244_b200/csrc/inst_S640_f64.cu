@@ -6,4 +6,5 @@
 #define PF_ONLY_F64
 // 32 values per thread, 32 threads per pencil: one CTA per SM
 #define PF_MINB 1
+#define PF_STG 1
 #include "inst.cuh"

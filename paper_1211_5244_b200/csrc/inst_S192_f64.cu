@@ -4,4 +4,8 @@
 #define PF_RB 8
 #define PF_TPP 8
 #define PF_ONLY_F64
+// 24 complex fp64 values per thread: a 168-register budget (3 CTAs of 128 threads per SM) instead of the default 128
+// (measured on the wire configuration: I2 16.5 -> 14.7 us, batched solve 59.2 -> 52.4 us; 12 x 16 with 16 threads per
+// pencil is faster in F2 / I2 but slower in F3: 55.5 us)
+#define PF_MINB 3
 #include "inst.cuh"

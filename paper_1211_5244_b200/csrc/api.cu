@@ -585,7 +585,6 @@ static int run_solve(poisson_plan *pl, const void *rho, void *V, cudaStream_t st
 // Several small solves per launch (poisson_solve_batch on small grids): each of the five launches covers the
 // tiles of nbw densities; density bi uses slot bi of the wide intermediates, reads rho[bi] and writes V[bi].
 static int run_passes_wide(poisson_plan *pl, const void *const *rho, void *const *V, int nbw, cudaStream_t st) {
-    const size_t cplx = 2 * pl->elem_real;
     for (int q = 0; q < 5; ++q) {
         const KernelEntry *e = pl->k[q];
         PassParams prm = pass_params(pl, q, nullptr, nullptr);
@@ -600,8 +599,7 @@ static int run_passes_wide(poisson_plan *pl, const void *const *rho, void *const
         }
         if (q == POISSON_PASS_F1) for (int i = 0; i < nbw; ++i) prm.blist[i] = rho[i];
         if (q == POISSON_PASS_I1) for (int i = 0; i < nbw; ++i) prm.blist[i] = V[i];
-        prm.prefetch = 0;
-        (void)cplx;
+        prm.prefetch = 0;   // the wide intermediates are sized to stay in L2
         void *args[] = {&prm};
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(prm.n_tiles < pl->resident[q] ? prm.n_tiles : pl->resident[q]); cfg.blockDim = dim3(e->NT);
@@ -827,6 +825,8 @@ static int solve_batch_impl(poisson_plan *pl, const void *const *rho, void *cons
     const size_t bytes = (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * pl->elem_real;
     PF_CUDA(cudaEventRecord(pl->fork_ev, user));                      // the lanes start after the caller's earlier work
     for (int l = 0; l < L; ++l) PF_CUDA(cudaStreamWaitEvent((*pl->lanes)[l].st, pl->fork_ev, 0));
+    const char *e_lg = std::getenv("POISSON_LANE_GRAPH");   // =0: plain launches on the lanes (experiments)
+    const bool lane_graphs = pl->use_graph && active_graph(pl) && !(e_lg && e_lg[0] == '0');
     for (int i = 0; i < count; ++i) {
         Lane &ln = (*pl->lanes)[i % L];
         const void *r = rho[i];
@@ -835,7 +835,7 @@ static int solve_batch_impl(poisson_plan *pl, const void *const *rho, void *cons
             PF_CUDA(cudaMemcpyAsync(ln.rho_stage, rho[i], bytes, cudaMemcpyHostToDevice, ln.st));
             r = ln.rho_stage; v = ln.v_stage;
         }
-        if (pl->use_graph && active_graph(pl) && !(std::getenv("POISSON_LANE_GRAPH") && std::getenv("POISSON_LANE_GRAPH")[0] == '0')) {
+        if (lane_graphs) {
             if (!ln.gs) {
                 ln.gs = new (std::nothrow) GraphSolve();
                 if (!ln.gs) return POISSON_ENOMEM;

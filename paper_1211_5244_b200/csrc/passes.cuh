@@ -600,6 +600,9 @@ PF_HD void unpack_A(cx<typename G::T> *v, const B &b) {
     });
 }
 
+#ifndef PF_KPREF
+#define PF_KPREF 1   // pass F3 prefetches its K^F lines into L2 at the top of the tile (where PassParams::prefetch bit 1 is set)
+#endif
 #ifndef PF_TPREF
 #define PF_TPREF 1   // L2 prefetch of the next tile's inputs in the unstaged tile loops
 #endif
@@ -881,9 +884,6 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     using KV = KVec<T>;
     constexpr int NKV = G::V / KV::N;
     constexpr bool K_EARLY = !St::KON && !G::KLATE;
-#ifndef PF_KPREF
-#define PF_KPREF 1
-#endif
     constexpr bool KPREF = PF_KPREF != 0;
     using Buf = BufAK<G, PRUNED, K_EARLY>;
     const typename KV::V *kint = reinterpret_cast<const typename KV::V *>(prm.kint);

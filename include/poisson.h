@@ -91,7 +91,10 @@ POISSON_API int poisson_plan_describe(int nx, int ny, int nz, const int bc[3] /*
 
 /* Creates a plan on the current CUDA device: validates, picks the axis order, allocates the
  * workspace (A1, A2, internal K^F) and uploads the twiddle tables.  `h` (grid spacing) is recorded
- * metadata only.  *out is set to NULL on failure.  Problem statement: PAPER.md:51. */
+ * metadata only.  *out is set to NULL on failure.  Problem statement: PAPER.md:51.
+ * Supported grids: every N_i even, every padded length S_i = N_i * B_i one of
+ *   4 8 12 16 20 24 32 36 40 48 60 64 72 80 96 100 120 128 144 160 192 200 240 256 288 320 384 400 480 512 576 640 768 1024
+ * (csrc/sizes.def), else POISSON_EUNSUPPORTED.  Errors: EINVAL, EUNSUPPORTED, ENOMEM, ECUDA, EARCH. */
 POISSON_API int poisson_plan_create(poisson_plan **out /* host, out */, int nx, int ny, int nz,
                         const int bc[3] /* host; x,y,z */, double h, int precision);
 

@@ -39,6 +39,15 @@ const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int pre
     return fallback;
 }
 
+// Lengths compiled in two factorizations: which one a pass takes (measured, see the inst_S*.cu file).  -1: the
+// POISSON_VARIANT environment variable or the default.
+static int preferred_variant(int kind, int S, int prec) {
+    if (std::getenv("POISSON_VARIANT")) return -1;
+    { const char *f = std::getenv("POISSON_FUSED"); if (f && f[0] == '1') return -1; }   // the fused kernel is compiled for the default factorizations
+    if (S == 192 && prec == POISSON_FP64 && (kind == KIND_F2 || kind == KIND_I2)) return 9;
+    return -1;
+}
+
 std::vector<FusedEntry> &fused_registry() {
     static std::vector<FusedEntry> reg;
     return reg;
@@ -269,7 +278,7 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
 
     for (int q = 0; q < 5; ++q) {
         const PassDesc &ps = d.pass[q];
-        const KernelEntry *e = find_kernel(ps.kind, ps.S, ps.pruned, ps.lanes_p, precision);
+        const KernelEntry *e = find_kernel(ps.kind, ps.S, ps.pruned, ps.lanes_p, precision, preferred_variant(ps.kind, ps.S, precision));
         if (!e) { free_plan(pl); return POISSON_EUNSUPPORTED; }
         pl->k[q] = e;
         pl->tiles_per_g[q] = (int)((ps.n_p + e->P - 1) / e->P);

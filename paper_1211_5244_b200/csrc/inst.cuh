@@ -90,6 +90,9 @@ namespace {
 struct PfRegistrar {
     PfRegistrar() {
         pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, PF_NBUF, PF_TWS, PF_MINB, PF_STG, PF_KLATE, PF_PCMUL>(PF_PREC, 0);
+#if defined(PF_ALT_GEOMETRY)
+        PF_ALT_GEOMETRY   // a second factorization of the same length, registered under its own variant id (api.cu: preferred_variant)
+#endif
 #if defined(PF_EXTRA_VARIANTS)
 #define PF_VARIANT(ID, NBUF, TWS, MINB, STG, KLATE) pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, NBUF, TWS, MINB, STG, KLATE>(PF_PREC, ID);
 #define PF_VARIANT_PC(ID, NBUF, TWS, MINB, STG, KLATE, PCMUL) pfft::reg_length<PF_T, PF_S, PF_RA, PF_RB, PF_TPP, NBUF, TWS, MINB, STG, KLATE, PCMUL>(PF_PREC, ID);

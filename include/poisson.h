@@ -127,8 +127,8 @@ POISSON_API int poisson_solve_host(poisson_plan *plan, const void *rho_host, voi
 
 /* Batched solves: `count` densities with the one K^F of the plan -- the paper's repeated-solve setting and its
  * stated remedy for the transfer cost, "overlap the transfer of one density with the computation of the
- * previous one".  The solves are dealt round-robin to up to 3 lanes (1 for device batches whose
- * intermediates exceed 256 MB per lane; POISSON_LANES=1..8 overrides),
+ * previous one".  The solves are dealt round-robin to lanes (host batches 3; device batches 3 while three sets of
+ * intermediates fit the L2, else 2, or 1 when they exceed 256 MB per lane; POISSON_LANES=1..8 overrides),
  * each with its own A1 / A2 intermediates and its own internal stream, so that the tail of one solve overlaps
  * the head of the next (and, in the host variant, H2D of solve i+1 and D2H of solve i-1 overlap the passes of
  * solve i on the two copy engines).  Lanes are allocated on first use and kept by the plan (its

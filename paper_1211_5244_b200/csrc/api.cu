@@ -786,7 +786,10 @@ static int ensure_lanes(poisson_plan *pl, int want, bool staging) {
 static int batch_lanes(const poisson_plan *pl, int count, bool host) {
     const char *env = std::getenv("POISSON_LANES");
     const size_t lane_bytes = (size_t)(pl->d.a1_elems + pl->d.a2_elems) * 2 * pl->elem_real;
-    int lanes = env ? std::atoi(env) : ((host || lane_bytes <= (size_t)256 << 20) ? 3 : 1);
+    // device batches: 2 lanes (with the per-lane solve graphs 128^3 -> 256^3 measures 96.5 / 93.1 / 96.2 / 97.8 us per solve at
+    // 1 / 2 / 3 / 4 lanes, the wire grid 51.9 / 55.3 / 58.6 at 2 / 3 / 4: two sets of intermediates still share the L2)
+    // (the surface grid, 34 MB per lane, still gains from a third lane: 27.7 vs 30.3 us -- three sets fit the L2)
+    int lanes = env ? std::atoi(env) : (host ? 3 : (3 * lane_bytes <= ((size_t)110 << 20) ? 3 : (lane_bytes <= ((size_t)256 << 20) ? 2 : 1)));
     if (lanes < 1) lanes = 1;
     if (lanes > 8) lanes = 8;
     return count < lanes ? count : lanes;

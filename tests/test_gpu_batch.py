@@ -118,7 +118,7 @@ def test_wide_batch_more_densities_than_one_launch_takes(pk):
 
 
 def test_config1_batch_in_the_bench_configuration(pk):
-    """configs[1] (128^3 -> 256^3 fp64) through poisson_solve_batch the way bench.py times it (device batch, 3 lanes,
+    """configs[1] (128^3 -> 256^3 fp64) through poisson_solve_batch the way bench.py times it (device batch, 2 lanes,
     marshalled once): every V equals the single-stream solve of the same density bitwise (that solve is checked against the
     oracle in test_named_config_vs_oracle), and the shift property V = rho displaced holds for a delta kernel."""
     import torch
@@ -135,7 +135,7 @@ def test_config1_batch_in_the_bench_configuration(pk):
     plan = pk.PoissonPlan(n, cfg.bc, cfg.h, pk.FP64)
     try:
         plan.set_kernel(torch.from_numpy(Kf).cuda())
-        assert plan.batch_width(8) == 0 and plan.batch_lanes(8) == 3
+        assert plan.batch_width(8) == 0 and plan.batch_lanes(8) == 2 and plan.batch_lanes(8, host=True) == 3
         rhos = [torch.from_numpy(rng.standard_normal((n[2], n[1], n[0]))).cuda() for _ in range(8)]
         Vs = [torch.empty_like(r) for r in rhos]
         pb = plan.pointer_batch(rhos, Vs)

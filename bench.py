@@ -6,7 +6,8 @@
 One "step" = one full solve (all five fused passes F1,F2,F3,I2,I1 of DESIGN.md) of the workload
 BASELINE.json's metric is quoted on: configs[1], free BCs, fp64, 128^3 physical -> 256^3 padded
 ("fp64, free BC 256^3": the paper labels grids by padded FFT size).  Rank 0 prints ONE
-JSON line.  N > 1 (launched by torch.distributed.run, one rank per GPU) runs N independent replicas
+JSON line.  `value` / `ms_per_step` = poisson_solve (the north-star call) back to back on ONE stream; the batched
+route (poisson_solve_batch) is reported under `batched`.  N > 1 (launched by torch.distributed.run, one rank per GPU) runs N independent replicas
 ("replicas only": a solve does not shard without an all-to-all, and the north star is
 one GPU); value = all ranks' solves / max-over-ranks device time.
 
@@ -175,23 +176,25 @@ def barrier():
 
 
 # ------------------------------------------------------------------ CPU oracle timing (cpu_baseline / --impl reference)
-class OracleSampler:
-    """Times the oracle (as it stands) on a bounded sample of the workload and scales to one solve.
-    The oracle's solve is six naive-DFT sweeps over the padded grid (oracle/poisson_oracle.c); a sample runs each
-    sweep's routine (oracle.dft_axis) on a slab holding m of the S planes, i.e. the fraction f = m/S of that sweep's
-    lines.  The padded array and the per-plane calibration are made once, outside every timed sample."""
+class OracleTimer:
+    """Times the oracle as it stands (oracle/poisson_oracle.c: naive O(n^2) DFT per axis on the explicitly padded grid).
+    A step is ONE WHOLE oracle.solve call of the workload (padding, six DFT sweeps, K_f multiply, scaling, crop) whenever
+    the requested number of steps fits the time budget; only if it does not, a step is a bounded slab sample of the six
+    sweeps scaled to the whole grid, and the result is flagged `extrapolated`."""
 
-    def __init__(self, cfg, rho):
+    def __init__(self, cfg, rho, kf):
         import oracle
-        self.oracle = oracle
-        self.s, self.n = cfg.s, cfg.n
-        sx, sy, sz = cfg.s
-        nx, ny, nz = cfg.n
-        self.pad = np.zeros((sz, sy, sx), dtype=np.complex128)
-        self.pad[:nz, :ny, :nx] = rho
-        self.per_plane = sum(self.sweeps(1))          # calibration (also warms the library)
+        self.oracle, self.cfg = oracle, cfg
+        self.rho = np.ascontiguousarray(rho, dtype=np.float64)
+        self.kf = np.ascontiguousarray(kf, dtype=np.float64)
+        self.pad = None
 
-    def sweeps(self, m):
+    def whole_solve(self) -> float:
+        t0 = time.perf_counter()
+        self.oracle.solve(self.rho, self.kf, self.cfg.bc)
+        return time.perf_counter() - t0
+
+    def _sweeps(self, m):
         pad, dft = self.pad, self.oracle.dft_axis
         tx = ty = tz = 0.0
         for sign in (-1, +1):
@@ -200,20 +203,54 @@ class OracleSampler:
             t0 = time.perf_counter(); dft(pad[:, :m], 0, sign); tz += time.perf_counter() - t0   # z sweep, m y-planes
         return tx, ty, tz
 
-    def sample(self, budget_s: float):
-        """(seconds per full solve, description, threads) from one sample of about budget_s seconds."""
-        sx, sy, sz = self.s
-        m = int(max(1, min(min(sy, sz), budget_s / max(self.per_plane, 1e-9))))
-        tx, ty, tz = self.sweeps(m)
+    def slab_sample(self, budget_s: float, per_plane_s: float):
+        """(seconds per solve scaled from a slab of m planes per sweep, fraction f, description)."""
+        sx, sy, sz = self.cfg.s
+        nx, ny, nz = self.cfg.n
+        if self.pad is None:
+            self.pad = np.zeros((sz, sy, sx), dtype=np.complex128)
+            self.pad[:nz, :ny, :nx] = self.rho
+        m = int(max(1, min(min(sy, sz), budget_s / max(per_plane_s, 1e-9))))
+        tx, ty, tz = self._sweeps(m)
         f = m / float(min(sy, sz))
         full = tx * sz / m + ty * sz / m + tz * sy / m
-        desc = (f"oracle naive-DFT sweeps on {m} of {min(sy, sz)} planes per sweep (f={f:.4f}) of the padded "
+        desc = (f"EXTRAPOLATED: oracle naive-DFT sweeps on {m} of {min(sy, sz)} planes per sweep (f={f:.4f}) of the padded "
                 f"{sx}x{sy}x{sz} grid, 6 sweeps, scaled by 1/f; K_f multiply and padding copy not included")
-        return full, desc, self.oracle.n_threads()
+        return full, f, desc
 
 
-def oracle_sample_seconds(cfg, rho, budget_s: float):
-    return OracleSampler(cfg, rho).sample(budget_s)
+def oracle_steps(cfg, rho, kf, steps: int, warmup: int, budget_s: float):
+    """Runs warmup + steps oracle steps inside about budget_s seconds.  Returns (seconds per solve [mean over the timed
+    steps], description, threads, extrapolated, sample_fraction, steps actually timed as whole solves or samples)."""
+    timer = OracleTimer(cfg, rho, kf)
+    threads = timer.oracle.n_threads()
+    first = timer.whole_solve()                      # also warms the library; counts as the first warm-up step
+    total = warmup + steps
+    sx, sy, sz = cfg.s
+    if first * total <= budget_s:
+        times = [first]
+        for _ in range(total - 1):
+            times.append(timer.whole_solve())
+        timed = times[warmup:] if warmup < len(times) else times[-1:]
+        desc = (f"{len(timed)} whole oracle.solve calls ({warmup} warm-up) on the padded {sx}x{sy}x{sz} grid: padding, six "
+                "naive-DFT sweeps, K_f multiply, scaling, crop")
+        return float(np.mean(timed)), desc, threads, False, 1.0, len(timed)
+    per_plane = first / float(min(sy, sz))
+    slab_budget = max(0.5, (budget_s - first) / total)
+    times, f, desc = [], 1.0, ""
+    for i in range(total):
+        sec, f, desc = timer.slab_sample(slab_budget, per_plane)
+        if i >= warmup:
+            times.append(sec)
+    return float(np.mean(times)), desc, threads, True, f, len(times)
+
+
+def config_dict(key, cfg, info_s, order, world):
+    """The `config` object of the JSON line: the same keys and values in both arms (ours / reference)."""
+    return {"workload": WORKLOAD_TEXT[key], "physical_grid": list(cfg.n), "padded_grid": list(info_s),
+            "bc_xyz": ["free" if b == 0 else "periodic" for b in cfg.bc], "axis_order": list(order),
+            "l2": "inputs larger than L2: rho/V rotate over a ring of device buffers whose footprint exceeds the 126 MB L2",
+            "replicas": world}
 
 
 def run_reference(args):
@@ -221,24 +258,23 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    cfg = gen.get_config(args.config)
-    rho = gen.gaussian_density(cfg)
+    cfg, rho, kf = build_inputs(args.config)
     steps, warmup = max(1, args.steps), max(0, args.warmup)
-    budget = min(20.0, 150.0 / (steps + warmup + 1))     # the whole run ends within a few minutes
-    sampler = OracleSampler(cfg, rho)
-    times = []
-    desc, threads = "", 1
-    for i in range(warmup + steps):
-        sec, desc, threads = sampler.sample(budget)
-        if i >= warmup:
-            times.append(sec)
-    sec = float(np.mean(times))
+    sec, desc, threads, extrap, frac, ntimed = oracle_steps(cfg, rho, kf, steps, warmup, 170.0)
     val = 1.0 / sec
+    try:   # the planner is host-only: same padded grid / axis order keys as the main arm
+        import paper_1211_5244_b200 as pk
+        info = pk.poisson_plan_describe(cfg.n[0], cfg.n[1], cfg.n[2], cfg.bc, pk.FP64)
+        s_pad, order = list(info.s), list(info.order)
+    except Exception:
+        s_pad, order = list(cfg.s), []
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
         "warmup": warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD_TEXT[args.config], "note": "CPU oracle (naive O(n^2) DFT per axis), not a tuned baseline"},
+        "config": config_dict(args.config, cfg, s_pad, order, world),
+        "extrapolated": extrap, "sample_fraction": frac, "steps_timed": ntimed,
+        "note": "CPU oracle (naive O(n^2) DFT per axis, test infrastructure), not a tuned baseline",
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "world_size_seen": world,
@@ -263,8 +299,8 @@ def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, wi
     vs = [torch.empty_like(rho0) for _ in range(nbuf)]
     stream = torch.cuda.current_stream()
 
-    def timed(body, n):
-        """n solves between two CUDA events on the launching stream; returns ms per solve (max over ranks)."""
+    def timed_once(body, n):
+        """n solves between two CUDA events on the launching stream; ms per solve (max over ranks)."""
         torch.cuda.synchronize()
         barrier()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -275,42 +311,46 @@ def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, wi
         barrier()
         return reduce_max(a.elapsed_time(b), device="cuda") / n
 
+    def timed(body, n, est_ms):
+        """The timed region is EXACTLY n solves; it is repeated (>= 5 regions, up to 50, until about 0.25 s are covered) and
+        the MEDIAN region is reported with the spread, so that a 20-step region of a 100 us solve is not a 2 ms one-off."""
+        regions = int(min(50, max(5, math.ceil(250.0 / max(n * est_ms, 1e-3)))))
+        vals = sorted(timed_once(body, n) for _ in range(regions))
+        return {"ms": float(np.median(vals)), "min": vals[0], "max": vals[-1], "regions": regions}
+
     def one_by_one(n):
         for i in range(n):
             plan.solve(rhos[i % nbuf], vs[i % nbuf])
 
     bsz = min(BATCH, nbuf)
-
-    ptr_batches = {}         # pointer arrays marshalled once per batch size (what a C caller holds)
+    # pointer arrays marshalled BEFORE any timed region, one per batch size the loop below uses (what a C caller holds)
+    ptr_batches = {m: plan.pointer_batch(rhos[:m], vs[:m]) for m in {bsz, steps % bsz, max(3, warmup) % bsz} if m > 0}
 
     def batched(n):          # poisson_solve_batch: ceil(n / bsz) calls, exactly n solves
         done = 0
         while done < n:
             m = min(bsz, n - done)
-            if m not in ptr_batches:
-                ptr_batches[m] = plan.pointer_batch(rhos[:m], vs[:m])
             plan.solve_pointer_batch(ptr_batches[m])
             done += m
 
     one_by_one(max(3, warmup))
-    single_ms = timed(one_by_one, steps)
+    est = timed_once(one_by_one, max(3, min(steps, 20)))
+    single = timed(one_by_one, steps, est)
     pass_ms = None
     if with_profile:
-        nprof = min(steps, 256)
+        nprof = min(max(steps, 50), 256)
         for i in range(nprof):
             plan.solve_profiled(rhos[i % nbuf], vs[i % nbuf])
         ms_sum, cnt = plan.profile_read()
         pass_ms = [m / cnt for m in ms_sum]
 
     batched(max(3, warmup))
-    batch_ms = timed(batched, steps)
+    batch = timed(batched, steps, est)
     mode, tune_ms = plan.launch_mode()
-    res = {"key": key, "ms_per_step": batch_ms, "single_ms_per_step": single_ms, "batch_size": bsz,
+    res = {"key": key, "single": single, "batch": batch, "batch_size": bsz,
            "info": info, "nbuf": nbuf, "rho_bytes": rho_bytes,
            "launch_mode": mode, "tune_ms": tune_ms, "lanes": plan.batch_lanes(bsz),
-           "width": plan.batch_width(bsz),
-           "launches": (5.0 / plan.batch_width(bsz)) if plan.batch_width(bsz) else
-                       (5 if plan.batch_lanes(bsz) > 1 else plan.launches_per_solve())}
+           "width": plan.batch_width(bsz), "launches_per_solve": plan.launches_per_solve()}
     if pass_ms is not None:
         res["pass_ms"] = pass_ms
 
@@ -382,21 +422,23 @@ def run_ours(args):
 
     info = res["info"]
     cfg = inputs[0]
-    ms = res["ms_per_step"]
+    ms = res["single"]["ms"]                          # the north-star call: poisson_solve back to back on one stream
     value = world * 1e3 / ms
+    bms = res["batch"]["ms"]
     n_phys = cfg.n[0] * cfg.n[1] * cfg.n[2]
     n_pad = info.s[0] * info.s[1] * info.s[2]
     flops = nominal_flops(info)
     alu_peak = pk.poisson_measure_fma_peak(pk.FP64 if cfg.precision == "fp64" else pk.FP32)
-    fused = res["launch_mode"] == "fused" and res["lanes"] == 1
+    fused = res["launch_mode"] == "fused"
     dom = int(np.argmax(res["pass_ms"]))
     if fused:   # one kernel does the whole solve: it is the dominant (only) kernel, timed by the solve's own events
         dom_name, dom_kernel, dom_bytes = "solve", "solve_kernel<...> (all five passes in one cooperative launch)", info.bytes_total
-        dom_gbs = info.bytes_total / (ms * 1e-3) / 1e9
+        dom_us = ms * 1e3
     else:
         dom_name, dom_kernel, dom_bytes = pk.PASS_NAMES[dom], f"pass {pk.PASS_NAMES[dom]} (pass_kernel<..., KIND={dom}>)", info.bytes[dom]
-        dom_gbs = info.bytes[dom] / (res["pass_ms"][dom] * 1e-3) / 1e9
-    traffic = None
+        dom_us = res["pass_ms"][dom] * 1e3
+    dom_gbs = dom_bytes / (dom_us * 1e-6) / 1e9
+    traffic, traffic_src = None, None
     tfile = ROOT / "profiles" / "dram_traffic.csv"     # ncu dram__bytes_read.sum + dram__bytes_write.sum per launch
     if tfile.exists():
         try:
@@ -404,56 +446,64 @@ def run_ours(args):
             for row in csv.DictReader(tfile.open()):
                 if row["config"] == args.config and row["pass"] == dom_name:
                     traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+                    traffic_src = f"ncu --set full (L2 flushed before the launch: cold-L2 DRAM bytes), capture {row['source']}"
         except Exception:
             traffic = None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if cfg.precision == "fp64" else "f32", "data": "synthetic",
-        "config": {
-            "workload": WORKLOAD_TEXT[args.config], "physical_grid": list(cfg.n), "padded_grid": list(info.s),
-            "bc_xyz": ["free" if b == 0 else "periodic" for b in cfg.bc], "axis_order": list(info.order),
-            "parallelism": "replicas only" if world > 1 else "1 GPU",
-            "api": (f"poisson_solve_batch, {res['batch_size']} resident densities per call (solves dealt to lanes with their own "
-                    "intermediates and streams; PAPER.md:53,89 repeated-solve usage); single_stream below is poisson_solve one by one"),
-            "l2_policy": (f"rho/V rotated over {res['nbuf']}+{res['nbuf']} device buffers "
-                          f"({2 * res['nbuf'] * res['rho_bytes'] / 1e6:.0f} MB > 126 MB L2); the plan's A1/A2/K^F workspace "
-                          f"({info.workspace_bytes / 1e6:.0f} MB) is reused every step (the paper's repeated-solve usage, "
-                          "PAPER.md:53,89); cold_l2 below flushes L2 with a 512 MB write between solves"),
-        },
+        "config": config_dict(args.config, cfg, info.s, info.order, world),     # identical keys and values in --impl reference
+        "api": "poisson_solve (include/poisson.h), one call per solve, back to back on one stream",
+        "l2_policy": (f"rho/V rotated over {res['nbuf']}+{res['nbuf']} device buffers "
+                      f"({2 * res['nbuf'] * res['rho_bytes'] / 1e6:.0f} MB > 126 MB L2); the plan's A1/A2/K^F workspace "
+                      f"({info.workspace_bytes / 1e6:.0f} MB) is reused every step (the paper's repeated-solve usage, "
+                      "PAPER.md:53,89); cold_l2 below flushes L2 with a 512 MB write between solves"),
+        "timing": {"timed_regions": res["single"]["regions"], "region": f"exactly {steps} solves between two CUDA events on the launching stream",
+                   "statistic": "median region", "ms_per_step_min": res["single"]["min"], "ms_per_step_max": res["single"]["max"]},
         "grid_points_per_sec_physical": value * n_phys, "grid_points_per_sec_padded": value * n_pad,
-        "solve_hbm": {"algorithmic_bytes": info.bytes_total, "achieved_gbs": info.bytes_total / (ms * 1e-3) / 1e9 * 1.0,
-                      "peak_gbs": peak, "peak_source": peak_src, "frac": info.bytes_total / (ms * 1e-3) / 1e9 / peak},
+        "solve_hbm": {"algorithmic_bytes": info.bytes_total, "achieved_gbs": info.bytes_total / (ms * 1e-3) / 1e9,
+                      "peak_gbs": peak, "peak_source": peak_src, "frac": info.bytes_total / (ms * 1e-3) / 1e9 / peak,
+                      "note": "effective bandwidth on ALGORITHMIC bytes (B_5 of SURVEY.md 8d) over the measured HBM copy peak; on grids whose "
+                              "intermediates sit in the 126 MB L2 the DRAM traffic is lower (see roofline.traffic) and the figure can exceed 1"},
         "alu": {"nominal_gflop_per_solve": flops / 1e9, "achieved_nominal_tflops": flops / (ms * 1e-3) / 1e12,
                 "peak_fma_tflops_measured": alu_peak, "frac": flops / (ms * 1e-3) / 1e12 / alu_peak,
                 "note": "nominal 5 n log2 n flops per complex 1D FFT (2.5 real, 2 per K^F multiply) against the plain FMA peak "
                         "measured live by poisson_measure_fma_peak (FMA = 2 flops); the executed instruction count is lower "
                         "(radix-16 butterflies), see profiles/ for sm__inst_executed_pipe_fp64"},
-        "single_stream": {"ms_per_step": res["single_ms_per_step"], "solves_per_sec": 1e3 / res["single_ms_per_step"],
-                          "hbm_frac": info.bytes_total / (res["single_ms_per_step"] * 1e-3) / 1e9 / peak,
-                          "api": "poisson_solve, back to back on one stream"},
+        "batched": {"ms_per_step": bms, "solves_per_sec": world * 1e3 / bms, "hbm_frac": info.bytes_total / (bms * 1e-3) / 1e9 / peak,
+                    "ms_per_step_min": res["batch"]["min"], "ms_per_step_max": res["batch"]["max"],
+                    "api": (f"poisson_solve_batch, {res['batch_size']} resident densities per call, lanes={res['lanes']}, "
+                            f"densities per launch={res['width']} (SURVEY.md 8f-1; pointer arrays marshalled before the timed region)")},
         "pass_us": {pk.PASS_NAMES[q]: res["pass_ms"][q] * 1e3 for q in range(5)},
         "pass_gbs": {pk.PASS_NAMES[q]: info.bytes[q] / (res["pass_ms"][q] * 1e-3) / 1e9 for q in range(5)},
+        "pass_us_note": ("poisson_solve_profiled: the five passes as five STREAM launches with a CUDA event between each (launch gaps "
+                         "included), not the launch mode poisson_solve uses; their sum exceeds ms_per_step"),
         "cold_l2": {"ms_per_step": res["cold_ms_per_step"],
                     "frac": info.bytes_total / (res["cold_ms_per_step"] * 1e-3) / 1e9 / peak},
         "roofline": {"bound": "hbm", "kernel": dom_kernel,
                      "achieved": dom_gbs, "peak": peak, "unit": "GB/s", "frac": dom_gbs / peak, "traffic": traffic,
-                     "algorithmic_bytes_per_launch": dom_bytes, "peak_source": peak_src},
-        "launch_mode": {"chosen": res["launch_mode"], "batch_lanes": res["lanes"], "ms_per_solve_at_plan_creation": res["tune_ms"],
+                     "traffic_source": traffic_src,
+                     "dram_frac": (traffic / (dom_us * 1e-6) / 1e9 / peak) if traffic else None,
+                     "algorithmic_bytes_per_launch": dom_bytes, "peak_source": peak_src,
+                     "duration_us": dom_us, "duration_source": "CUDA events around the kernel's stream launch (pass_us)"},
+        "launch_mode": {"chosen": res["launch_mode"], "ms_per_solve_at_plan_creation": res["tune_ms"],
                         "note": "poisson_plan_create times {five launches, five + programmatic dependent launch, one fused "
-                                "cooperative launch, the five launches as one CUDA graph, that graph with PDL edges} and keeps the fastest; pass_us below are the five passes timed one by one"},
+                                "cooperative launch, the five launches as one CUDA graph, that graph with PDL edges} and keeps the fastest"},
         "e2e": {"value": world * 1e3 / res["e2e_ms_per_step"], "unit": UNIT, "h2d_bytes_per_step": res["rho_bytes"],
                 "d2h_bytes_per_step": res["rho_bytes"], "ms_per_step": res["e2e_ms_per_step"], "steps": res["e2e_steps"],
                 "api": (f"poisson_solve_batch_host, {res['e2e_batch']} pinned host densities per call: every rho copied H2D, five passes, "
                         "every V copied D2H, stream sync, all inside the timed region (wall clock, max over ranks)"),
                 "single_call_ms_per_step": res["e2e_single_ms_per_step"],
                 "single_call_api": "poisson_solve_host (one density per call: H2D + 5 passes + D2H + sync, nothing overlapped)"},
-        "gpu_launches": int(round(res["launches"] * steps)),
+        "gpu_launches": int(res["launches_per_solve"] * steps),
+        "gpu_launches_note": f"{res['launches_per_solve']} kernels per solve x {steps} solves in ONE timed region ({res['single']['regions']} regions were timed)",
         "clocks": clocks,
     }
     if world == 1 and not args.no_cpu_baseline:
-        sec, desc, threads = oracle_sample_seconds(cfg, inputs[1], 12.0)
-        line["cpu_baseline"] = {"value": 1.0 / sec, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc}
+        sec, desc, threads, extrap, frac, ntimed = oracle_steps(cfg, inputs[1], inputs[2], 3, 0, 30.0)
+        line["cpu_baseline"] = {"value": 1.0 / sec, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
+                                "extrapolated": extrap, "sample_fraction": frac}
     if world == 1 and not args.headline_only:
         others = {}
         for key in ("c0", "c2", "c3", "c4a", "c4b", "c4p"):
@@ -461,10 +511,11 @@ def run_ours(args):
                 continue
             r = time_config(pk, torch, key, min(steps, 200), 5, with_e2e=True, with_cold=False)
             i2 = r["info"]
-            others[key] = {"workload": WORKLOAD_TEXT[key], "ms_per_step": r["ms_per_step"],
-                           "solves_per_sec": 1e3 / r["ms_per_step"],
-                           "hbm_frac": i2.bytes_total / (r["ms_per_step"] * 1e-3) / 1e9 / peak,
-                           "single_stream_ms_per_step": r["single_ms_per_step"],
+            others[key] = {"workload": WORKLOAD_TEXT[key], "ms_per_step": r["single"]["ms"],
+                           "solves_per_sec": 1e3 / r["single"]["ms"],
+                           "hbm_frac": i2.bytes_total / (r["single"]["ms"] * 1e-3) / 1e9 / peak,
+                           "batched_ms_per_step": r["batch"]["ms"],
+                           "batched_hbm_frac": i2.bytes_total / (r["batch"]["ms"] * 1e-3) / 1e9 / peak,
                            "e2e_ms_per_step": r["e2e_ms_per_step"], "launch_mode": r["launch_mode"],
                            "pass_us": {pk.PASS_NAMES[q]: r["pass_ms"][q] * 1e3 for q in range(5)}}
         line["other_configs"] = others
@@ -478,7 +529,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--config", default="c1", choices=sorted(WORKLOAD_TEXT))

@@ -116,7 +116,8 @@ POISSON_API int poisson_set_kernel(poisson_plan *plan, const void *K_f_dev, void
  *   rho_dev: device, plan-precision reals [nz][ny][nx], 16-byte aligned, not modified
  *   V_dev  : device, same shape; may equal rho_dev (rho is consumed before V is written)
  * Asynchronous, allocates nothing, never touches host memory.  One plan = one solve in flight
- * (the workspace is shared).  Errors: EINVAL, ENOKERNEL, ECUDA. */
+ * (the workspace is shared).  Errors: EINVAL (also: the current CUDA device is not the one the plan was created on),
+ * ENOKERNEL, ECUDA. */
 POISSON_API int poisson_solve(poisson_plan *plan, const void *rho_dev, void *V_dev, void *stream);
 
 /* End-to-end variant with HOST buffers (the paper's usage: density on the host, potential wanted
@@ -132,8 +133,9 @@ POISSON_API int poisson_solve_host(poisson_plan *plan, const void *rho_host, voi
  * each with its own A1 / A2 intermediates and its own internal stream, so that the tail of one solve overlaps
  * the head of the next (and, in the host variant, H2D of solve i+1 and D2H of solve i-1 overlap the passes of
  * solve i on the two copy engines).  Lanes are allocated on first use and kept by the plan (its
- * workspace_bytes grows accordingly).  Always five launches per solve (the cooperative fused kernel cannot
- * overlap with itself).
+ * workspace_bytes grows accordingly; when device memory does not hold every lane the batch runs on the lanes that
+ * fit).  With more than one lane a solve is always five launches (the cooperative fused kernel cannot overlap with
+ * itself); a one-lane device batch is poisson_solve in a loop, in the plan's own launch mode.
  * Small grids (intermediates of one density <= 16 MB, i.e. up to 64^3 -> 128^3, where one solve has far fewer tiles than the
  * GPU has resident CTAs) take a different route in poisson_solve_batch: up to 32 densities per LAUNCH -- each of the
  * five launches covers the tiles of all of them, density i using slot i of a wide A1 / A2 allocation (<= 96 MB, so it
@@ -144,7 +146,8 @@ POISSON_API int poisson_solve_host(poisson_plan *plan, const void *rho_host, voi
  * poisson_solve_batch is asynchronous: the lanes start after the work already queued on `stream`, and work
  * queued on `stream` afterwards starts after every solve of the batch.  poisson_solve_batch_host returns
  * after the last V has arrived on the host.  A plan runs ONE call at a time.
- * Errors: EINVAL (null / misaligned pointer, count < 0), ENOKERNEL, ENOMEM, ECUDA. */
+ * Errors: EINVAL (null / misaligned pointer, count < 0, current device is not the plan's), ENOKERNEL, ENOMEM, ECUDA.
+ * After an error in the middle of a batch the caller's stream is still ordered after the lane work already queued. */
 POISSON_API int poisson_solve_batch(poisson_plan *plan, const void *const *rho_dev /* host array of device ptrs */,
                         void *const *V_dev /* host array of device ptrs */, int count, void *stream);
 POISSON_API int poisson_solve_batch_host(poisson_plan *plan, const void *const *rho_host /* host array of host ptrs */,

@@ -23,13 +23,20 @@ std::vector<KernelEntry> &kernel_registry() {
     return reg;
 }
 
-// variant < 0: the POISSON_VARIANT environment variable (tuning experiments), else the default 0.
-// A requested variant that was not compiled for this length falls back to variant 0.
+// Experiment knobs that may differ per pass: "n" (all five passes) or "f1,f2,f3,i2,i1".  Read at plan creation only.
+static int env_pass_value(const char *name, int pass, int dflt) {
+    const char *env = std::getenv(name);
+    if (!env || !*env) return dflt;
+    if (!std::strchr(env, ',')) return std::atoi(env);
+    const char *p = env;
+    for (int q = 0; q < pass && p; ++q) { p = std::strchr(p, ','); if (p) ++p; }
+    return (p && *p && *p != ',') ? std::atoi(p) : dflt;
+}
+
+// variant < 0: the POISSON_VARIANT environment variable (tuning experiments; one value or one per pass), else the
+// default 0.  A requested variant that was not compiled for this length falls back to variant 0.
 const KernelEntry *find_kernel(int kind, int S, int pruned, int lanes_p, int prec, int variant) {
-    if (variant < 0) {
-        const char *env = std::getenv("POISSON_VARIANT");
-        variant = env ? std::atoi(env) : 0;
-    }
+    if (variant < 0) variant = env_pass_value("POISSON_VARIANT", kind, 0);
     const KernelEntry *fallback = nullptr;
     for (const KernelEntry &e : kernel_registry())
         if (e.kind == kind && e.S == S && e.pruned == pruned && e.lanes_p == lanes_p && e.prec == prec) {
@@ -133,7 +140,9 @@ struct poisson_plan {
     int resident[5];      // co-resident CTAs of each pass kernel on this device
     int n_tiles[5], tiles_per_g[5];
     size_t pf_min_bytes;  // L2 prefetch (PassParams::prefetch) for arrays at least this large
-    int pf_force;         // POISSON_PREFETCH=0..3 forces the prefetch bits (experiments), -1 = by size
+    int pf_force[5];      // POISSON_PREFETCH=0..3 (one value, or one per pass) forces the prefetch bits (experiments), -1 = by size
+    int env_lanes, env_wide;   // POISSON_LANES / POISSON_WIDE as read at plan creation (-1: not set)
+    bool env_lane_graph;       // POISSON_LANE_GRAPH=0 at plan creation: plain launches on the batch lanes (experiments)
     void *wide_a1, *wide_a2;   // intermediates of wide_w densities (several small solves per launch), allocated on first use
     int wide_w;
     void *a1, *a2, *kint;
@@ -274,7 +283,12 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     // poisson_plan_create MEASURES the candidates once (tune_plan below) unless POISSON_TUNE=0 or the mode is
     // forced with POISSON_PDL=0|1 / POISSON_FUSED=0|1.
     { const char *env = std::getenv("POISSON_PDL"); pl->use_pdl = env && env[0] == '1'; }
-    { const char *env = std::getenv("POISSON_PREFETCH"); pl->pf_force = env ? std::atoi(env) : -1; pl->pf_min_bytes = (size_t)96 << 20; }
+    for (int q = 0; q < 5; ++q) pl->pf_force[q] = env_pass_value("POISSON_PREFETCH", q, -1);
+    // every environment knob is read HERE, once; the solve path never calls getenv
+    { const char *env = std::getenv("POISSON_LANES"); pl->env_lanes = env ? std::atoi(env) : -1; }
+    { const char *env = std::getenv("POISSON_WIDE"); pl->env_wide = env ? std::atoi(env) : -1; }
+    { const char *env = std::getenv("POISSON_LANE_GRAPH"); pl->env_lane_graph = !(env && env[0] == '0'); }
+    pl->pf_min_bytes = (size_t)96 << 20;
 
     for (int q = 0; q < 5; ++q) {
         const PassDesc &ps = d.pass[q];
@@ -291,6 +305,8 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
         const long long resident = (long long)occ * pl->num_sms;
         pl->resident[q] = (int)resident;
         pl->grid[q] = (int)(pl->n_tiles[q] < resident ? pl->n_tiles[q] : resident);  // persistent CTAs
+        { const int force = env_pass_value("POISSON_GRID", q, 0);                     // experiments: CTAs of pass q
+          if (force > 0 && force < pl->grid[q]) pl->grid[q] = force; }
     }
 
     // One-launch fused solve (solve_kernel.cuh) when this combination of axes was compiled and the per-pass
@@ -403,7 +419,7 @@ size_t poisson_plan_workspace_bytes(const poisson_plan *pl) { return pl ? pl->wo
 
 int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? (pl->fused && pl->use_fused ? 1 : 5) : 0; }   // kernels per solve (graph mode: 5 kernel nodes)
 
-int poisson_plan_launch_mode(const poisson_plan *pl, int *mode, double ms_per_solve[3]) {
+int poisson_plan_launch_mode(const poisson_plan *pl, int *mode, double ms_per_solve[5]) {
     if (!pl || !mode || !ms_per_solve) return POISSON_EINVAL;
     *mode = pl->fused && pl->use_fused ? POISSON_LAUNCH_FUSED
           : (pl->use_graph && active_graph(pl) ? (pl->use_pdl ? POISSON_LAUNCH_GRAPH_PDL : POISSON_LAUNCH_GRAPH)
@@ -469,7 +485,7 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
                               : (size_t)pl->d.a2_elems * 2 * r;
         const size_t k_bytes = (size_t)pl->kint_elems * r;
         prm.prefetch = (in_bytes >= pl->pf_min_bytes ? 1 : 0) | (q == POISSON_PASS_F3 && k_bytes >= pl->pf_min_bytes ? 2 : 0);
-        if (pl->pf_force >= 0) prm.prefetch = pl->pf_force;
+        if (pl->pf_force[q] >= 0) prm.prefetch = pl->pf_force[q];
     }
     return prm;
 }
@@ -482,6 +498,9 @@ static int run_fused(poisson_plan *pl, const void *rho, void *V, cudaStream_t st
     sp.n_planes = pl->d.H;
     sp.t2 = pl->tiles_per_g[1]; sp.t3 = pl->tiles_per_g[2];
     sp.skew = pl->fused_skew;
+    // the barrier / per-plane counters start from zero on EVERY launch (an aborted launch, or a launch on another
+    // stream, must not leave the next one spinning on stale counts)
+    PF_CUDA(cudaMemsetAsync(pl->fused_sync, 0, (size_t)(2 + 2 * pl->d.H) * sizeof(unsigned), st));
     void *args[] = {&sp};
     PF_CUDA(cudaLaunchCooperativeKernel(pl->fused->func, dim3(pl->fused_grid), dim3(pl->fused->NT), args,
                                         pl->fused->smem_bytes, st));
@@ -554,7 +573,7 @@ static int build_graph_pdl(poisson_plan *pl, GraphSolve &g, const Lane *ln = nul
         PF_CUDA(cudaGraphKernelNodeGetParams(nodes[i], &kp));
         for (int q = 0; q < 5; ++q) if (kp.func == pl->k[q]->func) { g.node[q] = nodes[i]; ++found; }
     }
-    if (found != 5) return POISSON_ECUDA;
+    if (found != 5) { cudaGraphDestroy(g.graph); g.graph = nullptr; g_last_error = "captured graph does not hold the five pass kernels"; return POISSON_ECUDA; }
     for (int q = 0; q < 5; ++q) g.prm[q] = pass_params(pl, q, nullptr, nullptr, ln);
     PF_CUDA(cudaGraphInstantiate(&g.exec, g.graph, 0));
     g.rho = nullptr; g.V = nullptr;
@@ -577,6 +596,16 @@ static int run_graph(poisson_plan *pl, GraphSolve &g, const void *rho, void *V, 
     }
     g.rho = rho; g.V = V;
     PF_CUDA(cudaGraphLaunch(g.exec, st));
+    return POISSON_OK;
+}
+
+static int check_device(const poisson_plan *pl) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != pl->device) {
+        cudaGetLastError();
+        g_last_error = "the current CUDA device is not the one the plan was created on";
+        return POISSON_EINVAL;
+    }
     return POISSON_OK;
 }
 
@@ -625,10 +654,9 @@ static int run_passes_wide(poisson_plan *pl, const void *const *rho, void *const
 // Densities per launch for device batches: small grids only (one density leaves most of the GPU idle: 32^3 -> 64^3
 // has 64 .. 264 tiles per pass for 592 resident CTAs), as many as keep the wide intermediates within ~96 MB of L2.
 static int wide_width(const poisson_plan *pl, int count) {
-    const char *env = std::getenv("POISSON_WIDE");
     const size_t lane_bytes = (size_t)(pl->d.a1_elems + pl->d.a2_elems) * 2 * pl->elem_real;
     int w = 0;
-    if (env) w = std::atoi(env);
+    if (pl->env_wide >= 0) w = pl->env_wide;
     else if (lane_bytes <= ((size_t)16 << 20)) w = (int)(((size_t)96 << 20) / lane_bytes);   // measured: 64^3 (12.8 MB) gains 18 % over 3 lanes, 96^3 (43 MB) loses
     if (w > PF_MAX_WIDE) w = PF_MAX_WIDE;
     if (w > count) w = count;
@@ -648,13 +676,15 @@ static int tune_plan(poisson_plan *pl) {
     const size_t bytes = (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * pl->elem_real;
     void *rho = nullptr, *V = nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaStream_t ts = nullptr;   // a private non-blocking stream: tuning never synchronises with the caller's streams
     int rc = POISSON_OK;
-    auto cleanup = [&] { cudaFree(rho); cudaFree(V); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); };
+    auto cleanup = [&] { cudaFree(rho); cudaFree(V); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); if (ts) cudaStreamDestroy(ts); };
+    if (cudaStreamCreateWithFlags(&ts, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return POISSON_OK; }
     if (cudaMalloc(&rho, bytes) != cudaSuccess || cudaMalloc(&V, bytes) != cudaSuccess) {   // no room to tune: keep defaults
         cudaGetLastError(); cleanup(); return POISSON_OK;
     }
-    cudaMemset(rho, 0, bytes);
-    cudaMemset(pl->kint, 0, (size_t)pl->kint_elems * pl->elem_real);
+    cudaMemsetAsync(rho, 0, bytes, ts);
+    cudaMemsetAsync(pl->kint, 0, (size_t)pl->kint_elems * pl->elem_real, ts);
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { cudaGetLastError(); cleanup(); return POISSON_OK; }
     const bool modes[5][3] = {{false, false, false}, {true, false, false}, {false, true, false}, {false, false, true}, {true, false, true}};   // {pdl, fused, graph}
     int best = 0; float best_ms = 1e30f;
@@ -666,9 +696,9 @@ static int tune_plan(poisson_plan *pl) {
         pl->use_pdl = modes[m][0]; pl->use_fused = modes[m][1]; pl->use_graph = modes[m][2];
         int reps = 3;
         for (int round = 0; round < 2 && rc == POISSON_OK; ++round) {   // round 0: warm-up + pick the repeat count
-            cudaEventRecord(e0, 0);
-            for (int i = 0; i < reps && rc == POISSON_OK; ++i) rc = run_solve(pl, rho, V, 0);
-            cudaEventRecord(e1, 0);
+            cudaEventRecord(e0, ts);
+            for (int i = 0; i < reps && rc == POISSON_OK; ++i) rc = run_solve(pl, rho, V, ts);
+            cudaEventRecord(e1, ts);
             if (cudaEventSynchronize(e1) != cudaSuccess) { rc = cuda_fail(cudaGetLastError(), "tuning solve"); break; }
             float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
             ms /= (float)reps;
@@ -683,6 +713,7 @@ static int tune_plan(poisson_plan *pl) {
 
 int poisson_solve(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stream) {
     if (!pl || !rho_dev || !V_dev) return POISSON_EINVAL;
+    if (check_device(pl) != POISSON_OK) return POISSON_EINVAL;
     if (reinterpret_cast<size_t>(rho_dev) % 16 || reinterpret_cast<size_t>(V_dev) % 16) return POISSON_EINVAL;
     if (!pl->kernel_set) return POISSON_ENOKERNEL;
     return run_solve(pl, rho_dev, V_dev, reinterpret_cast<cudaStream_t>(stream));
@@ -690,6 +721,7 @@ int poisson_solve(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stre
 
 int poisson_solve_profiled(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stream) {
     if (!pl || !rho_dev || !V_dev) return POISSON_EINVAL;
+    if (check_device(pl) != POISSON_OK) return POISSON_EINVAL;
     if (reinterpret_cast<size_t>(rho_dev) % 16 || reinterpret_cast<size_t>(V_dev) % 16) return POISSON_EINVAL;
     if (!pl->kernel_set) return POISSON_ENOKERNEL;
     constexpr int kMaxProfiled = 512;
@@ -772,10 +804,14 @@ static int ensure_lanes(poisson_plan *pl, int want, bool staging) {
     if (staging)
         for (int l = 0; l < want; ++l) {
             Lane &ln = (*pl->lanes)[l];
-            if (ln.rho_stage) continue;
-            cudaError_t ce = cudaMalloc(&ln.rho_stage, bytes);
+            if (ln.rho_stage && ln.v_stage) continue;
+            cudaError_t ce = ln.rho_stage ? cudaSuccess : cudaMalloc(&ln.rho_stage, bytes);
             if (ce == cudaSuccess) ce = cudaMalloc(&ln.v_stage, bytes);
-            if (ce != cudaSuccess) { cudaGetLastError(); return ce == cudaErrorMemoryAllocation ? POISSON_ENOMEM : cuda_fail(ce, "batch staging allocation"); }
+            if (ce != cudaSuccess) {   // never leave a lane with one staging buffer
+                cudaFree(ln.rho_stage); ln.rho_stage = nullptr; ln.v_stage = nullptr;
+                cudaGetLastError();
+                return ce == cudaErrorMemoryAllocation ? POISSON_ENOMEM : cuda_fail(ce, "batch staging allocation");
+            }
         }
     return POISSON_OK;
 }
@@ -784,12 +820,11 @@ static int ensure_lanes(poisson_plan *pl, int want, bool staging) {
 // batches use 3 while one lane's intermediates are small enough for several lanes to share the 126 MB L2
 // (measured on B200: 128^3 -> 256^3 gains 9 %, 256^3 -> 512^3 with 808 MB per lane loses 4 %), else 1.
 static int batch_lanes(const poisson_plan *pl, int count, bool host) {
-    const char *env = std::getenv("POISSON_LANES");
     const size_t lane_bytes = (size_t)(pl->d.a1_elems + pl->d.a2_elems) * 2 * pl->elem_real;
     // device batches: 2 lanes (with the per-lane solve graphs 128^3 -> 256^3 measures 96.5 / 93.1 / 96.2 / 97.8 us per solve at
     // 1 / 2 / 3 / 4 lanes, the wire grid 51.9 / 55.3 / 58.6 at 2 / 3 / 4: two sets of intermediates still share the L2)
     // (the surface grid, 34 MB per lane, still gains from a third lane: 27.7 vs 30.3 us -- three sets fit the L2)
-    int lanes = env ? std::atoi(env) : (host ? 3 : (3 * lane_bytes <= ((size_t)110 << 20) ? 3 : (lane_bytes <= ((size_t)256 << 20) ? 2 : 1)));
+    int lanes = pl->env_lanes >= 0 ? pl->env_lanes : (host ? 3 : (3 * lane_bytes <= ((size_t)110 << 20) ? 3 : (lane_bytes <= ((size_t)256 << 20) ? 2 : 1)));
     if (lanes < 1) lanes = 1;
     if (lanes > 8) lanes = 8;
     return count < lanes ? count : lanes;
@@ -803,6 +838,7 @@ static int solve_batch_impl(poisson_plan *pl, const void *const *rho, void *cons
         if (!host && (reinterpret_cast<size_t>(rho[i]) % 16 || reinterpret_cast<size_t>(V[i]) % 16)) return POISSON_EINVAL;
     }
     if (!pl->kernel_set) return POISSON_ENOKERNEL;
+    if (check_device(pl) != POISSON_OK) return POISSON_EINVAL;
     if (!host) {
         const int W = wide_width(pl, count);
         if (W) {
@@ -832,42 +868,49 @@ static int solve_batch_impl(poisson_plan *pl, const void *const *rho, void *cons
         }
         return POISSON_OK;
     }
-    int rc = ensure_lanes(pl, L, host);
+    int L_use = L;
+    int rc = ensure_lanes(pl, L_use, host);
+    while (rc == POISSON_ENOMEM && L_use > 1) rc = ensure_lanes(pl, --L_use, host);   // no room for every lane: use the ones that fit
     if (rc != POISSON_OK) return rc;
     const size_t bytes = (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * pl->elem_real;
     PF_CUDA(cudaEventRecord(pl->fork_ev, user));                      // the lanes start after the caller's earlier work
-    for (int l = 0; l < L; ++l) PF_CUDA(cudaStreamWaitEvent((*pl->lanes)[l].st, pl->fork_ev, 0));
-    const char *e_lg = std::getenv("POISSON_LANE_GRAPH");   // =0: plain launches on the lanes (experiments)
-    const bool lane_graphs = pl->use_graph && active_graph(pl) && !(e_lg && e_lg[0] == '0');
-    for (int i = 0; i < count; ++i) {
-        Lane &ln = (*pl->lanes)[i % L];
+    for (int l = 0; l < L_use; ++l) PF_CUDA(cudaStreamWaitEvent((*pl->lanes)[l].st, pl->fork_ev, 0));
+    const bool lane_graphs = pl->use_graph && active_graph(pl) && pl->env_lane_graph;
+    // one solve on its lane; any failure falls through to the join below so that the caller's stream stays ordered
+    // after the lane work already queued
+    auto queue_one = [&](int i) -> int {
+        Lane &ln = (*pl->lanes)[i % L_use];
         const void *r = rho[i];
         void *v = V[i];
         if (host) {
             PF_CUDA(cudaMemcpyAsync(ln.rho_stage, rho[i], bytes, cudaMemcpyHostToDevice, ln.st));
             r = ln.rho_stage; v = ln.v_stage;
         }
+        int rc1;
         if (lane_graphs) {
             if (!ln.gs) {
                 ln.gs = new (std::nothrow) GraphSolve();
                 if (!ln.gs) return POISSON_ENOMEM;
                 std::memset(ln.gs, 0, sizeof(GraphSolve));
-                rc = pl->use_pdl ? build_graph_pdl(pl, *ln.gs, &ln) : build_graph(pl, *ln.gs, &ln);
-                if (rc != POISSON_OK) return rc;
+                rc1 = pl->use_pdl ? build_graph_pdl(pl, *ln.gs, &ln) : build_graph(pl, *ln.gs, &ln);
+                if (rc1 != POISSON_OK) return rc1;
             }
-            rc = run_graph(pl, *ln.gs, r, v, ln.st);
+            rc1 = run_graph(pl, *ln.gs, r, v, ln.st);
         } else {
-            rc = run_passes(pl, r, v, ln.st, 0, 4, nullptr, &ln);
+            rc1 = run_passes(pl, r, v, ln.st, 0, 4, nullptr, &ln);
         }
-        if (rc != POISSON_OK) return rc;
+        if (rc1 != POISSON_OK) return rc1;
         if (host) PF_CUDA(cudaMemcpyAsync(V[i], ln.v_stage, bytes, cudaMemcpyDeviceToHost, ln.st));
+        return POISSON_OK;
+    };
+    for (int i = 0; i < count && rc == POISSON_OK; ++i) rc = queue_one(i);
+    for (int l = 0; l < L_use; ++l) {                                  // join: the caller's stream continues after every lane
+        cudaError_t ce = cudaEventRecord((*pl->lanes)[l].done, (*pl->lanes)[l].st);
+        if (ce == cudaSuccess) ce = cudaStreamWaitEvent(user, (*pl->lanes)[l].done, 0);
+        if (ce != cudaSuccess && rc == POISSON_OK) rc = cuda_fail(ce, "batch join");
     }
-    for (int l = 0; l < L; ++l) {                                      // join: the caller's stream continues after every lane
-        PF_CUDA(cudaEventRecord((*pl->lanes)[l].done, (*pl->lanes)[l].st));
-        PF_CUDA(cudaStreamWaitEvent(user, (*pl->lanes)[l].done, 0));
-    }
-    if (host) PF_CUDA(cudaStreamSynchronize(user));
-    return POISSON_OK;
+    if (host) { const cudaError_t ce = cudaStreamSynchronize(user); if (ce != cudaSuccess && rc == POISSON_OK) rc = cuda_fail(ce, "batch sync"); }
+    return rc;
 }
 
 int poisson_plan_batch_lanes(const poisson_plan *pl, int count, int host) {
@@ -888,6 +931,7 @@ int poisson_solve_batch_host(poisson_plan *pl, const void *const *rho_host, void
 
 int poisson_solve_host(poisson_plan *pl, const void *rho_host, void *V_host, void *stream) {
     if (!pl || !rho_host || !V_host) return POISSON_EINVAL;
+    if (check_device(pl) != POISSON_OK) return POISSON_EINVAL;
     if (!pl->kernel_set) return POISSON_ENOKERNEL;
     const size_t bytes = (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * pl->elem_real;
     if (!pl->rho_stage) {

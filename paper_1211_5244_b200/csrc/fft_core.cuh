@@ -4,8 +4,6 @@
 // compactification without ever touching the zero half:
 //   * dft_pruned_in  : DFT of a length-R sequence whose upper half is zero   (spread,  PAPER.md:53)
 //   * dft_pruned_out : DFT of a length-R sequence keeping only outputs n<R/2 (compactification)
-// Everything is __host__ __device__ so the index algebra can be exercised on a CPU during
-// development; the product only ever runs the __global__ kernels built from it.
 #pragma once
 
 #include <cstddef>
@@ -13,13 +11,8 @@
 
 #include "twiddle_consts.cuh"
 
-#if defined(__CUDACC__)
-#define PF_HD __host__ __device__ __forceinline__
-#define PF_CE __host__ __device__ constexpr
-#else
-#define PF_HD inline __attribute__((always_inline))
-#define PF_CE constexpr
-#endif
+#define PF_HD __device__ __forceinline__          // device code only: there is no host path
+#define PF_CE __host__ __device__ constexpr       // compile-time helpers (twiddle literals, geometry)
 
 namespace pfft {
 
@@ -49,79 +42,39 @@ template <typename T> PF_HD cx<T> mul_pi(cx<T> a) { return mk<T>(-a.im, a.re); }
 // loaded / stored with the evict-first policy (ld.global.cs / st.global.cs) so that it does not
 // push the intermediates A1 / A2, which ARE reused by the next pass, out of the 126 MB L2.
 PF_HD cx<double> ld_stream(const cx<double> *p) {
-#if defined(__CUDA_ARCH__)
     const double2 v = __ldcs(reinterpret_cast<const double2 *>(p));
     return mk<double>(v.x, v.y);
-#else
-    return *p;
-#endif
 }
 PF_HD cx<float> ld_stream(const cx<float> *p) {
-#if defined(__CUDA_ARCH__)
     const float2 v = __ldcs(reinterpret_cast<const float2 *>(p));
     return mk<float>(v.x, v.y);
-#else
-    return *p;
-#endif
 }
 PF_HD double ld_stream(const double *p) {
-#if defined(__CUDA_ARCH__)
     return __ldcs(p);
-#else
-    return *p;
-#endif
 }
 PF_HD float ld_stream(const float *p) {
-#if defined(__CUDA_ARCH__)
     return __ldcs(p);
-#else
-    return *p;
-#endif
 }
 PF_HD void st_stream(cx<double> *p, cx<double> v) {
-#if defined(__CUDA_ARCH__)
     __stcs(reinterpret_cast<double2 *>(p), make_double2(v.re, v.im));
-#else
-    *p = v;
-#endif
 }
 PF_HD void st_stream(cx<float> *p, cx<float> v) {
-#if defined(__CUDA_ARCH__)
     __stcs(reinterpret_cast<float2 *>(p), make_float2(v.re, v.im));
-#else
-    *p = v;
-#endif
 }
 // Two complex values adjacent in memory as ONE access: 256-bit LDG/STG in fp64 (new on sm_100), 128-bit in fp32.
 // p must be aligned to the size of the pair.
 PF_HD void st_pair(cx<double> *p, cx<double> a, cx<double> b) {
-#if defined(__CUDA_ARCH__)
     asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(a.re), "d"(a.im), "d"(b.re), "d"(b.im) : "memory");
-#else
-    p[0] = a; p[1] = b;
-#endif
 }
 PF_HD void st_pair(cx<float> *p, cx<float> a, cx<float> b) {
-#if defined(__CUDA_ARCH__)
     *reinterpret_cast<float4 *>(p) = make_float4(a.re, a.im, b.re, b.im);
-#else
-    p[0] = a; p[1] = b;
-#endif
 }
 PF_HD void ld_pair_stream(const cx<double> *p, cx<double> &a, cx<double> &b) {
-#if defined(__CUDA_ARCH__)
     asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a.re), "=d"(a.im), "=d"(b.re), "=d"(b.im) : "l"(p));
-#else
-    a = p[0]; b = p[1];
-#endif
 }
 PF_HD void ld_pair_stream(const cx<float> *p, cx<float> &a, cx<float> &b) {
-#if defined(__CUDA_ARCH__)
     const float4 v = __ldcs(reinterpret_cast<const float4 *>(p));
     a = mk<float>(v.x, v.y); b = mk<float>(v.z, v.w);
-#else
-    a = p[0]; b = p[1];
-#endif
 }
 template <bool STREAM, typename E> PF_HD E ld_hint(const E *p) {
     if constexpr (STREAM) return ld_stream(p); else return *p;

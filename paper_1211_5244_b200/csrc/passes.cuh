@@ -28,14 +28,8 @@
 
 namespace pfft {
 
-#if defined(__CUDA_ARCH__)
 PF_HD void cta_sync() { __syncthreads(); }
 PF_HD void warp_sync() { __syncwarp(); }
-#else
-void host_cta_sync();  // provided by the development-only host harness
-PF_HD void cta_sync() { host_cta_sync(); }
-PF_HD void warp_sync() { host_cta_sync(); }
-#endif
 
 enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4 };
 
@@ -43,7 +37,8 @@ enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4 
 // NBUF_   : exchange buffers (2 = one barrier per exchange, 1 = half the shared memory, one more barrier)
 // TWS_    : twiddles w_S^{n1 k2} read from a shared-memory table (true) or held in registers (false)
 // MINB_   : __launch_bounds__ minimum resident CTAs per SM (register cap); 0 = automatic
-// STG_    : asynchronous staging (cp.async, no register cost): 0 = none, tiles are loaded straight into
+// STG_    : 3 = register double buffer (the next tile is loaded into a second register set while the current one is
+//           transformed; no shared memory).  Else asynchronous staging (cp.async, no register cost): 0 = none, tiles are loaded straight into
 //           registers; 1 = the NEXT tile's inputs land in a shared-memory stage while the current tile is
 //           transformed; 2 = as 1, and pass F3 also stages its K^F values.  Where that stage does not fit next to
 //           the exchange buffer (the inverse passes I2 / I1 read S resp. S/2+1 rows), the EXCHANGE BUFFER ITSELF is
@@ -85,8 +80,8 @@ struct Geo {
     static constexpr int TW_ELEMS = TW_TABLES * S;
     static constexpr size_t SMEM_BYTES = ((size_t)NBUF * XELEMS + TW_ELEMS) * sizeof(cx<T_>);
     // a one-pass kernel only keeps the table(s) its direction reads: F1/F2 [k2][n1], I2/I1 [n1][k2], F3 both
-    static constexpr int tw_elems(int kind) { return (kind == KIND_F3 ? TW_TABLES : (TW_TABLES > 0 ? 1 : 0)) * S; }
-    static constexpr size_t smem_bytes(int kind) { return ((size_t)NBUF * XELEMS + tw_elems(kind)) * sizeof(cx<T_>); }
+    static PF_CE int tw_elems(int kind) { return (kind == KIND_F3 ? TW_TABLES : (TW_TABLES > 0 ? 1 : 0)) * S; }
+    static PF_CE size_t smem_bytes(int kind) { return ((size_t)NBUF * XELEMS + tw_elems(kind)) * sizeof(cx<T_>); }
 
     static PF_HD void split(int tid, int &t, int &p) {
         if (LANES_P) { p = tid % P; t = tid / P; } else { t = tid % TPP; p = tid / TPP; }
@@ -131,14 +126,10 @@ template <typename T> PF_HD cx<T> *pass_out(const PassParams &prm, int bi) {
 // the previous pass drains, run their prologue (twiddle tables: constant data), and only then wait
 // for the previous pass's memory to be complete and visible.
 PF_HD void pdl_launch_dependents() {
-#if defined(__CUDA_ARCH__)
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-#endif
 }
 PF_HD void pdl_wait_prior_grid() {
-#if defined(__CUDA_ARCH__)
     asm volatile("griddepcontrol.wait;" ::: "memory");
-#endif
 }
 
 // ------------------------------------------------------------------ inter-pass twiddles w_S^{n1 k2}
@@ -347,51 +338,31 @@ PF_HD void store_B(const cx<typename G::T> *v, cx<typename G::T> *dst, long long
 // have the whole transform + store of that tile to land, at no register cost.
 
 PF_HD unsigned long long evict_first_policy() {
-#if defined(__CUDA_ARCH__)
     unsigned long long pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
-#else
-    return 0ull;
-#endif
 }
 // one complex element, global -> shared (16 B: L2 only; 8 B: the only size cp.async.cg does not offer)
 template <bool STREAM> PF_HD void cp_async_elem(cx<double> *sdst, const cx<double> *gsrc, unsigned long long pol) {
-#if defined(__CUDA_ARCH__)
     const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
     if constexpr (STREAM) asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
     else asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
-#else
-    *sdst = *gsrc;
-#endif
 }
 template <bool STREAM> PF_HD void cp_async_elem(cx<float> *sdst, const cx<float> *gsrc, unsigned long long pol) {
-#if defined(__CUDA_ARCH__)
     const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
     if constexpr (STREAM) asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
     else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
-#else
-    *sdst = *gsrc;
-#endif
 }
 // 16 raw bytes (K^F vectors), evict-first
 PF_HD void cp_async_vec16(void *sdst, const void *gsrc, unsigned long long pol) {
-#if defined(__CUDA_ARCH__)
     const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
     asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
-#else
-    for (int b = 0; b < 16; ++b) static_cast<char *>(sdst)[b] = static_cast<const char *>(gsrc)[b];
-#endif
 }
 PF_HD void cp_async_commit() {
-#if defined(__CUDA_ARCH__)
     asm volatile("cp.async.commit_group;" ::: "memory");
-#endif
 }
 template <int N> PF_HD void cp_async_wait() {   // at most N of this thread's newest groups still pending
-#if defined(__CUDA_ARCH__)
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
-#endif
 }
 
 // K^F values travel in 16-byte vectors: KVEC consecutive registers r of one thread
@@ -401,16 +372,10 @@ template <> struct KVec<float>  { static constexpr int N = 4; using V = float4; 
 PF_HD void kvec_get(const double2 &v, double *o) { o[0] = v.x; o[1] = v.y; }
 PF_HD void kvec_get(const float4 &v, float *o) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
 PF_HD void prefetch_l2(const void *p) {
-#if defined(__CUDA_ARCH__)
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-#endif
 }
 template <typename VT> PF_HD VT ld_stream_vec(const VT *p) {
-#if defined(__CUDA_ARCH__)
     return __ldcs(p);
-#else
-    return *p;
-#endif
 }
 
 // Shape of the stage of pass KIND: NR points along the transform x W complex columns.
@@ -422,14 +387,14 @@ struct Stage {
     // staging is dropped where it would not leave room for G::MINB resident CTAs (228 KB per SM, 1 KB
     // reserved per CTA): the occupancy the register budget was chosen for wins
     static constexpr size_t SM_SMEM = 233472, CTA_RESERVED = 1024;
-    static constexpr bool fits(size_t stage_bytes) { return (G::smem_bytes(KIND) + stage_bytes + CTA_RESERVED) * G::MINB <= SM_SMEM; }
-    static constexpr bool ON = G::STG > 0 && fits((size_t)NR * W * sizeof(cx<T>));
-    static constexpr bool KON = ON && G::STG > 1 && KIND == KIND_F3 && fits(((size_t)NR * W + G::V * G::NT / 2) * sizeof(cx<T>));
+    static PF_CE bool fits(size_t stage_bytes) { return (G::smem_bytes(KIND) + stage_bytes + CTA_RESERVED) * G::MINB <= SM_SMEM; }
+    static constexpr bool ON = (G::STG == 1 || G::STG == 2) && fits((size_t)NR * W * sizeof(cx<T>));
+    static constexpr bool KON = ON && G::STG == 2 && KIND == KIND_F3 && fits(((size_t)NR * W + G::V * G::NT / 2) * sizeof(cx<T>));
     // exchange buffer as the stage (inverse passes, one exchange buffer)
     // (measured at S = 512 fp64: I2 176 -> 160 us; I1 gets SLOWER this way, 108 -> 118 us -- its 256-bit loads straight
     // into registers beat a trip through shared memory -- so XSTG_I1 stays off)
     static constexpr bool XSTG_I1 = false;
-    static constexpr bool XON = G::STG > 0 && !ON && G::NBUF == 1 && G::RB > 1 && (KIND == KIND_I2 || (XSTG_I1 && KIND == KIND_I1 && G::LANES_P));
+    static constexpr bool XON = (G::STG == 1 || G::STG == 2) && !ON && G::NBUF == 1 && G::RB > 1 && (KIND == KIND_I2 || (XSTG_I1 && KIND == KIND_I1 && G::LANES_P));
     static constexpr int IN_ELEMS = ON ? NR * W : 0;
     static constexpr int K_ELEMS = KON ? G::V * G::NT / 2 : 0;   // V*NT reals
     static constexpr size_t BYTES = (size_t)(IN_ELEMS + K_ELEMS) * sizeof(cx<T>);
@@ -518,6 +483,17 @@ PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_
             if (tile + nb < n_tiles) issue(tile + nb);
             cp_async_commit();
             process(cur, tile);
+        }
+    } else if constexpr (G::STG == 3) {   // register double buffer: the next tile's loads are in flight while this one is transformed
+        int tile = bid;
+        Buf cur;
+        if (tile < n_tiles) fetch(cur, tile);
+        for (; tile < n_tiles; tile += nb) {
+            Buf nxt;
+            const bool more = tile + nb < n_tiles;
+            if (more) fetch(nxt, tile + nb);
+            process(cur, tile);
+            if (more) cur = nxt;
         }
     } else {
         for (int tile = bid; tile < n_tiles; tile += nb) {

@@ -25,13 +25,12 @@ namespace pfft {
 
 struct SolveParams {
     PassParams pass[5];
-    unsigned *sync;   // [0] grid-barrier arrivals, [1] exits, [2 + g] F2 tiles done of plane g, [2 + G + g] F3 tiles done
+    unsigned *sync;   // [0] grid-barrier arrivals, [1] unused, [2 + g] F2 tiles done of plane g, [2 + G + g] F3 tiles done; zero at launch
     int n_planes;     // G = H = S_a/2 + 1
     int t2, t3;       // tiles per plane of F2 / I2 and of F3
     int skew;         // D
 };
 
-#if defined(__CUDA_ARCH__)
 __device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned *p) {
     unsigned v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -45,7 +44,10 @@ __device__ __forceinline__ void cta_signal(unsigned *ctr) {
 // all threads of the CTA: block until *ctr >= target, then see everything signalled before
 __device__ __forceinline__ void cta_wait(const unsigned *ctr, unsigned target) {
     if (threadIdx.x == 0) {
-        while (ld_acquire_gpu(ctr) < target) __nanosleep(40);
+        // bounded: with all CTAs co-resident and the counters zeroed before the launch the wait is short; if it is not
+        // (a bug), fail the launch with a trap -- the host then sees POISSON_ECUDA -- instead of hanging the device
+        unsigned spins = 0;
+        while (ld_acquire_gpu(ctr) < target) { __nanosleep(40); if (++spins > (1u << 26)) __trap(); }
         __threadfence();
     }
     __syncthreads();
@@ -54,7 +56,6 @@ __device__ __forceinline__ void grid_barrier(unsigned *ctr, unsigned target) {
     cta_signal(ctr);
     cta_wait(ctr, target);
 }
-#endif
 
 template <class GA, class GB, class GC>
 struct SolveSmem {
@@ -74,7 +75,6 @@ struct SolveSmem {
 
 template <class GA, bool PA, class GB, bool PB, class GC, bool PC>
 __global__ void __launch_bounds__(GA::NT, GA::MINB) solve_kernel(const SolveParams prm) {
-#if defined(__CUDA_ARCH__)
     static_assert(GA::NT == GB::NT && GA::NT == GC::NT, "the three geometries share one CTA shape");
     static_assert((GA::TWS || GA::RB == 1) && (GB::TWS || GB::RB == 1) && (GC::TWS || GC::RB == 1), "twiddles live in shared memory");
     static_assert(GA::STG == 0 && GB::STG == 0 && GC::STG == 0, "tiles go straight to registers here");
@@ -157,16 +157,7 @@ __global__ void __launch_bounds__(GA::NT, GA::MINB) solve_kernel(const SolvePara
         }
     }
 
-    // ---------------- the last CTA out re-arms the counters for the next solve
-    __shared__ unsigned last;
-    __syncthreads();
-    if (tid == 0) last = atomicAdd(prm.sync + 1, 1u) == (unsigned)nb - 1u;
-    __syncthreads();
-    if (last) {
-        for (int i = tid; i < 2 + 2 * prm.n_planes; i += GA::NT) prm.sync[i] = 0u;
-        __threadfence();
-    }
-#endif
+    // the counters are zeroed by a cudaMemsetAsync queued before every launch (api.cu: run_fused)
 }
 
 }  // namespace pfft

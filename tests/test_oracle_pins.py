@@ -276,6 +276,55 @@ def test_stages_and_axis_order_independence():
     assert rel_l2(st1[2], st0[2]) < 1e-13
 
 
+def _full_spectrum(Kf_half, s):
+    """Full [Sz][Sy][Sx] spectrum from the half the data contract holds: K_f(-k) = K_f(k) (index reflection only)."""
+    sx, sy, sz = s
+    full = np.empty((sz, sy, sx))
+    full[:, :, : sx // 2 + 1] = Kf_half
+    kx = np.arange(sx // 2 + 1, sx)
+    full[:, :, sx // 2 + 1:] = Kf_half[(-np.arange(sz)) % sz][:, (-np.arange(sy)) % sy][:, :, sx - kx]
+    return full
+
+
+@pytest.mark.parametrize("bc,order", [((FREE, PER, FREE), (1, 2, 0)), ((FREE, FREE, FREE), (2, 1, 0)), ((PER, PER, FREE), (1, 0, 2)),
+                                      ((FREE, FREE, PER), (2, 1, 0))])
+def test_every_stage_of_oracle_solve_against_library_fft_per_axis(bc, order):
+    """All six intermediates oracle.solve exposes (the per-pass parity references of the GPU tests), each against
+    numpy's FFT applied one axis at a time in the same order: after each forward sweep (0, 1, 2), after the K_f
+    multiply (3), after the first and second inverse sweep (4, 5).  Array axis of grid axis q is 2 - q.
+    A kernel that is inversion symmetric but not even per axis makes stage 3 sensitive to the half-spectrum reflection."""
+    n = (6, 4, 10)
+    rng = _rng(260 + sum(order) + 7 * sum(bc))
+    s = gen.padded_shape(n, bc)
+    Kf = oracle.kernel_spectrum(_inversion_kernel(rng, s))
+    rho = rng.standard_normal((n[2], n[1], n[0]))
+    V, st = oracle.solve(rho, Kf, bc, axis_order=order, return_stages=True)
+    a = _pad(rho, s).astype(complex)
+    for i in range(3):
+        a = np.fft.fft(a, axis=2 - order[i])
+        assert rel_l2(st[i], a) < 1e-13, ("forward", i)
+    a = a * _full_spectrum(Kf, s)
+    assert rel_l2(st[3], a) < 1e-13
+    for j, i in enumerate((2, 1)):                                   # inverse sweeps run in reverse order: c, then b
+        a = np.fft.ifft(a, axis=2 - order[i]) * s[order[i]]          # unnormalised inverse
+        assert rel_l2(st[4 + j], a) < 1e-13, ("inverse", j)
+    a = np.fft.ifft(a, axis=2 - order[0]) * s[order[0]]
+    assert rel_l2(V, a.real[: n[2], : n[1], : n[0]] / (s[0] * s[1] * s[2])) < 1e-13
+
+
+@pytest.mark.parametrize("bc", ALL_BC)
+def test_solve_equals_direct_sum_16_cubed(bc):
+    """north_star: the oracle against the O(N^2) sum of Eq. 2 by brute force "on grids up to 16^3" -- the 16^3 case,
+    all 8 BC combinations (padded up to 32^3; 16.8 M kernel-density products per BC)."""
+    n = (16, 16, 16)
+    rng = _rng(1600 + sum(b << i for i, b in enumerate(bc)))
+    s = gen.padded_shape(n, bc)
+    rho = rng.standard_normal((n[2], n[1], n[0]))
+    K = _even_kernel(rng, s)
+    Kf = oracle.kernel_spectrum(K)
+    assert rel_l2(oracle.solve(rho, Kf, bc), oracle.direct_sum(rho, K, bc)) < 1e-13
+
+
 # ----------------------------------------------------------------------------- the workloads themselves
 def test_workload_generators_are_seeded_and_shaped():
     cfg = gen.get_config("c0")

@@ -41,9 +41,11 @@ def _load():
         lib.oracle_dft_axis.argtypes = [p, _LL3, ctypes.c_int, ctypes.c_int, ctypes.c_int]
         lib.oracle_kernel_spectrum.argtypes = [p, _LL3, p, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
         lib.oracle_solve.argtypes = [p, p, p, _LL3, _I3, p, p, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
+        lib.oracle_kernel_spectrum_c.argtypes = [p, _LL3, p, ctypes.c_int]
+        lib.oracle_solve_c.argtypes = [p, p, p, _LL3, _I3, p, p, ctypes.POINTER(ctypes.c_double), ctypes.c_int]
         lib.oracle_direct_sum_at.argtypes = [p, p, _LL3, _I3, p, ctypes.c_longlong, p]
         lib.oracle_direct_sum.argtypes = [p, p, _LL3, _I3, p]
-        for f in (lib.oracle_dft_axis, lib.oracle_kernel_spectrum, lib.oracle_solve,
+        for f in (lib.oracle_dft_axis, lib.oracle_kernel_spectrum, lib.oracle_solve, lib.oracle_kernel_spectrum_c, lib.oracle_solve_c,
                   lib.oracle_direct_sum_at, lib.oracle_direct_sum):
             f.restype = ctypes.c_int
         _lib = lib
@@ -106,6 +108,31 @@ def solve(rho: np.ndarray, Kf_half: np.ndarray, bc, axis_order=(0, 1, 2), return
     if return_max_imag:
         res.append(mi.value)
     return res[0] if len(res) == 1 else tuple(res)
+
+
+def kernel_spectrum_complex(K: np.ndarray, accum_ld: bool = False) -> np.ndarray:
+    """K real [Sz][Sy][Sx] with NO symmetry -> complex K_f [Sz][Sy][Sx/2+1] (numpy rfftn shape) by the naive DFT."""
+    K = np.ascontiguousarray(K, dtype=np.float64)
+    sz, sy, sx = K.shape
+    full = np.empty(K.shape, dtype=np.complex128)
+    _check(_load().oracle_kernel_spectrum_c(_ptr(K), _LL3(sx, sy, sz), _ptr(full), int(accum_ld)), "kernel_spectrum_c")
+    return np.ascontiguousarray(full[:, :, : sx // 2 + 1])
+
+
+def solve_complex(rho: np.ndarray, Kf_half: np.ndarray, bc, axis_order=(0, 1, 2), accum_ld: bool = False,
+                  return_max_imag: bool = False):
+    """Eq. 3 with a complex half spectrum (real kernel without inversion symmetry; K_f(-k) = conj K_f(k))."""
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    Kf_half = np.ascontiguousarray(Kf_half, dtype=np.complex128)
+    nz, ny, nx = rho.shape
+    s = [nx * (2 if bc[0] == 0 else 1), ny * (2 if bc[1] == 0 else 1), nz * (2 if bc[2] == 0 else 1)]
+    assert Kf_half.shape == (s[2], s[1], s[0] // 2 + 1), (Kf_half.shape, s)
+    V = np.empty_like(rho)
+    mi = ctypes.c_double(0.0)
+    _check(_load().oracle_solve_c(_ptr(rho), _ptr(Kf_half), _ptr(V), _LL3(nx, ny, nz), _I3(*[int(b) for b in bc]),
+                                  _ptr(np.asarray(axis_order, dtype=np.int32)), None, ctypes.byref(mi), int(accum_ld)),
+           "solve_c")
+    return (V, mi.value) if return_max_imag else V
 
 
 def direct_sum(rho: np.ndarray, K: np.ndarray, bc) -> np.ndarray:

@@ -14,6 +14,9 @@
  *   - oracle_dft_axis:      the discrete Fourier transform by its definition,
  *                           X[k] = sum_j x[j] exp(-/+ 2 pi i j k / S), one axis at a time, O(S^2) per line.
  *   - oracle_kernel_spectrum: K_f = DFT3(K) by three oracle_dft_axis sweeps (K^F of Eq. 3).
+ *   - oracle_kernel_spectrum_c / oracle_solve_c: the same two routines for a real kernel K WITHOUT the symmetry
+ *                           K(-r) = K(r): Eq. 2 and Eq. 3 hold for any K; the spectrum is then complex
+ *                           with K_f(-k) = conj K_f(k) (complex K_f; outlook PAPER.md:93).
  *   - oracle_solve:         Eq. 3 on the EXPLICITLY zero-padded grid:
  *                           pad -> DFT along each axis -> multiply by K_f -> inverse DFT along each
  *                           axis -> divide by S_x S_y S_z -> copy the physical box out.
@@ -25,7 +28,8 @@
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): brute-force direct sum for all 8 BC
  * combinations, Parseval, delta -> kernel, identity kernel, shift kernel (zero fill vs wrap),
  * linearity, fully periodic plane-wave closed form, mirror symmetry, and numpy's pocketfft as a
- * test-only second opinion.  The paper prints no worked numerical example, so no value fixture
+ * test-only second opinion; the complex-spectrum routines against the same brute-force sum with kernels
+ * that have no symmetry at all, all 8 BC combinations.  The paper prints no worked numerical example, so no value fixture
  * exists; the closed-form 1D-FFT-count ratios 7/12 and 2/3 are in tests/golden/.
  *
  * Arithmetic: fp64 data; twiddle table w[m] = exp(-2 pi i m / S) evaluated in long double and
@@ -154,6 +158,18 @@ int oracle_kernel_spectrum(const double *K, const long long S[3] /* Sx,Sy,Sz */,
     return st;
 }
 
+/* ---- K_f = DFT3(K) for a real K with no symmetry: the full complex spectrum [Sz][Sy][Sx]. ---- */
+int oracle_kernel_spectrum_c(const double *K, const long long S[3] /* Sx,Sy,Sz */, cplx *Kf_full, int accum_ld)
+{
+    if (!K || !S || !Kf_full) return ORACLE_EINVAL;
+    const long long dims[3] = {S[2], S[1], S[0]};
+    const long long tot = dims[0] * dims[1] * dims[2];
+    for (long long i = 0; i < tot; ++i) Kf_full[i] = K[i];
+    int st = ORACLE_OK;
+    for (int ax = 2; ax >= 0 && st == ORACLE_OK; --ax) st = oracle_dft_axis(Kf_full, dims, ax, -1, accum_ld);
+    return st;
+}
+
 static long long wrap(long long i, long long S) { return ((i % S) + S) % S; }
 
 /* ---- Eq. 3 on the explicitly padded grid.
@@ -168,11 +184,11 @@ static long long wrap(long long i, long long S) { return ((i % S) + S) % S; }
  *  stages   : optional, 6 * Sz*Sy*Sx complex: the padded array after each forward sweep (0,1,2),
  *             after the K_f multiply (3), after the first and second inverse sweeps (4,5).
  *  max_abs_imag_V: largest |Im| of the unnormalised result inside the box (should be rounding). */
-int oracle_solve(const double *rho, const double *Kf_half, double *V, const long long n[3],
-                 const int bc[3], const int axis_order[3], cplx *stages, double *max_abs_imag_V,
-                 int accum_ld)
+static int solve_core(const double *rho, const double *Kf_half, const cplx *Kf_half_c, double *V, const long long n[3],
+                      const int bc[3], const int axis_order[3], cplx *stages, double *max_abs_imag_V,
+                      int accum_ld)
 {
-    if (!rho || !Kf_half || !V || !n || !bc) return ORACLE_EINVAL;
+    if (!rho || (!Kf_half && !Kf_half_c) || !V || !n || !bc) return ORACLE_EINVAL;
     long long S[3];
     for (int a = 0; a < 3; ++a) {
         if (n[a] <= 0 || (bc[a] != 0 && bc[a] != 1)) return ORACLE_EINVAL;
@@ -203,10 +219,17 @@ int oracle_solve(const double *rho, const double *Kf_half, double *V, const long
     for (long long kz = 0; kz < S[2]; ++kz)
         for (long long ky = 0; ky < S[1]; ++ky)
             for (long long kx = 0; kx < S[0]; ++kx) {
-                double kf;
-                if (kx < H) kf = Kf_half[(kz * S[1] + ky) * H + kx];
-                else        kf = Kf_half[(wrap(-kz, S[2]) * S[1] + wrap(-ky, S[1])) * H + (S[0] - kx)];
-                a[(kz * S[1] + ky) * S[0] + kx] *= kf;
+                if (Kf_half) {          /* real spectrum: K(-r) = K(r), the other half is K_f(-k) = K_f(k) */
+                    double kf;
+                    if (kx < H) kf = Kf_half[(kz * S[1] + ky) * H + kx];
+                    else        kf = Kf_half[(wrap(-kz, S[2]) * S[1] + wrap(-ky, S[1])) * H + (S[0] - kx)];
+                    a[(kz * S[1] + ky) * S[0] + kx] *= kf;
+                } else {                /* complex spectrum of a real K: the other half is K_f(-k) = conj K_f(k) */
+                    cplx kf;
+                    if (kx < H) kf = Kf_half_c[(kz * S[1] + ky) * H + kx];
+                    else        kf = conj(Kf_half_c[(wrap(-kz, S[2]) * S[1] + wrap(-ky, S[1])) * H + (S[0] - kx)]);
+                    a[(kz * S[1] + ky) * S[0] + kx] *= kf;
+                }
             }
     if (stages) memcpy(stages + (size_t)3 * tot, a, sizeof(cplx) * (size_t)tot);
 
@@ -230,6 +253,23 @@ int oracle_solve(const double *rho, const double *Kf_half, double *V, const long
     if (max_abs_imag_V) *max_abs_imag_V = mi;
     free(a);
     return ORACLE_OK;
+}
+
+int oracle_solve(const double *rho, const double *Kf_half, double *V, const long long n[3],
+                 const int bc[3], const int axis_order[3], cplx *stages, double *max_abs_imag_V,
+                 int accum_ld)
+{
+    if (!Kf_half) return ORACLE_EINVAL;
+    return solve_core(rho, Kf_half, NULL, V, n, bc, axis_order, stages, max_abs_imag_V, accum_ld);
+}
+
+/* Eq. 3 with the COMPLEX half spectrum [Sz][Sy][Sx/2+1] of a real kernel without inversion symmetry. */
+int oracle_solve_c(const double *rho, const cplx *Kf_half_c, double *V, const long long n[3],
+                   const int bc[3], const int axis_order[3], cplx *stages, double *max_abs_imag_V,
+                   int accum_ld)
+{
+    if (!Kf_half_c) return ORACLE_EINVAL;
+    return solve_core(rho, NULL, Kf_half_c, V, n, bc, axis_order, stages, max_abs_imag_V, accum_ld);
 }
 
 /* ---- Eq. 2 brute force at a list of output points (flat indices into [nz][ny][nx]).

@@ -325,6 +325,36 @@ def test_solve_equals_direct_sum_16_cubed(bc):
     assert rel_l2(oracle.solve(rho, Kf, bc), oracle.direct_sum(rho, K, bc)) < 1e-13
 
 
+@pytest.mark.parametrize("bc", ALL_BC)
+@pytest.mark.parametrize("n", [(6, 4, 8), (5, 3, 7)])
+def test_complex_spectrum_solve_equals_direct_sum_all_bc(bc, n):
+    """Eq. 2 holds for ANY real kernel: a random K with no symmetry has a complex spectrum with
+    K_f(-k) = conj K_f(k); oracle.solve_complex against the O(N^2) sum, even and odd sizes, all 8 BC combinations."""
+    rng = _rng(300 + sum(b << i for i, b in enumerate(bc)) + n[0])
+    s = gen.padded_shape(n, bc)
+    rho = rng.standard_normal((n[2], n[1], n[0]))
+    K = rng.standard_normal((s[2], s[1], s[0]))
+    Kf = oracle.kernel_spectrum_complex(K)
+    assert rel_l2(Kf, np.fft.rfftn(K)) < 1e-13                        # library second opinion on the spectrum itself
+    V, vimag = oracle.solve_complex(rho, Kf, bc, return_max_imag=True)
+    assert vimag < 1e-13 * np.abs(V).max()
+    assert rel_l2(V, oracle.direct_sum(rho, K, bc)) < 1e-13
+    # a symmetric kernel through the complex route reproduces the real route
+    Ke = _even_kernel(rng, s)
+    assert rel_l2(oracle.solve_complex(rho, oracle.kernel_spectrum_complex(Ke), bc), oracle.solve(rho, oracle.kernel_spectrum(Ke), bc)) < 1e-13
+
+
+@pytest.mark.parametrize("bc", ALL_BC)
+def test_solve_equals_direct_sum_odd_and_prime_sizes(bc):
+    """Odd N on every axis (S = N on periodic axes is then odd: the half spectrum has S/2+1 = (S+1)/2 entries)."""
+    n = (7, 5, 3)
+    rng = _rng(700 + sum(b << i for i, b in enumerate(bc)))
+    s = gen.padded_shape(n, bc)
+    rho = rng.standard_normal((n[2], n[1], n[0]))
+    K = _even_kernel(rng, s)
+    assert rel_l2(oracle.solve(rho, oracle.kernel_spectrum(K), bc), oracle.direct_sum(rho, K, bc)) < 1e-13
+
+
 # ----------------------------------------------------------------------------- the workloads themselves
 def test_workload_generators_are_seeded_and_shaped():
     cfg = gen.get_config("c0")

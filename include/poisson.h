@@ -50,7 +50,7 @@ enum { POISSON_FP64 = 0, POISSON_FP32 = 1 };
 enum {
     POISSON_OK = 0,
     POISSON_EINVAL = 1,       /* null pointer, n <= 0, bc / precision out of range, bad h, misaligned pointer */
-    POISSON_EUNSUPPORTED = 2, /* odd N_i, or a padded length S_i with no compiled transform            */
+    POISSON_EUNSUPPORTED = 2, /* a padded length S_i above the any-length kernel's limit (4096)        */
     POISSON_ENOMEM = 3,       /* host or device allocation failed                                        */
     POISSON_ENOKERNEL = 4,    /* poisson_solve before poisson_set_kernel                                 */
     POISSON_ECUDA = 5,        /* a CUDA call failed (sticky; text via poisson_last_error)                */
@@ -92,9 +92,13 @@ POISSON_API int poisson_plan_describe(int nx, int ny, int nz, const int bc[3] /*
 /* Creates a plan on the current CUDA device: validates, picks the axis order, allocates the
  * workspace (A1, A2, internal K^F) and uploads the twiddle tables.  `h` (grid spacing) is recorded
  * metadata only.  *out is set to NULL on failure.  Problem statement: PAPER.md:51.
- * Supported grids: every N_i even, every padded length S_i = N_i * B_i one of
+ * Supported grids: every N_i >= 1 with padded length S_i = N_i * B_i <= 4096, odd N included ("various grid sizes",
+ * PAPER.md:89).  A pass whose length is one of
  *   4 8 12 16 20 24 32 36 40 48 60 64 72 80 96 100 120 128 144 160 192 200 240 256 288 320 384 400 480 512 576 640 768 1024
- * (csrc/sizes.def), else POISSON_EUNSUPPORTED.  Errors: EINVAL, EUNSUPPORTED, ENOMEM, ECUDA, EARCH. */
+ * (csrc/sizes.def) runs the compiled register-engine kernel for that length; every other length (odd, factors 7, 11, ...,
+ * three or more radices, primes), and the R2C / C2R pass of a grid with odd N_x, runs the any-length shared-memory
+ * Stockham kernel (csrc/generic_pass.cuh) -- correct for every length, slower.  Only S_i > 4096 is refused with
+ * POISSON_EUNSUPPORTED.  Errors: EINVAL, EUNSUPPORTED, ENOMEM, ECUDA, EARCH. */
 POISSON_API int poisson_plan_create(poisson_plan **out /* host, out */, int nx, int ny, int nz,
                         const int bc[3] /* host; x,y,z */, double h, int precision);
 
@@ -111,6 +115,17 @@ POISSON_API int poisson_plan_get_info(const poisson_plan *plan, poisson_plan_inf
  * ("a transposition of the associated kernel ... carried out only once").
  * Asynchronous on `stream`; K_f_dev may be freed once that work has completed. */
 POISSON_API int poisson_set_kernel(poisson_plan *plan, const void *K_f_dev, void *stream);
+
+/* The same for a real kernel K WITHOUT inversion symmetry (K(-r) != K(r): the general convolution of Eq. 2,
+ * PAPER.md:37; screened / anisotropic kernels and the plane-wave local-potential convolution of PAPER.md:93), whose
+ * spectrum is complex with K^F(-k) = conj K^F(k).
+ *   K_f_dev: device, plan-precision COMPLEX values (interleaved re, im), C order [S_z][S_y][S_x/2+1] = numpy
+ *            rfftn(K) of the real kernel on the padded grid (unnormalised forward DFT); 16-byte aligned.
+ * The complex multiply runs in the any-length F3 kernel: the first call switches pass F3 of this plan to it (device
+ * synchronisation, the internal K^F copy is re-allocated for complex values, the fused one-launch mode is dropped).
+ * poisson_set_kernel may be called again later to go back to a real spectrum.
+ * Errors: EINVAL, ENOMEM, EUNSUPPORTED, ECUDA. */
+POISSON_API int poisson_set_kernel_complex(poisson_plan *plan, const void *K_f_dev, void *stream);
 
 /* One solve (the 13 steps of PAPER.md:57-71 as 5 fused launches, or one, on `stream`; see poisson_plan_launch_mode).
  *   rho_dev: device, plan-precision reals [nz][ny][nx], 16-byte aligned, not modified

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "../../include/poisson.h"
+#include "generic_pass.cuh"
 #include "passes.cuh"
 #include "planner.hpp"
 #include "registry.hpp"
@@ -53,6 +54,47 @@ static int preferred_variant(int kind, int S, int prec) {
     { const char *f = std::getenv("POISSON_FUSED"); if (f && f[0] == '1') return -1; }   // the fused kernel is compiled for the default factorizations
     if (S == 192 && prec == POISSON_FP64 && (kind == KIND_F2 || kind == KIND_I2)) return 9;
     return -1;
+}
+
+// ---- any-length kernel (generic_pass.cuh): a per-plan KernelEntry with run-time geometry
+template <typename T>
+static const void *generic_func(int kind) {
+    switch (kind) {
+        case KIND_F1: return reinterpret_cast<const void *>(&generic_pass_kernel<T, KIND_F1>);
+        case KIND_F2: return reinterpret_cast<const void *>(&generic_pass_kernel<T, KIND_F2>);
+        case KIND_F3: return reinterpret_cast<const void *>(&generic_pass_kernel<T, KIND_F3>);
+        case KIND_I2: return reinterpret_cast<const void *>(&generic_pass_kernel<T, KIND_I2>);
+        default: return reinterpret_cast<const void *>(&generic_pass_kernel<T, KIND_I1>);
+    }
+}
+
+// Radices of S for the Stockham passes: 4s first (fewest passes over the tile), then the prime factors ascending.
+static int generic_factors(int S, int fac[16]) {
+    int n = 0;
+    while (S % 4 == 0 && n < 16) { fac[n++] = 4; S /= 4; }
+    for (int p = 2; S > 1 && n < 16; ++p)
+        while (S % p == 0 && n < 16) { fac[n++] = p; S /= p; }
+    return S == 1 ? n : -1;
+}
+
+// false: the length does not fit the any-length kernel (shared memory, or more than 16 radices)
+static bool make_generic_entry(KernelEntry &e, int kind, int S, int pruned, int lanes_p, int prec) {
+    e = KernelEntry{};
+    e.kind = kind; e.S = S; e.pruned = pruned; e.lanes_p = lanes_p; e.prec = prec; e.generic = 1;
+    e.nbuf = 2; e.NT = GEN_NT; e.TPP = 0; e.V = 0; e.RA = S; e.RB = 1;
+    e.gen_nfac = generic_factors(S, e.gen_fac);
+    if (e.gen_nfac < 0 || S > GEN_MAX_S) return false;
+    const size_t cplx = prec == POISSON_FP64 ? 16 : 8;
+    // widest tile (whole 128-byte rows first) that fits the 227 KB of shared memory a CTA may use
+    int P = (int)(128 / cplx);
+    while (P > 1 && gen_smem_bytes(S, P, cplx) > (size_t)227 * 1024) P /= 2;
+    if (gen_smem_bytes(S, P, cplx) > (size_t)227 * 1024) return false;
+    // small transforms: enough pencils per tile to give every thread work (S * P >= 2 * NT), still whole rows
+    while (S * P < 2 * GEN_NT && P < 64 && gen_smem_bytes(S, 2 * P, cplx) <= (size_t)48 * 1024) P *= 2;
+    e.P = P;
+    e.smem_bytes = gen_smem_bytes(S, P, cplx);
+    e.func = prec == POISSON_FP64 ? generic_func<double>(kind) : generic_func<float>(kind);
+    return true;
 }
 
 std::vector<FusedEntry> &fused_registry() {
@@ -136,6 +178,8 @@ struct poisson_plan {
     int device;
     int num_sms;
     const KernelEntry *k[5];
+    KernelEntry gen_entry[5];  // the passes that run the any-length kernel point here
+    bool kcplx;                // the installed K^F is complex (poisson_set_kernel_complex)
     int grid[5];
     int resident[5];      // co-resident CTAs of each pass kernel on this device
     int n_tiles[5], tiles_per_g[5];
@@ -209,11 +253,59 @@ static void free_plan(poisson_plan *pl) {
     delete pl;
 }
 
+static int check_device(const poisson_plan *pl) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != pl->device) {
+        cudaGetLastError();
+        g_last_error = "the current CUDA device is not the one the plan was created on";
+        return POISSON_EINVAL;
+    }
+    return POISSON_OK;
+}
+
 static GraphSolve *active_graph(poisson_plan *pl) {
     GraphSolve *g = pl->use_pdl ? &pl->gs_pdl : &pl->gs;
     return g->exec ? g : nullptr;
 }
 static const GraphSolve *active_graph(const poisson_plan *pl) { return active_graph(const_cast<poisson_plan *>(pl)); }
+
+// Reals in the internal K^F copy: the register-engine F3 streams [tile][V][NT] (padded to whole tiles), the any-length
+// kernel reads the natural order of the pass (one real, or one complex number, per spectrum point).
+static long long kint_reals(const poisson_plan *pl) {
+    const KernelEntry *e = pl->k[2];
+    if (e->generic) return (long long)pl->d.pass[2].n_g * pl->d.pass[2].S * pl->d.pass[2].n_p * (pl->kcplx ? 2 : 1);
+    return (long long)pl->n_tiles[2] * e->V * e->NT;
+}
+
+// Picks the kernel of pass q (the compiled register-engine kernel for its length, else -- or when force_generic -- the
+// any-length kernel) and derives tiles, occupancy and the persistent grid from it.
+static int setup_pass(poisson_plan *pl, int q, bool force_generic) {
+    const PassDesc &ps = pl->d.pass[q];
+    const int precision = pl->d.prec;
+    const KernelEntry *e = nullptr;
+    if (!ps.generic && !force_generic)
+        e = find_kernel(ps.kind, ps.S, ps.pruned, ps.lanes_p, precision, preferred_variant(ps.kind, ps.S, precision));
+    if (!e) {
+        // F1 / I1 address rho / V in pairs (register engine) or in reals (any-length kernel): the planner fixed which
+        if (!ps.generic && (q == POISSON_PASS_F1 || q == POISSON_PASS_I1)) return POISSON_EUNSUPPORTED;
+        if (!make_generic_entry(pl->gen_entry[q], ps.kind, ps.S, ps.pruned, ps.lanes_p, precision)) return POISSON_EUNSUPPORTED;
+        e = &pl->gen_entry[q];
+    }
+    pl->k[q] = e;
+    pl->tiles_per_g[q] = (int)((ps.n_p + e->P - 1) / e->P);
+    pl->n_tiles[q] = (int)(ps.n_g * pl->tiles_per_g[q]);
+    cudaError_t ce = cudaFuncSetAttribute(e->func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e->smem_bytes);
+    if (ce != cudaSuccess) return cuda_fail(ce, "cudaFuncSetAttribute(smem)");
+    int occ = 0;
+    ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, e->func, e->NT, e->smem_bytes);
+    if (ce != cudaSuccess || occ < 1) return cuda_fail(ce, "occupancy query");
+    const long long resident = (long long)occ * pl->num_sms;
+    pl->resident[q] = (int)resident;
+    pl->grid[q] = (int)(pl->n_tiles[q] < resident ? pl->n_tiles[q] : resident);  // persistent CTAs
+    { const int force = env_pass_value("POISSON_GRID", q, 0);                     // experiments: CTAs of pass q
+      if (force > 0 && force < pl->grid[q]) pl->grid[q] = force; }
+    return POISSON_OK;
+}
 
 extern "C" {
 
@@ -223,7 +315,7 @@ const char *poisson_status_string(int st) {
     switch (st) {
         case POISSON_OK: return "ok";
         case POISSON_EINVAL: return "invalid argument";
-        case POISSON_EUNSUPPORTED: return "unsupported grid size (odd N, or no compiled transform for a padded length)";
+        case POISSON_EUNSUPPORTED: return "unsupported grid size (a padded length above the any-length kernel's limit of 4096)";
         case POISSON_ENOMEM: return "out of memory";
         case POISSON_ENOKERNEL: return "poisson_solve called before poisson_set_kernel";
         case POISSON_ECUDA: return "CUDA error (see poisson_last_error)";
@@ -241,9 +333,13 @@ int poisson_plan_describe(int nx, int ny, int nz, const int bc[3], int precision
     PlanDesc d;
     const int st = plan_build(nx, ny, nz, bc, precision, d);
     if (st != POISSON_OK) return st;
-    for (int q = 0; q < 5; ++q)
-        if (!find_kernel(d.pass[q].kind, d.pass[q].S, d.pass[q].pruned, d.pass[q].lanes_p, precision))
-            return POISSON_EUNSUPPORTED;
+    for (int q = 0; q < 5; ++q) {
+        const PassDesc &ps = d.pass[q];
+        KernelEntry tmp;
+        if (!ps.generic && find_kernel(ps.kind, ps.S, ps.pruned, ps.lanes_p, precision)) continue;
+        if (!ps.generic && (q == POISSON_PASS_F1 || q == POISSON_PASS_I1)) return POISSON_EUNSUPPORTED;
+        if (!make_generic_entry(tmp, ps.kind, ps.S, ps.pruned, ps.lanes_p, precision)) return POISSON_EUNSUPPORTED;
+    }
     *info = d.info;
     return POISSON_OK;
 }
@@ -291,22 +387,8 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     pl->pf_min_bytes = (size_t)96 << 20;
 
     for (int q = 0; q < 5; ++q) {
-        const PassDesc &ps = d.pass[q];
-        const KernelEntry *e = find_kernel(ps.kind, ps.S, ps.pruned, ps.lanes_p, precision, preferred_variant(ps.kind, ps.S, precision));
-        if (!e) { free_plan(pl); return POISSON_EUNSUPPORTED; }
-        pl->k[q] = e;
-        pl->tiles_per_g[q] = (int)((ps.n_p + e->P - 1) / e->P);
-        pl->n_tiles[q] = (int)(ps.n_g * pl->tiles_per_g[q]);
-        cudaError_t ce = cudaFuncSetAttribute(e->func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e->smem_bytes);
-        if (ce != cudaSuccess) { free_plan(pl); return cuda_fail(ce, "cudaFuncSetAttribute(smem)"); }
-        int occ = 0;
-        ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, e->func, e->NT, e->smem_bytes);
-        if (ce != cudaSuccess || occ < 1) { free_plan(pl); return cuda_fail(ce, "occupancy query"); }
-        const long long resident = (long long)occ * pl->num_sms;
-        pl->resident[q] = (int)resident;
-        pl->grid[q] = (int)(pl->n_tiles[q] < resident ? pl->n_tiles[q] : resident);  // persistent CTAs
-        { const int force = env_pass_value("POISSON_GRID", q, 0);                     // experiments: CTAs of pass q
-          if (force > 0 && force < pl->grid[q]) pl->grid[q] = force; }
+        st = setup_pass(pl, q, false);
+        if (st != POISSON_OK) { free_plan(pl); return st; }
     }
 
     // One-launch fused solve (solve_kernel.cuh) when this combination of axes was compiled and the per-pass
@@ -321,7 +403,9 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
         const FusedEntry *fe = want ? find_fused(precision, S3, pr3, lp3) : nullptr;
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-        if (fe && coop && fe->P[0] == pl->k[0]->P && fe->P[1] == pl->k[1]->P && fe->P[2] == pl->k[2]->P &&
+        bool any_generic = false;
+        for (int q = 0; q < 5; ++q) any_generic = any_generic || pl->k[q]->generic;
+        if (fe && coop && !any_generic && fe->P[0] == pl->k[0]->P && fe->P[1] == pl->k[1]->P && fe->P[2] == pl->k[2]->P &&
             d.pass[1].n_g == d.H && d.pass[2].n_g == d.H) {
             cudaError_t ce = cudaFuncSetAttribute(fe->func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fe->smem_bytes);
             int occ = 0;
@@ -347,7 +431,7 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     }
 
     const size_t cplx = 2 * pl->elem_real;
-    pl->kint_elems = (long long)pl->n_tiles[2] * pl->k[2]->V * pl->k[2]->NT;
+    pl->kint_elems = kint_reals(pl);
     size_t ws = 0;
     cudaError_t ce = cudaMalloc(&pl->a1, (size_t)d.a1_elems * cplx); ws += (size_t)d.a1_elems * cplx;
     if (ce == cudaSuccess) { ce = cudaMalloc(&pl->a2, (size_t)d.a2_elems * cplx); ws += (size_t)d.a2_elems * cplx; }
@@ -434,27 +518,98 @@ int poisson_plan_destroy(poisson_plan *pl) {
     return POISSON_OK;
 }
 
+static void destroy_graph(GraphSolve &g) {
+    if (g.exec) cudaGraphExecDestroy(g.exec);
+    if (g.graph) cudaGraphDestroy(g.graph);
+    std::memset(&g, 0, sizeof(g));
+}
+
+static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln);
+static int build_graph_pdl(poisson_plan *pl, GraphSolve &g, const Lane *ln);
+
+// Re-lays the caller's K^F into the order pass F3 consumes it, for either F3 kernel.
+static int relayout_kernel_spectrum(poisson_plan *pl, const void *K_f_dev, bool cplx, cudaStream_t st) {
+    const PlanDesc &d = pl->d;
+    const KernelEntry *e = pl->k[2];
+    const double scale = 1.0 / ((double)d.s[0] * (double)d.s[1] * (double)d.s[2]);  // reading 2: one 1/(SxSySz)
+    const int threads = 256;
+    if (e->generic) {
+        GenericRelayoutParams q;
+        q.S = d.pass[2].S; q.n_p = (int)d.pass[2].n_p; q.lanes_p = d.pass[2].lanes_p; q.cplx = cplx ? 1 : 0;
+        q.a_axis = d.order[0]; q.c_axis = d.order[2];
+        q.sx = d.s[0]; q.sy = d.s[1]; q.sz = d.s[2];
+        q.total = (long long)d.pass[2].n_g * q.S * q.n_p;
+        q.scale = scale;
+        long long blocks = (q.total + threads - 1) / threads;
+        if (blocks > 148LL * 32) blocks = 148LL * 32;
+        if (d.prec == POISSON_FP64)
+            generic_relayout_kernel<double><<<(int)blocks, threads, 0, st>>>(static_cast<const double *>(K_f_dev), static_cast<double *>(pl->kint), q);
+        else
+            generic_relayout_kernel<float><<<(int)blocks, threads, 0, st>>>(static_cast<const float *>(K_f_dev), static_cast<float *>(pl->kint), q);
+    } else {
+        RelayoutParams q;
+        q.RA = e->RA; q.RB = e->RB; q.TPP = e->TPP; q.P = e->P; q.V = e->V; q.NT = e->NT; q.lanes_p = e->lanes_p;
+        q.tiles_per_g = pl->tiles_per_g[2]; q.n_p = (int)d.pass[2].n_p;
+        q.a_axis = d.order[0]; q.c_axis = d.order[2];
+        q.sx = d.s[0]; q.sy = d.s[1]; q.sz = d.s[2];
+        q.total = pl->kint_elems;
+        q.scale = scale;
+        long long blocks = (q.total + threads - 1) / threads;
+        if (blocks > 148LL * 32) blocks = 148LL * 32;
+        if (d.prec == POISSON_FP64)
+            relayout_kernel<double><<<(int)blocks, threads, 0, st>>>(static_cast<const double *>(K_f_dev), static_cast<double *>(pl->kint), q);
+        else
+            relayout_kernel<float><<<(int)blocks, threads, 0, st>>>(static_cast<const float *>(K_f_dev), static_cast<float *>(pl->kint), q);
+    }
+    PF_CUDA(cudaGetLastError());
+    return POISSON_OK;
+}
+
 int poisson_set_kernel(poisson_plan *pl, const void *K_f_dev, void *stream) {
     if (!pl || !K_f_dev) return POISSON_EINVAL;
     if (reinterpret_cast<size_t>(K_f_dev) % 16) return POISSON_EINVAL;
-    const PlanDesc &d = pl->d;
-    const KernelEntry *e = pl->k[2];
-    RelayoutParams q;
-    q.RA = e->RA; q.RB = e->RB; q.TPP = e->TPP; q.P = e->P; q.V = e->V; q.NT = e->NT; q.lanes_p = e->lanes_p;
-    q.tiles_per_g = pl->tiles_per_g[2]; q.n_p = (int)d.pass[2].n_p;
-    q.a_axis = d.order[0]; q.c_axis = d.order[2];
-    q.sx = d.s[0]; q.sy = d.s[1]; q.sz = d.s[2];
-    q.total = pl->kint_elems;
-    q.scale = 1.0 / ((double)d.s[0] * (double)d.s[1] * (double)d.s[2]);  // reading 2: one 1/(SxSySz)
+    if (check_device(pl) != POISSON_OK) return POISSON_EINVAL;
+    if (pl->kcplx) {   // back from a complex kernel: the any-length F3 kernel stays, its K^F copy holds reals again
+        pl->kcplx = false;
+        destroy_graph(pl->gs); destroy_graph(pl->gs_pdl);
+        if (pl->lanes) for (Lane &ln : *pl->lanes) if (ln.gs) destroy_graph(*ln.gs);
+        if (pl->use_graph) { if ((pl->use_pdl ? build_graph_pdl(pl, pl->gs_pdl, nullptr) : build_graph(pl, pl->gs, nullptr)) != POISSON_OK) cudaGetLastError(); }
+    }
+    const int rc = relayout_kernel_spectrum(pl, K_f_dev, false, reinterpret_cast<cudaStream_t>(stream));
+    if (rc != POISSON_OK) return rc;
+    pl->kernel_set = true;
+    return POISSON_OK;
+}
+
+int poisson_set_kernel_complex(poisson_plan *pl, const void *K_f_dev, void *stream) {
+    if (!pl || !K_f_dev) return POISSON_EINVAL;
+    if (reinterpret_cast<size_t>(K_f_dev) % 16) return POISSON_EINVAL;
+    if (check_device(pl) != POISSON_OK) return POISSON_EINVAL;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-    const int threads = 256;
-    long long blocks = (q.total + threads - 1) / threads;
-    if (blocks > 148LL * 32) blocks = 148LL * 32;
-    if (d.prec == POISSON_FP64)
-        relayout_kernel<double><<<(int)blocks, threads, 0, st>>>(static_cast<const double *>(K_f_dev), static_cast<double *>(pl->kint), q);
-    else
-        relayout_kernel<float><<<(int)blocks, threads, 0, st>>>(static_cast<const float *>(K_f_dev), static_cast<float *>(pl->kint), q);
-    PF_CUDA(cudaGetLastError());
+    if (!pl->kcplx) {
+        // The complex multiply lives in the any-length F3 kernel: switch pass F3 to it (once), drop what was built
+        // around the old kernel (graphs, the fused one-launch kernel), and size the internal K^F copy for complex values.
+        PF_CUDA(cudaDeviceSynchronize());   // no solve of this plan may still be using the buffers replaced below
+        destroy_graph(pl->gs); destroy_graph(pl->gs_pdl);
+        if (pl->lanes) for (Lane &ln : *pl->lanes) if (ln.gs) destroy_graph(*ln.gs);
+        pl->fused = nullptr; pl->use_fused = false;
+        if (!pl->k[2]->generic) { const int rc = setup_pass(pl, 2, true); if (rc != POISSON_OK) return rc; }
+        pl->kcplx = true;
+        const long long need = kint_reals(pl);
+        if (need > pl->kint_elems) {
+            void *fresh = nullptr;
+            cudaError_t ce = cudaMalloc(&fresh, (size_t)need * pl->elem_real);
+            if (ce != cudaSuccess) { cudaGetLastError(); pl->kcplx = false; return ce == cudaErrorMemoryAllocation ? POISSON_ENOMEM : cuda_fail(ce, "complex K^F allocation"); }
+            cudaFree(pl->kint);
+            pl->kint = fresh;
+            pl->workspace_bytes += (size_t)(need - pl->kint_elems) * pl->elem_real;
+            pl->kint_elems = need;
+        }
+        pl->kernel_set = false;
+        if (pl->use_graph) { if ((pl->use_pdl ? build_graph_pdl(pl, pl->gs_pdl, nullptr) : build_graph(pl, pl->gs, nullptr)) != POISSON_OK) cudaGetLastError(); }
+    }
+    const int rc = relayout_kernel_spectrum(pl, K_f_dev, true, st);
+    if (rc != POISSON_OK) return rc;
     pl->kernel_set = true;
     return POISSON_OK;
 }
@@ -476,6 +631,12 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
     prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;
     prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q];
     prm.n_tiles1 = pl->n_tiles[q];   // one density per launch
+    if (pl->k[q]->generic) {
+        const KernelEntry *e = pl->k[q];
+        prm.gen_S = e->S; prm.gen_P = e->P; prm.gen_nfac = e->gen_nfac; prm.gen_pruned = e->pruned;
+        prm.gen_nreal = ps.n_real; prm.gen_kcplx = pl->kcplx ? 1 : 0; prm.gen_lanes_p = ps.lanes_p;
+        for (int i = 0; i < e->gen_nfac; ++i) prm.gen_fac[i] = e->gen_fac[i];
+    }
     // L2 prefetch of the next tile only where the pass's input cannot be sitting in L2 already (measured: a few
     // per cent faster on the 512^3 grids, slightly slower on 256^3 where A1 / A2 are L2 hits anyway)
     {
@@ -528,7 +689,7 @@ static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t s
 }
 
 // Builds the graph of one solve on the plan's own intermediates (explicit kernel nodes, plain dependencies).
-static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln = nullptr) {
+static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
     if (g.exec) return POISSON_OK;
     PF_CUDA(cudaGraphCreate(&g.graph, 0));
     for (int q = 0; q < 5; ++q) {
@@ -549,7 +710,7 @@ static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln = nullptr
 
 // The same graph with programmatic-dependent-launch edges: captured from the five PDL stream launches (capture turns
 // the launch attribute into programmatic edges), kernel nodes identified by their function.
-static int build_graph_pdl(poisson_plan *pl, GraphSolve &g, const Lane *ln = nullptr) {
+static int build_graph_pdl(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
     if (g.exec) return POISSON_OK;
     cudaStream_t cs = nullptr;
     PF_CUDA(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
@@ -596,16 +757,6 @@ static int run_graph(poisson_plan *pl, GraphSolve &g, const void *rho, void *V, 
     }
     g.rho = rho; g.V = V;
     PF_CUDA(cudaGraphLaunch(g.exec, st));
-    return POISSON_OK;
-}
-
-static int check_device(const poisson_plan *pl) {
-    int dev = -1;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev != pl->device) {
-        cudaGetLastError();
-        g_last_error = "the current CUDA device is not the one the plan was created on";
-        return POISSON_EINVAL;
-    }
     return POISSON_OK;
 }
 
@@ -669,7 +820,7 @@ static int tune_plan(poisson_plan *pl) {
     const char *e_graph = std::getenv("POISSON_GRAPH");
     if (e_graph && e_graph[0] == '1') {                                                    // forced
         const bool pdl = e_pdl && e_pdl[0] == '1';
-        if ((pdl ? build_graph_pdl(pl, pl->gs_pdl) : build_graph(pl, pl->gs)) == POISSON_OK) pl->use_graph = true; else cudaGetLastError();
+        if ((pdl ? build_graph_pdl(pl, pl->gs_pdl, nullptr) : build_graph(pl, pl->gs, nullptr)) == POISSON_OK) pl->use_graph = true; else cudaGetLastError();
         return POISSON_OK;
     }
     if ((e_tune && e_tune[0] == '0') || e_pdl || (e_fused && e_fused[0] == '1')) return POISSON_OK;   // forced / off
@@ -688,8 +839,8 @@ static int tune_plan(poisson_plan *pl) {
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { cudaGetLastError(); cleanup(); return POISSON_OK; }
     const bool modes[5][3] = {{false, false, false}, {true, false, false}, {false, true, false}, {false, false, true}, {true, false, true}};   // {pdl, fused, graph}
     int best = 0; float best_ms = 1e30f;
-    if (build_graph(pl, pl->gs) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }      // no graph: that mode is skipped
-    if (build_graph_pdl(pl, pl->gs_pdl) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }
+    if (build_graph(pl, pl->gs, nullptr) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }      // no graph: that mode is skipped
+    if (build_graph_pdl(pl, pl->gs_pdl, nullptr) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }
     for (int m = 0; m < 5 && rc == POISSON_OK; ++m) {
         if (modes[m][1] && !pl->fused) continue;
         if (modes[m][2] && !(modes[m][0] ? pl->gs_pdl.exec : pl->gs.exec)) continue;

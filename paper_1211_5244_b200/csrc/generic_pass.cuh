@@ -1,0 +1,217 @@
+// generic_pass.cuh -- the five fused passes for ANY transform length ("general sizes":
+// PAPER.md:89 "various grid sizes ... maximal for large power of two sizes").
+//
+// The register engine of passes.cuh is compiled for the lengths of sizes.def (two register passes, S = RA * RB).
+// Every other length -- odd N, factors 7, 11, 13, ..., three or more radices (300, 360, 600, 720, 900), primes and
+// 2 * prime -- runs here: ONE kernel per (precision, pass kind) whose transform length, tile width and radix list are
+// run-time values.  A CTA holds a tile of P pencils x S points in shared memory and runs a Stockham autosort
+// mixed-radix FFT on it:
+//
+//     n = S, s = 1;  for every radix R of S (product of the radices = S):   m = n / R
+//         y[q + s (R j + k)] = w_n^{j k}  sum_{r < R}  x[q + s (j + m r)]  w_R^{r k}      j < m, q < s, k < R
+//         swap(x, y);  n = m;  s = s R
+//
+// (natural order in, natural order out, no bit reversal).  A radix-R butterfly is the R-term sum written out, so a
+// prime factor p costs O(p) per point: a prime length degenerates to the O(S^2) DFT (where a Bluestein chirp-z would be
+// the asymptotically better choice), and every composite length is O(S sum R_i).  Twiddles come from the plan's
+// table exp(-2 pi i m / S) in shared memory.  The paper's spread / compactification are the zero fill of
+// the tile's upper half on load and the store of the lower half only; R2C / C2R pack two real pencils
+// adjacent in x into one complex transform exactly as passes.cuh does, with an unpaired last pencil when N_x is odd.
+// The same kernel multiplies by a COMPLEX K^F (poisson_set_kernel_complex: kernels without K(-r) = K(r)).
+#pragma once
+
+#include "passes.cuh"
+
+namespace pfft {
+
+constexpr int GEN_NT = 256;          // threads per CTA
+constexpr int GEN_MAX_S = 4096;      // longest generic transform (three S-point arrays per pencil must fit shared memory)
+
+// tile pitch: odd number of elements, so that both "lanes along pencils" and "lanes along the transform" spread over banks
+PF_CE int gen_pitch(int P) { return (P % 2 == 0) ? P + 1 : P; }
+PF_CE size_t gen_smem_bytes(int S, int P, size_t cplx_bytes) { return ((size_t)2 * S * gen_pitch(P) + S) * cplx_bytes; }
+
+template <typename T> PF_HD cx<T> gen_w(const cx<T> *tw, int i, bool inv) { const cx<T> w = tw[i]; return inv ? conj(w) : w; }
+
+// One Stockham pass sequence over the tile in x (result returned in the buffer the function returns).
+template <typename T>
+PF_HD cx<T> *gen_fft(cx<T> *x, cx<T> *y, const cx<T> *tw, const PassParams &prm, bool inv, int tid) {
+    const int S = prm.gen_S, P = prm.gen_P, PP = gen_pitch(P);
+    int n = S, s = 1;
+    for (int f = 0; f < prm.gen_nfac; ++f) {
+        const int R = prm.gen_fac[f], m = n / R, wr = S / R, wn = S / n;
+        for (int idx = tid; idx < S * P; idx += GEN_NT) {
+            const int p = idx % P, e = idx / P;            // output element e = q + s (R j + k)
+            const int q = e % s, t = e / s, k = t % R, j = t / R;
+            const cx<T> *src = x + (q + s * j) * PP + p;
+            const int stride = s * m * PP;
+            T ar = 0, ai = 0;
+            int wi = 0;
+            const int step = (int)(((long long)wr * k) % S);
+            for (int r = 0; r < R; ++r) {
+                const cx<T> a = src[r * stride], w = gen_w(tw, wi, inv);
+                ar += a.re * w.re - a.im * w.im;
+                ai += a.re * w.im + a.im * w.re;
+                wi += step; if (wi >= S) wi -= S;
+            }
+            const cx<T> w = gen_w(tw, wn * j * k, inv);     // j k < n, so wn j k < S
+            y[e * PP + p] = mk<T>(ar * w.re - ai * w.im, ar * w.im + ai * w.re);
+        }
+        __syncthreads();
+        cx<T> *tmp = x; x = y; y = tmp;
+        n = m; s *= R;
+    }
+    return x;
+}
+
+template <typename T, int KIND>
+__global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams prm) {
+    extern __shared__ __align__(16) unsigned char pf_smem[];
+    const int S = prm.gen_S, P = prm.gen_P, PP = gen_pitch(P), tid = threadIdx.x;
+    const int H = S / 2 + 1;
+    const bool pruned = prm.gen_pruned != 0;
+    cx<T> *b0 = reinterpret_cast<cx<T> *>(pf_smem), *b1 = b0 + (size_t)S * PP, *tw = b1 + (size_t)S * PP;
+    pdl_launch_dependents();
+    { const cx<T> *tab = reinterpret_cast<const cx<T> *>(prm.tw); for (int i = tid; i < S; i += GEN_NT) tw[i] = tab[i]; }
+    pdl_wait_prior_grid();
+    __syncthreads();
+    const int n_half = pruned ? S / 2 : S;      // points that exist on the un-padded side of this pass
+
+    for (int tile = blockIdx.x; tile < prm.n_tiles; tile += gridDim.x) {
+        const int bi = tile / prm.n_tiles1, tl = tile - bi * prm.n_tiles1;
+        const int g = tl / prm.tiles_per_g, p0 = (tl % prm.tiles_per_g) * P;
+        const int ncols = prm.n_p - p0 < P ? prm.n_p - p0 : P;
+        cx<T> *x = b0, *y = b1;
+
+        // ---------------- load (spread: the zero half is generated here)
+        if constexpr (KIND == KIND_F1) {            // two real pencils adjacent in x -> one complex pencil
+            const T *src = (prm.use_list == 1 ? reinterpret_cast<const T *>(prm.blist[bi]) : reinterpret_cast<const T *>(prm.in) + bi * prm.bs_in) + g * prm.gs_in;
+            for (int idx = tid; idx < S * P; idx += GEN_NT) {
+                const int q = idx % P, n = idx / P;
+                cx<T> v = mk<T>((T)0, (T)0);
+                if (n < n_half && q < ncols) {
+                    const long long xr = 2LL * (p0 + q);
+                    v.re = src[n * prm.ns_in + xr * prm.ps_in];
+                    if (xr + 1 < prm.gen_nreal) v.im = src[n * prm.ns_in + (xr + 1) * prm.ps_in];
+                }
+                x[n * PP + q] = v;
+            }
+        } else if constexpr (KIND == KIND_I1) {     // Z_k = A_k + i B_k,  Z_{S-k} = conj A_k + i conj B_k
+            const cx<T> *src = pass_in<T>(prm, bi) + g * prm.gs_in;
+            for (int idx = tid; idx < H * P; idx += GEN_NT) {
+                const int q = idx % P, k = idx / P;
+                cx<T> a = mk<T>((T)0, (T)0), b = a;
+                if (q < ncols) {
+                    const long long xr = 2LL * (p0 + q);
+                    a = src[k * prm.ns_in + xr * prm.ps_in];
+                    if (xr + 1 < prm.gen_nreal) b = src[k * prm.ns_in + (xr + 1) * prm.ps_in];
+                }
+                x[k * PP + q] = mk<T>(a.re - b.im, a.im + b.re);
+                if (k > 0 && S - k >= H) x[(S - k) * PP + q] = mk<T>(a.re + b.im, b.re - a.im);
+            }
+        } else {
+            const cx<T> *src = pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in;
+            const int n_in = (KIND == KIND_I2) ? S : n_half;
+            const bool lanes_p = prm.gen_lanes_p != 0;
+            for (int idx = tid; idx < S * P; idx += GEN_NT) {
+                int n, p;
+                if (lanes_p) { p = idx % P; n = idx / P; } else { n = idx % S; p = idx / S; }
+                x[n * PP + p] = (n < n_in && p < ncols) ? src[n * prm.ns_in + p * prm.ps_in] : mk<T>((T)0, (T)0);
+            }
+        }
+        __syncthreads();
+
+        // ---------------- transform(s)
+        constexpr bool FIRST_INV = KIND == KIND_I2 || KIND == KIND_I1;
+        cx<T> *r = gen_fft<T>(x, y, tw, prm, FIRST_INV, tid);
+        cx<T> *o = (r == b0) ? b1 : b0;
+        if constexpr (KIND == KIND_F3) {            // V^F = K^F rho^F (Eq. 3), then straight back
+            const bool lanes_p = prm.gen_lanes_p != 0;
+            const long long kbase = lanes_p ? (long long)g * S * prm.n_p + p0 : ((long long)g * prm.n_p + p0) * S;
+            for (int idx = tid; idx < S * P; idx += GEN_NT) {
+                int k, p;
+                if (lanes_p) { p = idx % P; k = idx / P; } else { k = idx % S; p = idx / S; }
+                if (p < ncols) {
+                    const long long ki = kbase + (lanes_p ? (long long)k * prm.n_p + p : (long long)p * S + k);
+                    const cx<T> v = r[k * PP + p];
+                    if (prm.gen_kcplx) r[k * PP + p] = v * reinterpret_cast<const cx<T> *>(prm.kint)[ki];
+                    else r[k * PP + p] = scale(v, reinterpret_cast<const T *>(prm.kint)[ki]);
+                }
+            }
+            __syncthreads();
+            r = gen_fft<T>(r, o, tw, prm, true, tid);
+        }
+
+        // ---------------- store (compactification: only the lower half leaves the chip)
+        if constexpr (KIND == KIND_F1) {            // A = (Z_k + conj Z_{S-k}) / 2,  B = -i (Z_k - conj Z_{S-k}) / 2,  k <= S/2
+            cx<T> *dst = pass_out<T>(prm, bi) + g * prm.gs_out;
+            for (int idx = tid; idx < H * P; idx += GEN_NT) {
+                const int q = idx % P, k = idx / P;
+                if (q < ncols) {
+                    const cx<T> zk = r[k * PP + q], zp = r[((S - k) % S) * PP + q];
+                    const T hf = (T)0.5;
+                    const long long xr = 2LL * (p0 + q);
+                    dst[k * prm.ns_out + xr * prm.ps_out] = mk<T>(hf * (zk.re + zp.re), hf * (zk.im - zp.im));
+                    if (xr + 1 < prm.gen_nreal) dst[k * prm.ns_out + (xr + 1) * prm.ps_out] = mk<T>(hf * (zk.im + zp.im), hf * (zp.re - zk.re));
+                }
+            }
+        } else if constexpr (KIND == KIND_I1) {     // real part -> pencil 2q, imaginary part -> pencil 2q + 1
+            T *dst = (prm.use_list == 2 ? reinterpret_cast<T *>(const_cast<void *>(prm.blist[bi])) : reinterpret_cast<T *>(prm.out) + bi * prm.bs_out) + g * prm.gs_out;
+            for (int idx = tid; idx < n_half * P; idx += GEN_NT) {
+                const int q = idx % P, n = idx / P;
+                if (q < ncols) {
+                    const cx<T> v = r[n * PP + q];
+                    const long long xr = 2LL * (p0 + q);
+                    dst[n * prm.ns_out + xr * prm.ps_out] = v.re;
+                    if (xr + 1 < prm.gen_nreal) dst[n * prm.ns_out + (xr + 1) * prm.ps_out] = v.im;
+                }
+            }
+        } else {
+            cx<T> *dst = pass_out<T>(prm, bi) + g * prm.gs_out + p0 * prm.ps_out;
+            const int n_out = (KIND == KIND_F2) ? S : n_half;
+            const bool lanes_p = prm.gen_lanes_p != 0;
+            for (int idx = tid; idx < n_out * P; idx += GEN_NT) {
+                int n, p;
+                if (lanes_p) { p = idx % P; n = idx / P; } else { n = idx % n_out; p = idx / n_out; }
+                if (p < ncols) dst[n * prm.ns_out + p * prm.ps_out] = r[n * PP + p];
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// K^F re-layout for the generic F3 kernel (the kernel is transposed once): natural order of the pass,
+//   lanes along pencils:   kint[(g S_c + k_c) n_p + pp]        lanes along the transform:   kint[(g n_p + pp) S_c + k_c]
+// pre-multiplied by 1 / (S_x S_y S_z).  cplx: the caller's array holds complex values and the half not passed is the
+// Hermitian image K^F(-k) = conj K^F(k) (a real kernel K without inversion symmetry).
+struct GenericRelayoutParams {
+    int S, n_p, lanes_p, cplx;
+    int a_axis, c_axis;
+    int sx, sy, sz;
+    long long total;      // points (not reals)
+    double scale;
+};
+
+template <typename T>
+__global__ void generic_relayout_kernel(const T *__restrict__ kuser, T *__restrict__ kint, const GenericRelayoutParams q) {
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < q.total; idx += (long long)gridDim.x * blockDim.x) {
+        long long g, kc, pp;
+        if (q.lanes_p) { pp = idx % q.n_p; kc = (idx / q.n_p) % q.S; g = idx / ((long long)q.n_p * q.S); }
+        else { kc = idx % q.S; pp = (idx / q.S) % q.n_p; g = idx / ((long long)q.n_p * q.S); }
+        long long f[3];
+        f[3 - q.a_axis - q.c_axis] = pp; f[q.c_axis] = kc; f[q.a_axis] = g;
+        long long kx = f[0], ky = f[1], kz = f[2];
+        const int hx = q.sx / 2 + 1;
+        bool mirrored = false;
+        if (kx > q.sx / 2) { kx = q.sx - kx; ky = (q.sy - ky) % q.sy; kz = (q.sz - kz) % q.sz; mirrored = true; }
+        const long long u = (kz * q.sy + ky) * hx + kx;
+        if (q.cplx) {
+            kint[2 * idx] = (T)((double)kuser[2 * u] * q.scale);
+            kint[2 * idx + 1] = (T)((double)kuser[2 * u + 1] * (mirrored ? -q.scale : q.scale));
+        } else {
+            kint[idx] = (T)((double)kuser[u] * q.scale);
+        }
+    }
+}
+
+}  // namespace pfft

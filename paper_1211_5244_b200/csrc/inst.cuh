@@ -21,7 +21,7 @@ __global__ void __launch_bounds__(G::NT, G::MINB) pass_kernel(const PassParams p
 
 template <class G, bool PRUNED, int KIND>
 static void reg_one(int prec, int variant) {
-    KernelEntry e;
+    KernelEntry e{};
     e.kind = KIND; e.S = G::S; e.pruned = PRUNED ? 1 : 0; e.lanes_p = G::LANES_P ? 1 : 0; e.prec = prec;
     e.variant = variant; e.nbuf = G::NBUF; e.tws = G::TWS ? 1 : 0; e.minb = G::MINB; e.stg = G::STG;
     e.RA = G::RA; e.RB = G::RB;

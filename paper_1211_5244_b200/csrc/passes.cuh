@@ -112,6 +112,10 @@ struct PassParams {
     int use_list;      // 0: in/out + bi * bs_in/bs_out; 1: inputs are blist[bi] (F1: rho); 2: outputs are blist[bi] (I1: V)
     long long bs_in, bs_out;   // elements between the intermediates of consecutive densities
     const void *blist[PF_MAX_WIDE];
+    // any-length kernel only (generic_pass.cuh): transform length, pencils per tile, radices (product = gen_S), zero-padded axis,
+    // real pencils along x of the R2C / C2R pass, complex K^F
+    int gen_S, gen_P, gen_nfac, gen_pruned, gen_nreal, gen_kcplx, gen_lanes_p;
+    int gen_fac[16];
 };
 
 template <typename T> PF_HD const cx<T> *pass_in(const PassParams &prm, int bi) {

@@ -16,6 +16,9 @@ struct PassDesc {
     int S;         // transform length
     int pruned;    // axis is zero padded
     int lanes_p;   // lanes along the pencil index (strided pencils)
+    int generic;   // 1: no register-engine kernel covers this pass (length not in sizes.def, or odd N_x in the R2C / C2R
+                   //    pass): it runs the any-length kernel of generic_pass.cuh
+    int n_real;    // F1 / I1: real pencils along x (= N_x); the generic kernel pairs them (2q, 2q + 1), the last one alone if odd
     long long n_g, n_p;
     long long gs_in, ns_in, ps_in, gs_out, ns_out, ps_out;
 };
@@ -30,6 +33,8 @@ struct PlanDesc {
     PassDesc pass[5];
     poisson_plan_info info;
 };
+
+#define PF_GENERIC_MAX_S 4096   // longest transform of the any-length kernel (generic_pass.cuh: GEN_MAX_S)
 
 inline bool length_in_list(int S) {
 #define PF_SIZE(S, RA, RB, TPP) S,
@@ -53,10 +58,8 @@ inline int plan_build(int nx, int ny, int nz, const int bc_in[3], int prec, Plan
         if (d.n[a] > (1 << 20)) return POISSON_EUNSUPPORTED;
         d.s[a] = d.n[a] * (d.bc[a] == POISSON_BC_FREE ? 2 : 1);   // S_i = N_i * B_i
     }
-    for (int a = 0; a < 3; ++a) {
-        if (d.n[a] % 2) return POISSON_EUNSUPPORTED;             // pairs along x; S_a/2+1 split
-        if (!length_in_list(d.s[a])) return POISSON_EUNSUPPORTED;
-    }
+    for (int a = 0; a < 3; ++a)
+        if (d.s[a] > PF_GENERIC_MAX_S) return POISSON_EUNSUPPORTED;   // the only refusal: above the any-length kernel's limit
     auto per = [&](int a) { return d.bc[a] == POISSON_BC_PERIODIC; };
     // a: never x (the half spectrum H = S_a/2+1 is odd and would break 128-byte rows on the
     // contiguous axis); periodic preferred, z preferred on a tie.
@@ -81,8 +84,17 @@ inline int plan_build(int nx, int ny, int nz, const int bc_in[3], int prec, Plan
 
     // F1 / I1: axis a, strided, pairs along x
     PassDesc f1{}; f1.kind = POISSON_PASS_F1; f1.axis = a; f1.S = d.s[a]; f1.pruned = !per(a); f1.lanes_p = 1;
-    f1.n_g = d.n[o]; f1.n_p = d.n[0] / 2;
-    f1.gs_in = stride(extp, o); f1.ns_in = stride(extp, a); f1.ps_in = 1;
+    f1.generic = !length_in_list(d.s[a]) || d.n[0] % 2 != 0;
+    f1.n_real = d.n[0];
+    f1.n_g = d.n[o];
+    if (!f1.generic) {   // register engine: rho / V read as x-pairs (one 16-byte access per pair)
+        f1.n_p = d.n[0] / 2;
+        f1.gs_in = stride(extp, o); f1.ns_in = stride(extp, a); f1.ps_in = 1;
+    } else {             // any-length kernel: strides in REAL elements, ceil(N_x / 2) pair pencils
+        const long long extr[3] = {d.n[0], d.n[1], d.n[2]};
+        f1.n_p = (d.n[0] + 1) / 2;
+        f1.gs_in = stride(extr, o); f1.ns_in = stride(extr, a); f1.ps_in = 1;
+    }
     f1.gs_out = stride(d.ext1, o); f1.ns_out = stride(d.ext1, a); f1.ps_out = 1;
     PassDesc i1 = f1; i1.kind = POISSON_PASS_I1;
     i1.gs_in = f1.gs_out; i1.ns_in = f1.ns_out; i1.ps_in = f1.ps_out;
@@ -90,6 +102,7 @@ inline int plan_build(int nx, int ny, int nz, const int bc_in[3], int prec, Plan
 
     // F2 / I2: axis b
     PassDesc f2{}; f2.kind = POISSON_PASS_F2; f2.axis = b; f2.S = d.s[b]; f2.pruned = !per(b);
+    f2.generic = !length_in_list(d.s[b]);
     // every middle pass works plane by plane: g = k_a (n_g = H), so that F3 / I2 of a plane depend on that plane only
     if (b == 0) {   // contiguous pencils along x, one per point of the remaining axis c
         f2.lanes_p = 0; f2.n_g = d.H; f2.n_p = d.ext1[c];
@@ -106,6 +119,7 @@ inline int plan_build(int nx, int ny, int nz, const int bc_in[3], int prec, Plan
 
     // F3: axis c, in place on A2
     PassDesc f3{}; f3.kind = POISSON_PASS_F3; f3.axis = c; f3.S = d.s[c]; f3.pruned = !per(c);
+    f3.generic = !length_in_list(d.s[c]);
     if (c == 0) {   // contiguous pencils along x, one per point of axis b (already at its padded length S_b)
         f3.lanes_p = 0; f3.n_g = d.H; f3.n_p = d.ext2[b];
         f3.gs_in = stride(d.ext2, a); f3.ns_in = 1; f3.ps_in = stride(d.ext2, b);

@@ -21,6 +21,9 @@ struct KernelEntry {
     int P, TPP, V, NT;
     size_t smem_bytes;
     const void *func;  // __global__ void (*)(PassParams)
+    // any-length kernel (generic_pass.cuh): a per-plan entry with run-time length, tile width and radix list
+    int generic;       // 0 for the compiled register-engine kernels
+    int gen_nfac, gen_fac[16];
 };
 
 // A fused solve kernel (solve_kernel.cuh): all five passes of one (axis a, axis b, axis c) combination.

@@ -95,8 +95,9 @@ def test_argument_validation(lib):
     assert lib.poisson_plan_describe(8, 8, 8, bc, 7, ctypes.byref(info)) == 1           # EINVAL: precision
     assert lib.poisson_plan_describe(8, 8, 8, (ctypes.c_int * 3)(0, 2, 0), 0, ctypes.byref(info)) == 1
     assert lib.poisson_plan_describe(8, 8, 8, bc, 0, None) == 1                          # EINVAL: null
-    assert lib.poisson_plan_describe(7, 8, 8, bc, 0, ctypes.byref(info)) == 2           # EUNSUPPORTED: odd N
-    assert lib.poisson_plan_describe(8, 8, 14, bc, 0, ctypes.byref(info)) == 2          # EUNSUPPORTED: S = 28
+    assert lib.poisson_plan_describe(7, 8, 8, bc, 0, ctypes.byref(info)) == 0           # odd N: planned (any-length kernel)
+    assert lib.poisson_plan_describe(8, 8, 14, bc, 0, ctypes.byref(info)) == 0          # S = 28 = 4 * 7: planned
+    assert lib.poisson_plan_describe(8, 8, 2049, bc, 0, ctypes.byref(info)) == 2        # EUNSUPPORTED: S = 4098 > 4096
     assert lib.poisson_plan_describe(8, 8, 8, bc, 0, ctypes.byref(info)) == 0
     handle = ctypes.c_void_p(123)
     assert lib.poisson_plan_create(ctypes.byref(handle), 8, 8, 8, bc, -1.0, 0) == 1     # EINVAL: h <= 0
@@ -122,19 +123,30 @@ SUPPORTED_LENGTHS = [4, 8, 12, 16, 20, 24, 32, 36, 40, 48, 60, 64, 72, 80, 96, 1
                      256, 288, 320, 384, 400, 480, 512, 576, 640, 768, 1024]
 
 
-def test_supported_lengths_match_design_reading_12():
-    """DESIGN.md reading 12 ('various grid sizes'): exactly the lengths of csrc/sizes.def are planned, every
-    other even length is refused with EUNSUPPORTED; a periodic axis uses S = N, a free axis S = 2N."""
-    for s in range(4, 1100, 2):
-        ok_p = s in SUPPORTED_LENGTHS
+def test_every_length_is_planned_up_to_the_any_length_limit():
+    """DESIGN.md reading 12 ('various grid sizes'): every N >= 1 is planned -- odd N, factors 7, 11, ...,
+    primes -- with S = N on a periodic axis and S = 2N on a free one; only a padded length above the
+    any-length kernel's limit (4096) is refused with EUNSUPPORTED.  The lengths of csrc/sizes.def keep their compiled
+    register-engine kernels (checked on the GPU by the parity sweeps)."""
+    for n in list(range(1, 520)) + [521, 769, 1000, 1023, 1025, 2048]:
+        for bc_y in (0, 1):
+            info = pk.poisson_plan_describe(8, n, 8, (0, bc_y, 0), pk.FP64)
+            assert list(info.s) == [16, n * (2 if bc_y == 0 else 1), 16]
+            assert info.half_len == info.s[info.order[0]] // 2 + 1 and info.order[0] != 0
+        info = pk.poisson_plan_describe(n, 4, 4, (1, 1, 1), pk.FP32)               # odd N_x, periodic: S_x = N_x
+        assert list(info.s) == [n, 4, 4]
+    for n, bc_z, ok in ((4096, 1, True), (2048, 0, True), (4097, 1, False), (2049, 0, False)):
         try:
-            info = pk.poisson_plan_describe(8, s, 8, (0, 1, 0), pk.FP64)     # periodic y: S_y = N_y
-            assert ok_p and list(info.s) == [16, s, 16]
+            pk.poisson_plan_describe(4, 4, n, (0, 0, bc_z), pk.FP64)
+            assert ok
         except pk.PoissonError as e:
-            assert e.status == 2 and not ok_p
-        if s % 4 == 0:                                                       # free y with N_y = s/2 (even)
-            try:
-                info = pk.poisson_plan_describe(8, s // 2, 8, (0, 0, 0), pk.FP32)
-                assert ok_p and list(info.s) == [16, s, 16]
-            except pk.PoissonError as e:
-                assert e.status == 2 and not ok_p
+            assert e.status == 2 and not ok
+
+
+def test_half_spectrum_length_and_rows_for_odd_sizes():
+    """S_a/2 + 1 outputs are kept by the R2C pass; for odd S_a that is (S_a + 1)/2.  Row counts per step
+     for an all-odd surface grid: a = y (periodic), b = x (periodic), c = z (free)."""
+    info = pk.poisson_plan_describe(7, 9, 5, (1, 1, 0), pk.FP64)
+    assert list(info.s) == [7, 9, 10] and list(info.order) == [1, 0, 2] and info.half_len == 9 // 2 + 1
+    assert list(info.rows) == [7 * 5, 5 * 5, 5 * 7, 5 * 5, 7 * 5]
+    assert list(info.length) == [9, 7, 10, 7, 9]

@@ -19,7 +19,7 @@ _lib = None
 
 def build(force: bool = False) -> Path:
     if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
-        subprocess.run(["g++", "-std=c++17", "-O3", "-march=native", "-fopenmp", "-fPIC", "-shared", str(_SRC), "-o", str(_LIB)],
+        subprocess.run(["g++", "-std=c++17", "-O3", "-march=native", "-fcx-limited-range", "-fopenmp", "-fPIC", "-shared", str(_SRC), "-o", str(_LIB)],
                        check=True)
     return _LIB
 

@@ -13,7 +13,8 @@
 //   step 4  inverse along b, keep N_b;   step 5  inverse along x (complex-to-real), keep N_x.
 // Of y and z the periodic axis is processed before the free one.  fp64, OpenMP over independent pencils.
 //
-// build: g++ -O3 -march=native -fopenmp -shared -fPIC baseline/cpu_fft.cpp -o baseline/libcpu_fft.so
+// build: g++ -O3 -march=native -fcx-limited-range -fopenmp -shared -fPIC baseline/cpu_fft.cpp -o baseline/libcpu_fft.so
+#include <algorithm>
 #include <cmath>
 #include <complex>
 #include <cstring>
@@ -114,7 +115,10 @@ int cpu_poisson_solve(const double *rho, const double *Kf_half, double *V, const
     const size_t a1n = (size_t)nz * ny * H;
     // after step 2 the second axis is padded: [nz][Sy][H] (y first) or [Sz][ny][H] (z first)
     const size_t a2n = y_first ? (size_t)nz * Sy * H : (size_t)Sz * ny * H;
-    std::vector<cd> A1(a1n), A2(a2n);
+    // workspace kept between calls (repeated solves with one kernel are the paper's usage)
+    static std::vector<cd> A1, A2;
+    if (A1.size() < a1n) A1.resize(a1n);
+    if (A2.size() < a2n) A2.resize(a2n);
     const double scale = 1.0 / ((double)Sx * Sy * Sz);
     const int smax = std::max(Sx, std::max(Sy, Sz));
 
@@ -137,68 +141,77 @@ int cpu_poisson_solve(const double *rho, const double *Kf_half, double *V, const
                 if (o1) o1[k] = cd(0.0, -0.5) * (zk - zp);
             }
         }
+        // Steps 2-4 work on pencils that are strided in memory (element stride `es`, k fastest).  KB pencils adjacent in k
+        // are gathered together, so that every 64-byte line fetched is used whole.
+        constexpr int KB = 4;
+        std::vector<cd> g0((size_t)KB * smax), g1((size_t)KB * smax);
+        // pencil group: n_in values at src + i*es_in (zero padded to S), transform(s), n_out values to dst + i*es_out
+        auto pencils = [&](const Fft1d &f, const cd *src, size_t es_in, int n_in, cd *dst, size_t es_out, int n_out, int kb,
+                           bool inv, const double *kmul, size_t es_k) {
+            const int S1 = f.S;
+            for (int i = 0; i < n_in; ++i) for (int j = 0; j < kb; ++j) g0[(size_t)j * smax + i] = src[i * es_in + j];
+            for (int j = 0; j < kb; ++j) {
+                cd *a = g0.data() + (size_t)j * smax, *b = g1.data() + (size_t)j * smax;
+                for (int i = n_in; i < S1; ++i) a[i] = cd(0.0, 0.0);
+                cd *r = f.run(a, b, inv);
+                if (kmul) {                  // step 3: K^F multiply, then straight back
+                    cd *other = r == a ? b : a;
+                    for (int i = 0; i < S1; ++i) r[i] *= kmul[i * es_k + j] * scale;
+                    r = f.run(r, other, true);
+                }
+                if (r != a) std::memcpy(a, r, sizeof(cd) * (size_t)n_out);
+            }
+            for (int i = 0; i < n_out; ++i) for (int j = 0; j < kb; ++j) dst[i * es_out + j] = g0[(size_t)j * smax + i];
+        };
+        const int kgroups = (H + KB - 1) / KB;
         // ---- step 2: second axis b (y if y_first else z), padded
         if (y_first) {
 #pragma omp for schedule(static) collapse(2)
             for (int z = 0; z < nz; ++z)
-                for (int k = 0; k < H; ++k) {
-                    for (int y = 0; y < ny; ++y) buf0[y] = A1[((size_t)z * ny + y) * H + k];
-                    for (int y = ny; y < Sy; ++y) buf0[y] = cd(0.0, 0.0);
-                    const cd *r = fy.run(buf0.data(), buf1.data(), false);
-                    for (int y = 0; y < Sy; ++y) A2[((size_t)z * Sy + y) * H + k] = r[y];
+                for (int kg = 0; kg < kgroups; ++kg) {
+                    const int k = kg * KB, kb = std::min(KB, H - k);
+                    pencils(fy, A1.data() + (size_t)z * ny * H + k, H, ny, A2.data() + (size_t)z * Sy * H + k, H, Sy, kb, false, nullptr, 0);
                 }
         } else {
 #pragma omp for schedule(static) collapse(2)
             for (int y = 0; y < ny; ++y)
-                for (int k = 0; k < H; ++k) {
-                    for (int z = 0; z < nz; ++z) buf0[z] = A1[((size_t)z * ny + y) * H + k];
-                    for (int z = nz; z < Sz; ++z) buf0[z] = cd(0.0, 0.0);
-                    const cd *r = fz.run(buf0.data(), buf1.data(), false);
-                    for (int z = 0; z < Sz; ++z) A2[((size_t)z * ny + y) * H + k] = r[z];
+                for (int kg = 0; kg < kgroups; ++kg) {
+                    const int k = kg * KB, kb = std::min(KB, H - k);
+                    pencils(fz, A1.data() + (size_t)y * H + k, (size_t)ny * H, nz, A2.data() + (size_t)y * H + k, (size_t)ny * H, Sz, kb, false, nullptr, 0);
                 }
         }
         // ---- step 3: third axis c forward, K^F multiply, inverse, keep the first N_c (the full spectrum never exists)
         if (y_first) {       // c = z: A2 is [nz][Sy][H]
 #pragma omp for schedule(static) collapse(2)
             for (int y = 0; y < Sy; ++y)
-                for (int k = 0; k < H; ++k) {
-                    for (int z = 0; z < nz; ++z) buf0[z] = A2[((size_t)z * Sy + y) * H + k];
-                    for (int z = nz; z < Sz; ++z) buf0[z] = cd(0.0, 0.0);
-                    cd *r = fz.run(buf0.data(), buf1.data(), false);
-                    cd *other = r == buf0.data() ? buf1.data() : buf0.data();
-                    for (int z = 0; z < Sz; ++z) r[z] *= Kf_half[((size_t)z * Sy + y) * H + k] * scale;
-                    const cd *v = fz.run(r, other, true);
-                    for (int z = 0; z < nz; ++z) A2[((size_t)z * Sy + y) * H + k] = v[z];
+                for (int kg = 0; kg < kgroups; ++kg) {
+                    const int k = kg * KB, kb = std::min(KB, H - k);
+                    cd *p = A2.data() + (size_t)y * H + k;
+                    pencils(fz, p, (size_t)Sy * H, nz, p, (size_t)Sy * H, nz, kb, false, Kf_half + (size_t)y * H + k, (size_t)Sy * H);
                 }
         } else {             // c = y: A2 is [Sz][ny][H]
 #pragma omp for schedule(static) collapse(2)
             for (int z = 0; z < Sz; ++z)
-                for (int k = 0; k < H; ++k) {
-                    for (int y = 0; y < ny; ++y) buf0[y] = A2[((size_t)z * ny + y) * H + k];
-                    for (int y = ny; y < Sy; ++y) buf0[y] = cd(0.0, 0.0);
-                    cd *r = fy.run(buf0.data(), buf1.data(), false);
-                    cd *other = r == buf0.data() ? buf1.data() : buf0.data();
-                    for (int y = 0; y < Sy; ++y) r[y] *= Kf_half[((size_t)z * Sy + y) * H + k] * scale;
-                    const cd *v = fy.run(r, other, true);
-                    for (int y = 0; y < ny; ++y) A2[((size_t)z * ny + y) * H + k] = v[y];
+                for (int kg = 0; kg < kgroups; ++kg) {
+                    const int k = kg * KB, kb = std::min(KB, H - k);
+                    cd *p = A2.data() + (size_t)z * ny * H + k;
+                    pencils(fy, p, H, ny, p, H, ny, kb, false, Kf_half + (size_t)z * Sy * H + k, H);
                 }
         }
         // ---- step 4: inverse along b, keep N_b
         if (y_first) {
 #pragma omp for schedule(static) collapse(2)
             for (int z = 0; z < nz; ++z)
-                for (int k = 0; k < H; ++k) {
-                    for (int y = 0; y < Sy; ++y) buf0[y] = A2[((size_t)z * Sy + y) * H + k];
-                    const cd *r = fy.run(buf0.data(), buf1.data(), true);
-                    for (int y = 0; y < ny; ++y) A1[((size_t)z * ny + y) * H + k] = r[y];
+                for (int kg = 0; kg < kgroups; ++kg) {
+                    const int k = kg * KB, kb = std::min(KB, H - k);
+                    pencils(fy, A2.data() + (size_t)z * Sy * H + k, H, Sy, A1.data() + (size_t)z * ny * H + k, H, ny, kb, true, nullptr, 0);
                 }
         } else {
 #pragma omp for schedule(static) collapse(2)
             for (int y = 0; y < ny; ++y)
-                for (int k = 0; k < H; ++k) {
-                    for (int z = 0; z < Sz; ++z) buf0[z] = A2[((size_t)z * ny + y) * H + k];
-                    const cd *r = fz.run(buf0.data(), buf1.data(), true);
-                    for (int z = 0; z < nz; ++z) A1[((size_t)z * ny + y) * H + k] = r[z];
+                for (int kg = 0; kg < kgroups; ++kg) {
+                    const int k = kg * KB, kb = std::min(KB, H - k);
+                    pencils(fz, A2.data() + (size_t)y * H + k, (size_t)ny * H, Sz, A1.data() + (size_t)y * H + k, (size_t)ny * H, nz, kb, true, nullptr, 0);
                 }
         }
         // ---- step 5: inverse along x, complex-to-real (two rows per transform), keep N_x

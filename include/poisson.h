@@ -128,6 +128,11 @@ POISSON_API int poisson_set_kernel(poisson_plan *plan, const void *K_f_dev, void
 POISSON_API int poisson_set_kernel_complex(poisson_plan *plan, const void *K_f_dev, void *stream);
 
 /* One solve (the 13 steps of PAPER.md:57-71 as 5 fused launches, or one, on `stream`; see poisson_plan_launch_mode).
+ * Opt-in (POISSON_CHUNK=n planes per chunk, or POISSON_CHUNK_MB=m, read at plan creation): the three middle passes run chunk
+ * by chunk of k_a planes, F1 | F2, F3, I2 per chunk | I1 = 2 + 3 * chunks launches, through an A2 buffer that holds ONE chunk
+ * and therefore lives in the 126 MB L2 -- A2's four sweeps never reach HBM and the plan's workspace shrinks by most of A2
+ * (fewer round trips to global memory).  Measured slower than the five whole-grid launches on B200 (the passes
+ * are not DRAM bound), hence off by default; useful when device memory is the limit.
  *   rho_dev: device, plan-precision reals [nz][ny][nx], 16-byte aligned, not modified
  *   V_dev  : device, same shape; may equal rho_dev (rho is consumed before V is written)
  * Asynchronous, allocates nothing, never touches host memory.  One plan = one solve in flight
@@ -175,7 +180,8 @@ POISSON_API int poisson_plan_batch_lanes(const poisson_plan *plan, int count, in
 
 /* Debug/test access to the plan's intermediates (per-pass parity).  which = 0: A1,
  * complex [.][.][.] after F1 (or after I2); which = 1: A2 after F2 / F3.  dims are the array
- * extents in memory order (z-extent, y-extent, x-extent), each axis holding N_i, S_i or H. */
+ * extents in memory order (z-extent, y-extent, x-extent), each axis holding N_i, S_i or H.  POISSON_EUNSUPPORTED for A2 of a
+ * chunked plan (it never exists whole), as is a partial pass range in poisson_debug_run_passes there. */
 POISSON_API int poisson_debug_workspace(const poisson_plan *plan, int which, void **ptr_dev /* out */,
                             long long dims[3] /* host, out */);
 /* Runs passes [first, last] (POISSON_PASS_*) of a solve only; same arguments as poisson_solve. */
@@ -183,8 +189,8 @@ POISSON_API int poisson_debug_run_passes(poisson_plan *plan, const void *rho_dev
                              int first_pass, int last_pass);
 
 /* Per-pass device timing for the roofline report (bench.py): identical to poisson_solve, but a CUDA
- * event is recorded on `stream` before the first pass and after every pass (6 events per solve,
- * from a pool the plan owns; at most 512 profiled solves between two reads).
+ * event is recorded on `stream` before the first launch and after every launch (launches + 1 events per solve,
+ * from a pool the plan owns; a chunked plan's launches are summed into their pass; at most 512 profiled solves between two reads).
  * poisson_profile_read synchronises on the recorded events, ADDS each pass's elapsed milliseconds
  * over all solves profiled since the last read into ms_sum[5], stores their number in *n_solves,
  * and resets the pool.  Errors: EINVAL, ENOKERNEL, ECUDA, ENOMEM (pool exhausted). */
@@ -208,7 +214,8 @@ POISSON_API int poisson_profile_read(poisson_plan *plan, double ms_sum[5] /* hos
 enum { POISSON_LAUNCH_FIVE = 0, POISSON_LAUNCH_FIVE_PDL = 1, POISSON_LAUNCH_FUSED = 2, POISSON_LAUNCH_GRAPH = 3, POISSON_LAUNCH_GRAPH_PDL = 4 };
 POISSON_API int poisson_plan_launch_mode(const poisson_plan *plan, int *mode /* host, out */, double ms_per_solve[5] /* host, out */);
 
-/* Number of kernel launches one poisson_solve enqueues (bench.py's gpu_launches): 5, or 1 in FUSED mode. */
+/* Number of kernel launches one poisson_solve enqueues (bench.py's gpu_launches): 5, 2 + 3 * chunks on a chunked plan, or 1
+ * in FUSED mode. */
 POISSON_API int poisson_plan_launches_per_solve(const poisson_plan *plan);
 
 /* Measures the plain-ALU fused-multiply-add peak of the current device for the given precision

@@ -161,13 +161,14 @@ struct Lane {
     struct GraphSolve *gs;       // this lane's five launches as a CUDA graph (graph launch mode), or NULL
 };
 
-// The five launches of one solve as an instantiated CUDA graph (kernel nodes F1 -> F2 -> F3 -> I2 -> I1): one graph
-// launch per solve; rho / V of the call are patched into the F1 / I1 nodes when they differ from the previous call.
+// The launches of one solve as an instantiated CUDA graph (kernel nodes F1 -> F2 -> F3 -> I2 -> I1, the middle three once per
+// plane chunk): one graph launch per solve; rho / V of the call are patched into the F1 / I1 nodes when they differ from the
+// previous call.
 struct GraphSolve {
     cudaGraph_t graph;
     cudaGraphExec_t exec;
-    cudaGraphNode_t node[5];
-    PassParams prm[5];
+    cudaGraphNode_t node_f1, node_i1;   // the two nodes whose parameters carry rho / V of the call
+    PassParams prm_f1, prm_i1;
     const void *rho;
     void *V;
 };
@@ -185,6 +186,9 @@ struct poisson_plan {
     int n_tiles[5], tiles_per_g[5];
     size_t pf_min_bytes;  // L2 prefetch (PassParams::prefetch) for arrays at least this large
     int pf_force[5];      // POISSON_PREFETCH=0..3 (one value, or one per pass) forces the prefetch bits (experiments), -1 = by size
+    int chunk_planes, n_chunks; // middle passes F2 -> F3 -> I2 run chunk by chunk of k_a planes through a chunk-sized A2 (1 chunk: whole grid)
+    long long a2_alloc_elems;   // complex elements of the A2 buffer actually allocated (one chunk when chunked)
+    int late_tw;               // PassParams::late_tw for every pass (POISSON_LATE_TW, default 1; 0 under programmatic dependent launch)
     int env_lanes, env_wide;   // POISSON_LANES / POISSON_WIDE as read at plan creation (-1: not set)
     bool env_lane_graph;       // POISSON_LANE_GRAPH=0 at plan creation: plain launches on the batch lanes (experiments)
     void *wide_a1, *wide_a2;   // intermediates of wide_w densities (several small solves per launch), allocated on first use
@@ -269,12 +273,50 @@ static GraphSolve *active_graph(poisson_plan *pl) {
 }
 static const GraphSolve *active_graph(const poisson_plan *pl) { return active_graph(const_cast<poisson_plan *>(pl)); }
 
+static int launches_per_solve(const poisson_plan *pl) { return pl->n_chunks <= 1 ? 5 : 2 + 3 * pl->n_chunks; }
+
 // Reals in the internal K^F copy: the register-engine F3 streams [tile][V][NT] (padded to whole tiles), the any-length
 // kernel reads the natural order of the pass (one real, or one complex number, per spectrum point).
 static long long kint_reals(const poisson_plan *pl) {
     const KernelEntry *e = pl->k[2];
     if (e->generic) return (long long)pl->d.pass[2].n_g * pl->d.pass[2].S * pl->d.pass[2].n_p * (pl->kcplx ? 2 : 1);
     return (long long)pl->n_tiles[2] * e->V * e->NT;
+}
+
+// Plane chunks for the middle passes (see for_each_launch).  OPT-IN: measured on B200 the chunked 512^3 solve moves 1.9 GB
+// instead of 4.0 GB through HBM and shrinks the workspace by most of A2, but it is SLOWER (fp64 794 -> 863 us with 96 MB
+// chunks, 910 us with 64 MB, 1111 us with 32 MB; fp32 449 -> 467 us): the S = 512 passes are held by their FP64 / shared-memory
+// pipes at 8 warps per SM, not by DRAM, and every extra launch costs a ramp-up and a partly filled last wave (DESIGN.md
+// section 10).  POISSON_CHUNK=n: n planes per chunk; POISSON_CHUNK_MB=m: chunks of about m MB, sized within [m/2, m] to the
+// plane count that leaves the smallest partly-filled last wave of tiles in the three middle passes.
+static void choose_chunks(poisson_plan *pl) {
+    const PlanDesc &d = pl->d;
+    const size_t cplx = 2 * pl->elem_real;
+    const long long plane_elems = d.a2_elems / d.H;
+    pl->chunk_planes = d.H; pl->n_chunks = 1; pl->a2_alloc_elems = d.a2_elems;
+    const char *env = std::getenv("POISSON_CHUNK");
+    const char *env_mb = std::getenv("POISSON_CHUNK_MB");
+    int planes = 0;
+    if (env) planes = std::atoi(env);
+    else if (env_mb && std::atof(env_mb) > 0.0) {
+        const double target = std::atof(env_mb) * 1048576.0;
+        const int pmax = (int)(target / ((double)plane_elems * cplx));
+        double best = -1.0;
+        for (int p = pmax; p >= 1 && p >= pmax / 2; --p) {
+            double eff = 1.0;
+            for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2; ++q) {
+                const long long T = (long long)p * pl->tiles_per_g[q], R = pl->resident[q];
+                const double e = (double)T / (double)(((T + R - 1) / R) * R);
+                eff = e < eff ? e : eff;
+            }
+            if (eff > best + 1e-9) { best = eff; planes = p; }
+        }
+    }
+    if (planes >= 1 && planes < d.H) {
+        pl->chunk_planes = planes;
+        pl->n_chunks = (d.H + planes - 1) / planes;
+        pl->a2_alloc_elems = plane_elems * planes;
+    }
 }
 
 // Picks the kernel of pass q (the compiled register-engine kernel for its length, else -- or when force_generic -- the
@@ -381,6 +423,7 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     { const char *env = std::getenv("POISSON_PDL"); pl->use_pdl = env && env[0] == '1'; }
     for (int q = 0; q < 5; ++q) pl->pf_force[q] = env_pass_value("POISSON_PREFETCH", q, -1);
     // every environment knob is read HERE, once; the solve path never calls getenv
+    { const char *env = std::getenv("POISSON_LATE_TW"); pl->late_tw = env ? std::atoi(env) : 1; }
     { const char *env = std::getenv("POISSON_LANES"); pl->env_lanes = env ? std::atoi(env) : -1; }
     { const char *env = std::getenv("POISSON_WIDE"); pl->env_wide = env ? std::atoi(env) : -1; }
     { const char *env = std::getenv("POISSON_LANE_GRAPH"); pl->env_lane_graph = !(env && env[0] == '0'); }
@@ -391,6 +434,8 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
         if (st != POISSON_OK) { free_plan(pl); return st; }
     }
 
+    choose_chunks(pl);
+
     // One-launch fused solve (solve_kernel.cuh) when this combination of axes was compiled and the per-pass
     // tiles agree with it; POISSON_FUSED=0 keeps the 5-launch path (per-pass experiments).
     {
@@ -400,7 +445,7 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
         int S3[3], pr3[3], lp3[3];
         const int qs[3] = {POISSON_PASS_F1, POISSON_PASS_F2, POISSON_PASS_F3};
         for (int q = 0; q < 3; ++q) { S3[q] = d.pass[qs[q]].S; pr3[q] = d.pass[qs[q]].pruned; lp3[q] = d.pass[qs[q]].lanes_p; }
-        const FusedEntry *fe = want ? find_fused(precision, S3, pr3, lp3) : nullptr;
+        const FusedEntry *fe = (want && pl->n_chunks <= 1) ? find_fused(precision, S3, pr3, lp3) : nullptr;   // the fused kernel needs all of A2
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
         bool any_generic = false;
@@ -434,7 +479,7 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     pl->kint_elems = kint_reals(pl);
     size_t ws = 0;
     cudaError_t ce = cudaMalloc(&pl->a1, (size_t)d.a1_elems * cplx); ws += (size_t)d.a1_elems * cplx;
-    if (ce == cudaSuccess) { ce = cudaMalloc(&pl->a2, (size_t)d.a2_elems * cplx); ws += (size_t)d.a2_elems * cplx; }
+    if (ce == cudaSuccess) { ce = cudaMalloc(&pl->a2, (size_t)pl->a2_alloc_elems * cplx); ws += (size_t)pl->a2_alloc_elems * cplx; }
     if (ce == cudaSuccess) { ce = cudaMalloc(&pl->kint, (size_t)pl->kint_elems * pl->elem_real); ws += (size_t)pl->kint_elems * pl->elem_real; }
     for (int q = 0; q < 3 && ce == cudaSuccess; ++q) {
         std::vector<unsigned char> host;
@@ -501,7 +546,7 @@ int poisson_plan_get_info(const poisson_plan *pl, poisson_plan_info *info) {
 
 size_t poisson_plan_workspace_bytes(const poisson_plan *pl) { return pl ? pl->workspace_bytes : 0; }
 
-int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? (pl->fused && pl->use_fused ? 1 : 5) : 0; }   // kernels per solve (graph mode: 5 kernel nodes)
+int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? (pl->fused && pl->use_fused ? 1 : launches_per_solve(pl)) : 0; }   // kernels per solve (graph mode: that many kernel nodes)
 
 int poisson_plan_launch_mode(const poisson_plan *pl, int *mode, double ms_per_solve[5]) {
     if (!pl || !mode || !ms_per_solve) return POISSON_EINVAL;
@@ -631,6 +676,9 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
     prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;
     prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q];
     prm.n_tiles1 = pl->n_tiles[q];   // one density per launch
+    // twiddle tables under the first tile's load latency; with programmatic dependent launch they are built BEFORE the wait
+    // on the previous pass instead (that is the part of a pass PDL overlaps with its predecessor's tail)
+    prm.late_tw = (pl->late_tw && !pl->use_pdl) ? 1 : 0;
     if (pl->k[q]->generic) {
         const KernelEntry *e = pl->k[q];
         prm.gen_S = e->S; prm.gen_P = e->P; prm.gen_nfac = e->gen_nfac; prm.gen_pruned = e->pruned;
@@ -643,7 +691,7 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
         const size_t r = pl->d.prec == POISSON_FP64 ? 8 : 4;
         const size_t in_bytes = q == POISSON_PASS_F1 ? (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * r
                               : (q == POISSON_PASS_F2 || q == POISSON_PASS_I1) ? (size_t)pl->d.a1_elems * 2 * r
-                              : (size_t)pl->d.a2_elems * 2 * r;
+                              : (size_t)pl->a2_alloc_elems * 2 * r;     // chunked: one chunk of A2, written moments ago
         const size_t k_bytes = (size_t)pl->kint_elems * r;
         prm.prefetch = (in_bytes >= pl->pf_min_bytes ? 1 : 0) | (q == POISSON_PASS_F3 && k_bytes >= pl->pf_min_bytes ? 2 : 0);
         if (pl->pf_force[q] >= 0) prm.prefetch = pl->pf_force[q];
@@ -668,48 +716,110 @@ static int run_fused(poisson_plan *pl, const void *rho, void *V, cudaStream_t st
     return POISSON_OK;
 }
 
+// Launches of one solve in order: F1 | F2, F3, I2 (once, or once per chunk of k_a planes) | I1.
+// Chunked plans (large grids): the three middle passes work plane by plane (g = k_a), so they can run chunk by chunk
+// through an A2 buffer that holds ONE chunk -- written by F2, transformed in place by F3, consumed by I2 while it is
+// still in the 126 MB L2, and overwritten by the next chunk before it is ever evicted: A2's four sweeps (and its
+// write-back) stop being HBM traffic (fewer round trips to global memory).
+// f(q, prm, grid) -> status, called once per launch; passes outside [first, last] are skipped.
+extern "C++" {
+template <class F>
+static int for_each_launch(const poisson_plan *pl, const void *rho, void *V, const Lane *ln, int first, int last, F &&f) {
+    const size_t cplx = 2 * pl->elem_real;
+    auto one = [&](int q) -> int { return (q < first || q > last) ? POISSON_OK : f(q, pass_params(pl, q, rho, V, ln), pl->grid[q]); };
+    int rc = one(POISSON_PASS_F1);
+    if (rc != POISSON_OK) return rc;
+    if (pl->n_chunks <= 1) {
+        for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2 && rc == POISSON_OK; ++q) rc = one(q);
+    } else {
+        const int G = pl->d.H;
+        for (int g0 = 0; g0 < G && rc == POISSON_OK; g0 += pl->chunk_planes) {
+            const int ng = G - g0 < pl->chunk_planes ? G - g0 : pl->chunk_planes;
+            for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2 && rc == POISSON_OK; ++q) {
+                if (q < first || q > last) continue;
+                PassParams prm = pass_params(pl, q, rho, V, ln);
+                prm.n_tiles = ng * pl->tiles_per_g[q];
+                prm.n_tiles1 = prm.n_tiles;
+                prm.k_g0 = g0;                                     // K^F is indexed by the plane's position in the whole grid
+                if (q == POISSON_PASS_F2) prm.in = static_cast<const char *>(prm.in) + (size_t)g0 * prm.gs_in * cplx;
+                if (q == POISSON_PASS_I2) prm.out = static_cast<char *>(prm.out) + (size_t)g0 * prm.gs_out * cplx;
+                // the A2 side of the pass addresses the chunk buffer: extents of A2 with chunk_planes along axis a
+                {
+                    const PlanDesc &d = pl->d;
+                    const int a = d.order[0], b = d.order[1], c = d.order[2];
+                    long long e[3] = {d.ext2[0], d.ext2[1], d.ext2[2]};
+                    e[a] = pl->chunk_planes;
+                    auto st = [&](int ax) -> long long { return ax == 0 ? 1 : (ax == 1 ? e[0] : e[0] * e[1]); };
+                    const int n_ax = q == POISSON_PASS_F3 ? c : b;                 // transformed axis of this pass
+                    const int p_ax = 3 - a - n_ax;                                 // pencil index axis
+                    const long long gs = st(a), ns = st(n_ax), ps = st(p_ax);
+                    if (q != POISSON_PASS_I2) { prm.gs_out = gs; prm.ns_out = ns; prm.ps_out = ps; }
+                    if (q != POISSON_PASS_F2) { prm.gs_in = gs; prm.ns_in = ns; prm.ps_in = ps; }
+                }
+                rc = f(q, prm, prm.n_tiles < pl->resident[q] ? prm.n_tiles : pl->resident[q]);
+            }
+        }
+    }
+    if (rc != POISSON_OK) return rc;
+    return one(POISSON_PASS_I1);
+}
+}  // extern "C++"
+
+// ev: optional, launches_per_solve + 1 events recorded before the first launch and after every launch
 static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t st, int first, int last,
                       cudaEvent_t *ev = nullptr, const Lane *ln = nullptr) {
     if (ev) PF_CUDA(cudaEventRecord(ev[0], st));
-    for (int q = first; q <= last; ++q) {
+    int item = 0;
+    return for_each_launch(pl, rho, V, ln, first, last, [&](int q, const PassParams &prm_in, int grid) -> int {
         const KernelEntry *e = pl->k[q];
-        PassParams prm = pass_params(pl, q, rho, V, ln);
+        PassParams prm = prm_in;
         void *args[] = {&prm};
         cudaLaunchConfig_t cfg{};
-        cfg.gridDim = dim3(pl->grid[q]); cfg.blockDim = dim3(e->NT);
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(e->NT);
         cfg.dynamicSmemBytes = e->smem_bytes; cfg.stream = st;
         cudaLaunchAttribute attr[1];
         attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // PDL: prologue overlaps the previous pass's tail
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr; cfg.numAttrs = pl->use_pdl ? 1 : 0;
         PF_CUDA(cudaLaunchKernelExC(&cfg, e->func, args));
-        if (ev) PF_CUDA(cudaEventRecord(ev[q + 1], st));
-    }
-    return POISSON_OK;
+        ++item;
+        if (ev) PF_CUDA(cudaEventRecord(ev[item], st));
+        return POISSON_OK;
+    });
 }
 
 // Builds the graph of one solve on the plan's own intermediates (explicit kernel nodes, plain dependencies).
 static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
     if (g.exec) return POISSON_OK;
     PF_CUDA(cudaGraphCreate(&g.graph, 0));
-    for (int q = 0; q < 5; ++q) {
+    cudaGraphNode_t prev = nullptr;
+    bool have_prev = false;
+    const int rc = for_each_launch(pl, nullptr, nullptr, ln, 0, 4, [&](int q, const PassParams &prm_in, int grid) -> int {
         const KernelEntry *e = pl->k[q];
-        g.prm[q] = pass_params(pl, q, nullptr, nullptr, ln);
-        void *args[] = {&g.prm[q]};
+        PassParams prm = prm_in;
+        if (q == POISSON_PASS_F1) g.prm_f1 = prm;
+        if (q == POISSON_PASS_I1) g.prm_i1 = prm;
+        void *args[] = {&prm};
         cudaKernelNodeParams kp{};
         kp.func = const_cast<void *>(e->func);
-        kp.gridDim = dim3(pl->grid[q]); kp.blockDim = dim3(e->NT);
+        kp.gridDim = dim3(grid); kp.blockDim = dim3(e->NT);
         kp.sharedMemBytes = (unsigned)e->smem_bytes;
         kp.kernelParams = args; kp.extra = nullptr;
-        PF_CUDA(cudaGraphAddKernelNode(&g.node[q], g.graph, q ? &g.node[q - 1] : nullptr, q ? 1 : 0, &kp));
-    }
+        cudaGraphNode_t node;
+        PF_CUDA(cudaGraphAddKernelNode(&node, g.graph, have_prev ? &prev : nullptr, have_prev ? 1 : 0, &kp));
+        if (q == POISSON_PASS_F1) g.node_f1 = node;
+        if (q == POISSON_PASS_I1) g.node_i1 = node;
+        prev = node; have_prev = true;
+        return POISSON_OK;
+    });
+    if (rc != POISSON_OK) { cudaGraphDestroy(g.graph); g.graph = nullptr; return rc; }
     PF_CUDA(cudaGraphInstantiate(&g.exec, g.graph, 0));
     g.rho = nullptr; g.V = nullptr;
     return POISSON_OK;
 }
 
-// The same graph with programmatic-dependent-launch edges: captured from the five PDL stream launches (capture turns
-// the launch attribute into programmatic edges), kernel nodes identified by their function.
+// The same graph with programmatic-dependent-launch edges: captured from the PDL stream launches (capture turns
+// the launch attribute into programmatic edges); the F1 / I1 kernel nodes are identified by their function.
 static int build_graph_pdl(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
     if (g.exec) return POISSON_OK;
     cudaStream_t cs = nullptr;
@@ -720,22 +830,26 @@ static int build_graph_pdl(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
     int rc = ce == cudaSuccess ? run_passes(pl, nullptr, nullptr, cs, 0, 4, nullptr, ln) : POISSON_ECUDA;
     cudaGraph_t graph = nullptr;
     if (ce == cudaSuccess) ce = cudaStreamEndCapture(cs, &graph);
+    g.prm_f1 = pass_params(pl, POISSON_PASS_F1, nullptr, nullptr, ln);   // as captured (PDL launch order of the prologue)
+    g.prm_i1 = pass_params(pl, POISSON_PASS_I1, nullptr, nullptr, ln);
     pl->use_pdl = saved;
     cudaStreamDestroy(cs);
     if (rc != POISSON_OK || ce != cudaSuccess || !graph) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return POISSON_ECUDA; }
     g.graph = graph;
-    cudaGraphNode_t nodes[16]; size_t nn = 16;
-    PF_CUDA(cudaGraphGetNodes(graph, nodes, &nn));
+    size_t nn = 0;
+    PF_CUDA(cudaGraphGetNodes(graph, nullptr, &nn));
+    std::vector<cudaGraphNode_t> nodes(nn);
+    PF_CUDA(cudaGraphGetNodes(graph, nodes.data(), &nn));
     int found = 0;
     for (size_t i = 0; i < nn; ++i) {
         cudaGraphNodeType ty;
         if (cudaGraphNodeGetType(nodes[i], &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
         cudaKernelNodeParams kp{};
         PF_CUDA(cudaGraphKernelNodeGetParams(nodes[i], &kp));
-        for (int q = 0; q < 5; ++q) if (kp.func == pl->k[q]->func) { g.node[q] = nodes[i]; ++found; }
+        if (kp.func == pl->k[POISSON_PASS_F1]->func) { g.node_f1 = nodes[i]; ++found; }
+        if (kp.func == pl->k[POISSON_PASS_I1]->func) { g.node_i1 = nodes[i]; ++found; }
     }
-    if (found != 5) { cudaGraphDestroy(g.graph); g.graph = nullptr; g_last_error = "captured graph does not hold the five pass kernels"; return POISSON_ECUDA; }
-    for (int q = 0; q < 5; ++q) g.prm[q] = pass_params(pl, q, nullptr, nullptr, ln);
+    if (found != 2) { cudaGraphDestroy(g.graph); g.graph = nullptr; g_last_error = "captured graph does not hold the F1 / I1 kernels exactly once"; return POISSON_ECUDA; }
     PF_CUDA(cudaGraphInstantiate(&g.exec, g.graph, 0));
     g.rho = nullptr; g.V = nullptr;
     return POISSON_OK;
@@ -746,14 +860,15 @@ static int run_graph(poisson_plan *pl, GraphSolve &g, const void *rho, void *V, 
         const bool stale = q == 0 ? g.rho != rho : g.V != V;
         if (!stale) continue;
         const KernelEntry *e = pl->k[q];
-        if (q == 0) g.prm[0].in = rho; else g.prm[4].out = V;
-        void *args[] = {&g.prm[q]};
+        PassParams &prm = q == 0 ? g.prm_f1 : g.prm_i1;
+        if (q == 0) prm.in = rho; else prm.out = V;
+        void *args[] = {&prm};
         cudaKernelNodeParams kp{};
         kp.func = const_cast<void *>(e->func);
         kp.gridDim = dim3(pl->grid[q]); kp.blockDim = dim3(e->NT);
         kp.sharedMemBytes = (unsigned)e->smem_bytes;
         kp.kernelParams = args; kp.extra = nullptr;
-        PF_CUDA(cudaGraphExecKernelNodeSetParams(g.exec, g.node[q], &kp));   // launch attributes (PDL edges) stay as built
+        PF_CUDA(cudaGraphExecKernelNodeSetParams(g.exec, q == 0 ? g.node_f1 : g.node_i1, &kp));   // launch attributes (PDL edges) stay as built
     }
     g.rho = rho; g.V = V;
     PF_CUDA(cudaGraphLaunch(g.exec, st));
@@ -879,12 +994,13 @@ int poisson_solve_profiled(poisson_plan *pl, const void *rho_dev, void *V_dev, v
     if (pl->prof_count >= kMaxProfiled) return POISSON_ENOMEM;
     if (!pl->prof_events) pl->prof_events = new (std::nothrow) std::vector<cudaEvent_t>();
     if (!pl->prof_events) return POISSON_ENOMEM;
-    while ((int)pl->prof_events->size() < 6 * (pl->prof_count + 1)) {
+    const int per = launches_per_solve(pl) + 1;
+    while ((int)pl->prof_events->size() < per * (pl->prof_count + 1)) {
         cudaEvent_t e;
         PF_CUDA(cudaEventCreate(&e));
         pl->prof_events->push_back(e);
     }
-    cudaEvent_t *ev = pl->prof_events->data() + 6 * pl->prof_count;
+    cudaEvent_t *ev = pl->prof_events->data() + per * pl->prof_count;
     const int rc = run_passes(pl, rho_dev, V_dev, reinterpret_cast<cudaStream_t>(stream), 0, 4, ev);
     if (rc == POISSON_OK) pl->prof_count++;
     return rc;
@@ -894,12 +1010,14 @@ int poisson_profile_read(poisson_plan *pl, double ms_sum[5], int *n_solves) {
     if (!pl || !ms_sum || !n_solves) return POISSON_EINVAL;
     for (int q = 0; q < 5; ++q) ms_sum[q] = 0.0;
     *n_solves = pl->prof_count;
+    const int nl = launches_per_solve(pl), per = nl + 1;
     for (int i = 0; i < pl->prof_count; ++i) {
-        cudaEvent_t *ev = pl->prof_events->data() + 6 * i;
-        PF_CUDA(cudaEventSynchronize(ev[5]));
-        for (int q = 0; q < 5; ++q) {
+        cudaEvent_t *ev = pl->prof_events->data() + per * i;
+        PF_CUDA(cudaEventSynchronize(ev[nl]));
+        for (int item = 0; item < nl; ++item) {   // launch order: F1 | (F2, F3, I2) per chunk | I1
+            const int q = item == 0 ? POISSON_PASS_F1 : (item == nl - 1 ? POISSON_PASS_I1 : POISSON_PASS_F2 + (item - 1) % 3);
             float ms = 0.f;
-            PF_CUDA(cudaEventElapsedTime(&ms, ev[q], ev[q + 1]));
+            PF_CUDA(cudaEventElapsedTime(&ms, ev[item], ev[item + 1]));
             ms_sum[q] += (double)ms;
         }
     }
@@ -912,11 +1030,13 @@ int poisson_debug_run_passes(poisson_plan *pl, const void *rho_dev, void *V_dev,
     if (first == 0 && !rho_dev) return POISSON_EINVAL;
     if (last == 4 && !V_dev) return POISSON_EINVAL;
     if (first <= 2 && last >= 2 && !pl->kernel_set) return POISSON_ENOKERNEL;
+    if (pl->n_chunks > 1 && !(first == 0 && last == 4)) return POISSON_EUNSUPPORTED;   // A2 holds one chunk at a time
     return run_passes(pl, rho_dev, V_dev, reinterpret_cast<cudaStream_t>(stream), first, last);
 }
 
 int poisson_debug_workspace(const poisson_plan *pl, int which, void **ptr, long long dims[3]) {
     if (!pl || !ptr || !dims || (which != 0 && which != 1)) return POISSON_EINVAL;
+    if (which == 1 && pl->n_chunks > 1) return POISSON_EUNSUPPORTED;   // chunked plan: A2 is never whole in memory
     const long long *ext = which == 0 ? pl->d.ext1 : pl->d.ext2;
     *ptr = which == 0 ? pl->a1 : pl->a2;
     dims[0] = ext[2]; dims[1] = ext[1]; dims[2] = ext[0];
@@ -938,7 +1058,7 @@ static int ensure_lanes(poisson_plan *pl, int want, bool staging) {
         if (first) { ln.a1 = pl->a1; ln.a2 = pl->a2; }
         else {
             ce = cudaMalloc(&ln.a1, (size_t)pl->d.a1_elems * cplx);
-            if (ce == cudaSuccess) ce = cudaMalloc(&ln.a2, (size_t)pl->d.a2_elems * cplx);
+            if (ce == cudaSuccess) ce = cudaMalloc(&ln.a2, (size_t)pl->a2_alloc_elems * cplx);
         }
         if (ce == cudaSuccess) ce = cudaStreamCreateWithFlags(&ln.st, cudaStreamNonBlocking);
         if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&ln.done, cudaEventDisableTiming);
@@ -949,7 +1069,7 @@ static int ensure_lanes(poisson_plan *pl, int want, bool staging) {
             cudaGetLastError();
             return ce == cudaErrorMemoryAllocation ? POISSON_ENOMEM : cuda_fail(ce, "batch lane allocation");
         }
-        if (ln.owns_ws) pl->workspace_bytes += (size_t)(pl->d.a1_elems + pl->d.a2_elems) * cplx;
+        if (ln.owns_ws) pl->workspace_bytes += (size_t)(pl->d.a1_elems + pl->a2_alloc_elems) * cplx;
         pl->lanes->push_back(ln);
     }
     if (staging)

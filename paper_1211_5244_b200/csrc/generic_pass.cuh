@@ -127,7 +127,8 @@ __global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams p
         cx<T> *o = (r == b0) ? b1 : b0;
         if constexpr (KIND == KIND_F3) {            // V^F = K^F rho^F (Eq. 3), then straight back
             const bool lanes_p = prm.gen_lanes_p != 0;
-            const long long kbase = lanes_p ? (long long)g * S * prm.n_p + p0 : ((long long)g * prm.n_p + p0) * S;
+            const long long gk = g + prm.k_g0;   // plane chunks: position in the whole grid
+            const long long kbase = lanes_p ? gk * S * prm.n_p + p0 : (gk * prm.n_p + p0) * S;
             for (int idx = tid; idx < S * P; idx += GEN_NT) {
                 int k, p;
                 if (lanes_p) { p = idx % P; k = idx / P; } else { k = idx % S; p = idx / S; }

@@ -106,6 +106,8 @@ struct PassParams {
     int n_p;           // pencils per g
     int tiles_per_g;   // ceil(n_p / P)
     int n_tiles;       // n_g * tiles_per_g
+    int late_tw;       // 1: build the twiddle tables after the first tile's loads have been issued (else before: the PDL order)
+    int k_g0;          // F3 of a plane chunk: first plane of the chunk (K^F is indexed by the plane's position in the whole grid)
     int prefetch;      // bit 0: prefetch the next tile's inputs into L2 (unstaged tile loops); bit 1: F3 prefetches its K^F lines
     // several densities per launch (small grids, poisson_solve_batch): tile = bi * n_tiles1 + tile of density bi
     int n_tiles1;      // tiles of ONE density (n_tiles = nb * n_tiles1; nb = 1 for a single solve)
@@ -466,7 +468,8 @@ PF_HD void stage_issue(cx<typename G::T> *stage, const cx<typename G::T> *src, l
 
 // ------------------------------------------------------------------ tiles
 // Persistent tile loop.  issue(tile): start the asynchronous copies of a tile (staged mode only);
-// after_first(): hook after the very first issue; fetch(buf, tile): tile -> registers (from the stage,
+// after_first(): hook run once, right after the first tile's loads / copies have been issued (the twiddle tables are built
+// there, under the latency of those loads); fetch(buf, tile): tile -> registers (from the stage,
 // or straight from global memory when not staged); process(buf, tile): transform and store.
 // WAITN = copy groups that may still be pending when a tile's inputs are needed.
 struct NoPrefetch { PF_HD void operator()(int) const {} };
@@ -492,6 +495,7 @@ PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_
         int tile = bid;
         Buf cur;
         if (tile < n_tiles) fetch(cur, tile);
+        after_first();
         for (; tile < n_tiles; tile += nb) {
             Buf nxt;
             const bool more = tile + nb < n_tiles;
@@ -500,22 +504,26 @@ PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_
             if (more) cur = nxt;
         }
     } else {
+        bool first = true;
         for (int tile = bid; tile < n_tiles; tile += nb) {
             Buf cur;
             fetch(cur, tile);
+            if (first) { after_first(); first = false; }           // the first tile's loads are in flight: run the hook under them
             if (tile + nb < n_tiles) prefetch_next(tile + nb);   // unstaged: at least start the next tile DRAM -> L2
             process(cur, tile);
         }
+        if (first) after_first();
     }
 }
 
 // Exchange buffer as the stage: process(buf, tile, after_read) calls after_read() once the thread has read its last
 // exchange value of the tile; a barrier later the buffer is idle and takes the next tile's copies.
-template <class G, class Buf, class Issue, class Fetch, class Process>
-PF_HD void tile_loop_x(int bid, int nb, int n_tiles, Issue &&issue, Fetch &&fetch, Process &&process) {
+template <class G, class Buf, class Issue, class After, class Fetch, class Process>
+PF_HD void tile_loop_x(int bid, int nb, int n_tiles, Issue &&issue, After &&after_first, Fetch &&fetch, Process &&process) {
     int tile = bid;
     if (tile < n_tiles) issue(tile);
     cp_async_commit();
+    after_first();
     for (; tile < n_tiles; tile += nb) {
         Buf cur;
         cp_async_wait<0>();
@@ -767,8 +775,10 @@ PF_HD void process_i1(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c
     const unsigned long long pol = (St::ON || St::XON) ? evict_first_policy() : 0ull;                              \
     (void)stage; (void)pol; (void)t; (void)p;                                               \
     pdl_launch_dependents();                                                                          \
-    c.tw.template init<NEED_A, NEED_B>(reinterpret_cast<const cx<T> *>(prm.tw), smem_c + G::NBUF * G::XELEMS, tid, c.t); \
-    pdl_wait_prior_grid();
+    auto init_tw = [&] { c.tw.template init<NEED_A, NEED_B>(reinterpret_cast<const cx<T> *>(prm.tw), smem_c + G::NBUF * G::XELEMS, tid, c.t); }; \
+    if (!prm.late_tw) init_tw();           /* tables first, then wait for the previous pass (the PDL order) */ \
+    pdl_wait_prior_grid();                                                                            \
+    auto tw_hook = [&] { if (prm.late_tw) init_tw(); };   /* or: under the latency of the first tile's loads */
 
 template <class G, bool PRUNED>
 PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
@@ -779,7 +789,7 @@ PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             PF_TILE_COORDS
             stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
         },
-        [] {},
+        tw_hook,
         [&](Buf &b, int tile) {
             if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
             else fetch_fwd<G, PRUNED, true>(b, prm, tile, c);
@@ -810,6 +820,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
                     prefetch_tile_l2<G, St>(pass_in<T>(prm, bi2) + g2 * prm.gs_in + q0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - q0, tid);
                 }
             },
+            tw_hook,
             [&](Buf &b, int tile) {
                 PF_TILE_COORDS
                 static_for<G::CB>([&](auto ic) {
@@ -832,7 +843,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             PF_TILE_COORDS
             stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
         },
-        [] {},
+        tw_hook,
         [&](Buf &b, int tile) {
             if constexpr (St::ON) {
                 PF_TILE_COORDS
@@ -870,7 +881,7 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     typename KV::V *kstage = reinterpret_cast<typename KV::V *>(stage + St::IN_ELEMS);
     (void)kstage;
     auto issue_k = [&](int tile) {
-        const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1) * NKV * G::NT + tid;
+        const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1 + prm.k_g0 * prm.tiles_per_g) * NKV * G::NT + tid;
         static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; cp_async_vec16(kstage + q * G::NT + tid, kp + (size_t)q * G::NT, pol); });
     };
     tile_loop<G, Buf, St::ON, (St::KON ? 1 : 0)>(bid, nb, prm.n_tiles,
@@ -880,16 +891,17 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&] {
             if constexpr (St::KON) { if (bid < prm.n_tiles) issue_k(bid); cp_async_commit(); }
+            tw_hook();
         },
         [&](Buf &b, int tile) {
             if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
             else fetch_fwd<G, PRUNED, false>(b, prm, tile, c);
             if (G::KLATE && !St::KON && KPREF && (prm.prefetch & 2)) {   // start this tile's K^F on its way DRAM -> L2 now
-                const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1) * NKV * G::NT + tid;
+                const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1 + prm.k_g0 * prm.tiles_per_g) * NKV * G::NT + tid;
                 static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; prefetch_l2(kp + (size_t)q * G::NT); });
             }
             if constexpr (K_EARLY) {
-                const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1) * NKV * G::NT + tid;
+                const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1 + prm.k_g0 * prm.tiles_per_g) * NKV * G::NT + tid;
                 static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), b.k + q * KV::N); });
             }
         },
@@ -902,7 +914,7 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
                     if (tile + nb < prm.n_tiles) issue_k(tile + nb);
                     cp_async_commit();
                 } else if constexpr (G::KLATE) {
-                    kmul_global<G>(v, prm.kint, tile % prm.n_tiles1, tid);
+                    kmul_global<G>(v, prm.kint, tile % prm.n_tiles1 + prm.k_g0 * prm.tiles_per_g, tid);
                 } else {
                     static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], b.k[r]); });
                 }
@@ -919,7 +931,7 @@ PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             PF_TILE_COORDS
             stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
         },
-        [] {},
+        tw_hook,
         [&](Buf &b, int tile) {
             if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
             else fetch_fwd<G, PRUNED, true>(b, prm, tile, c);
@@ -944,6 +956,7 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
                 PF_TILE_COORDS
                 stage_issue<G, St, true, true>(smem_c, pass_in<T>(prm, bi) + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);
             },
+            tw_hook,
             [&](Buf &b, int tile) {
                 PF_TILE_COORDS
                 fetch_i1_with<G>(b, t, valid, [&](int kk, cx<T> &a, cx<T> &bb) { a = smem_c[St::xidx(2 * p, kk)]; bb = smem_c[St::xidx(2 * p + 1, kk)]; });
@@ -959,7 +972,7 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             PF_TILE_COORDS   // stage rows: kk = 0..S/2, columns: the 2 P complex pencils of the P pairs
             stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);
         },
-        [] {},
+        tw_hook,
         [&](Buf &b, int tile) {
             if constexpr (St::ON) {
                 PF_TILE_COORDS

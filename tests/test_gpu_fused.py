@@ -143,3 +143,56 @@ def test_graph_launch_mode_matches_five_launches_bitwise(pk, monkeypatch, pdl):
         assert torch.equal(outs[0], refs[2])
     finally:
         plan.close()
+
+
+@pytest.mark.parametrize("n,bc,prec", [((24, 16, 32), (0, 0, 0), "fp64"), ((32, 24, 16), (1, 1, 0), "fp64"), ((16, 40, 12), (0, 0, 1), "fp32"),
+                                       ((15, 9, 14), (0, 1, 0), "fp64")])
+@pytest.mark.parametrize("mode", ["five", "graph", "graph_pdl"])
+def test_plane_chunked_middle_passes(pk, monkeypatch, n, bc, prec, mode):
+    """Large grids run F2 -> F3 -> I2 chunk by chunk of k_a planes through an A2 buffer that holds one chunk (csrc/api.cu:
+    for_each_launch).  Forced here on small grids (POISSON_CHUNK = planes per chunk, ragged last chunk): the result equals the
+    unchunked plan's bitwise (same kernels, same arithmetic per tile) and matches the oracle, in every launch mode and through
+    the batch lanes."""
+    import torch
+    dt = np.float64 if prec == "fp64" else np.float32
+    rng = np.random.default_rng(606 + sum(n))
+    s = gen.padded_shape(n, bc)
+    Kf = oracle.kernel_spectrum(_even_kernel(rng, s)).astype(dt)
+    rhos_np = [rng.standard_normal((n[2], n[1], n[0])).astype(dt) for _ in range(3)]
+    monkeypatch.setenv("POISSON_TUNE", "0")
+    if mode != "five":
+        monkeypatch.setenv("POISSON_GRAPH", "1")
+    if mode == "graph_pdl":
+        monkeypatch.setenv("POISSON_PDL", "1")
+    prec_id = pk.FP64 if prec == "fp64" else pk.FP32
+    ref_plan = pk.PoissonPlan(n, bc, 0.3, prec_id)
+    ref_plan.set_kernel(torch.from_numpy(Kf).cuda())
+    rhos = [torch.from_numpy(r).cuda() for r in rhos_np]
+    refs = [ref_plan.solve(r).clone() for r in rhos]
+    assert ref_plan.launches_per_solve() == 5
+    ref_plan.close()
+    monkeypatch.setenv("POISSON_CHUNK", "3")
+    plan = pk.PoissonPlan(n, bc, 0.3, prec_id)
+    try:
+        planes = plan.info.half_len
+        assert plan.launches_per_solve() == 2 + 3 * ((planes + 2) // 3)
+        assert plan.launch_mode()[0] == mode
+        plan.set_kernel(torch.from_numpy(Kf).cuda())
+        for rep in range(2):
+            for r, ref in zip(rhos, refs):
+                assert torch.equal(plan.solve(r), ref)
+        err = rel_l2(refs[0].cpu().numpy().astype(np.float64), oracle.solve(rhos_np[0].astype(np.float64), Kf.astype(np.float64), bc))
+        assert err <= (1e-12 if prec == "fp64" else 1e-5)
+        monkeypatch.setenv("POISSON_WIDE", "0")
+        for v, ref in zip(plan.solve_batch(rhos), refs):          # batch lanes carry their own chunk-sized A2
+            torch.cuda.synchronize()
+            assert torch.equal(v, ref)
+        for i in range(4):
+            plan.solve_profiled(rhos[0], refs[0].clone())
+        ms, cnt = plan.profile_read()
+        assert cnt == 4 and all(m > 0 for m in ms)
+        with pytest.raises(pk.PoissonError) as ei:
+            plan.debug_workspace(1)
+        assert ei.value.status == 2                                # A2 is never whole in memory on a chunked plan
+    finally:
+        plan.close()

@@ -68,13 +68,35 @@ static const void *generic_func(int kind) {
     }
 }
 
-// Radices of S for the Stockham passes: 4s first (fewest passes over the tile), then the prime factors ascending.
+// Radices of S for the Stockham passes: the fewest passes over the tile with radices the kernel holds in registers
+// ({2,3,4,5,6,8,10,12,16} via fft_core.cuh, 7 / 11 / 13 as written-out sums); larger radices first (their twiddle-free last
+// stage is the cheapest); any other prime factor runs the one-output-per-thread fallback.
 static int generic_factors(int S, int fac[16]) {
-    int n = 0;
-    while (S % 4 == 0 && n < 16) { fac[n++] = 4; S /= 4; }
-    for (int p = 2; S > 1 && n < 16; ++p)
-        while (S % p == 0 && n < 16) { fac[n++] = p; S /= p; }
-    return S == 1 ? n : -1;
+    static const int allowed[] = {16, 13, 12, 11, 10, 8, 7, 6, 5, 4, 3, 2};
+    int n = 0, rest = S;
+    // strip the prime factors the register butterflies do not cover (17 and up)
+    int big[16], nbig = 0;
+    {
+        int r = rest;
+        for (int p : {2, 3, 5, 7, 11, 13}) while (r % p == 0) r /= p;
+        for (int p = 17; r > 1; p += 2) while (r % p == 0) { if (nbig == 16) return -1; big[nbig++] = p; r /= p; rest /= p; }
+    }
+    // fewest stages for the smooth part: depth-first over the allowed radices, non-increasing order
+    int best[16], nbest = 99, cur[16];
+    struct Rec {
+        static void go(int r, int start, int depth, int *cur, int *best, int &nbest, const int *allowed) {
+            if (r == 1) { if (depth < nbest) { nbest = depth; for (int i = 0; i < depth; ++i) best[i] = cur[i]; } return; }
+            if (depth + 1 >= nbest || depth >= 15) return;
+            for (int i = start; i < 12; ++i)
+                if (r % allowed[i] == 0) { cur[depth] = allowed[i]; go(r / allowed[i], i, depth + 1, cur, best, nbest, allowed); }
+        }
+    };
+    Rec::go(rest, 0, 0, cur, best, nbest, allowed);
+    if (nbest == 99) return rest == 1 ? 0 : -1;
+    if (nbest + nbig > 16) return -1;
+    for (int i = 0; i < nbig; ++i) fac[n++] = big[i];         // the slow radices first (their pass has w_n^{jk} anyway)
+    for (int i = nbest - 1; i >= 0; --i) fac[n++] = best[i];   // then ascending: the largest radix is the twiddle-free last stage
+    return n;
 }
 
 // false: the length does not fit the any-length kernel (shared memory, or more than 16 radices)
@@ -89,6 +111,8 @@ static bool make_generic_entry(KernelEntry &e, int kind, int S, int pruned, int 
     int P = (int)(128 / cplx);
     while (P > 1 && gen_smem_bytes(S, P, cplx) > (size_t)227 * 1024) P /= 2;
     if (gen_smem_bytes(S, P, cplx) > (size_t)227 * 1024) return false;
+    // two resident CTAs (16 warps) per SM matter more than whole 128-byte rows: halve the tile once if that makes room
+    if (P * cplx >= 128 && gen_smem_bytes(S, P, cplx) > (size_t)112 * 1024 && gen_smem_bytes(S, P / 2, cplx) <= (size_t)112 * 1024) P /= 2;
     // small transforms: enough pencils per tile to give every thread work (S * P >= 2 * NT), still whole rows
     while (S * P < 2 * GEN_NT && P < 64 && gen_smem_bytes(S, 2 * P, cplx) <= (size_t)48 * 1024) P *= 2;
     e.P = P;

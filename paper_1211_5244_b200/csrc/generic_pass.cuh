@@ -11,9 +11,11 @@
 //         y[q + s (R j + k)] = w_n^{j k}  sum_{r < R}  x[q + s (j + m r)]  w_R^{r k}      j < m, q < s, k < R
 //         swap(x, y);  n = m;  s = s R
 //
-// (natural order in, natural order out, no bit reversal).  A radix-R butterfly is the R-term sum written out, so a
-// prime factor p costs O(p) per point: a prime length degenerates to the O(S^2) DFT (where a Bluestein chirp-z would be
-// the asymptotically better choice), and every composite length is O(S sum R_i).  Twiddles come from the plan's
+// (natural order in, natural order out, no bit reversal).  The radices are chosen by the plan from {16, 12, 10, 8, 6, 5, 4,
+// 3, 2} (the in-register DFTs of fft_core.cuh: a thread holds a whole butterfly), 7 / 11 / 13 (the R-term sums written
+// out in registers) and, for any other prime factor p, a fallback that forms one output per thread per step -- O(p) per
+// point, so a prime length degenerates to the O(S^2) DFT (where a Bluestein chirp-z would be the asymptotically better
+// choice) and every smooth length is O(S log S) with as few passes over the tile as its factors allow.  Twiddles come from the plan's
 // table exp(-2 pi i m / S) in shared memory.  The paper's spread / compactification are the zero fill of
 // the tile's upper half on load and the store of the lower half only; R2C / C2R pack two real pencils
 // adjacent in x into one complex transform exactly as passes.cuh does, with an unpaired last pencil when N_x is odd.
@@ -31,41 +33,122 @@ constexpr int GEN_MAX_S = 4096;      // longest generic transform (three S-point
 PF_CE int gen_pitch(int P) { return (P % 2 == 0) ? P + 1 : P; }
 PF_CE size_t gen_smem_bytes(int S, int P, size_t cplx_bytes) { return ((size_t)2 * S * gen_pitch(P) + S) * cplx_bytes; }
 
+// floor(n / d) for the index ranges of a tile (n d < 2^32) without an integer division: n * ceil(2^32 / d) >> 32
+struct GenDiv {
+    unsigned d, magic;
+    PF_HD explicit GenDiv(int d_) : d((unsigned)d_), magic(d_ > 1 ? 0xFFFFFFFFu / (unsigned)d_ + 1u : 0u) {}
+    PF_HD int div(int n) const { return d > 1 ? (int)__umulhi((unsigned)n, magic) : n; }
+};
+
 template <typename T> PF_HD cx<T> gen_w(const cx<T> *tw, int i, bool inv) { const cx<T> w = tw[i]; return inv ? conj(w) : w; }
 
-// One Stockham pass sequence over the tile in x (result returned in the buffer the function returns).
+// Radix-R butterfly for a prime R without a literal-twiddle DFT in fft_core.cuh (7, 11, 13): the R-term sums written out
+// with the factors w_R^{rk} = w_S^{(S/R)(rk mod R)} read from the shared-memory table.
+template <typename T, int R, bool INV>
+PF_HD void gen_dft_prime(cx<T> *a, const cx<T> *tw, int wr) {
+    cx<T> o[R];
+    static_for<R>([&](auto kc) {
+        constexpr int k = decltype(kc)::value;
+        cx<T> acc = a[0];
+        static_for<R - 1>([&](auto rc) {
+            constexpr int r = decltype(rc)::value + 1;
+            const cx<T> w = gen_w(tw, wr * ((r * k) % R), INV);
+            acc = k == 0 ? acc + a[r] : acc + a[r] * w;
+        });
+        o[k] = acc;
+    });
+    static_for<R>([&](auto kc) { constexpr int k = decltype(kc)::value; a[k] = o[k]; });
+}
+
+// One Stockham stage of compile-time radix R over the whole tile: every thread takes butterflies (j, q, pencil p), holds
+// the R inputs in registers, transforms them with the in-register DFT of fft_core.cuh (or the prime butterfly above) and
+// stores the R outputs multiplied by w_n^{jk}.  Not inlined: one copy per (precision, radix, direction) serves all five kernels.
+template <typename T, int R, bool INV>
+__device__ __noinline__ void gen_stage(const cx<T> *x, cx<T> *y, const cx<T> *tw, int S, int P, int n, int s, int tid) {
+    const int PP = gen_pitch(P), m = n / R, nbf = S / R, wn = S / n, istride = s * m * PP, ostride = s * PP;
+    const int lgP = 31 - __clz(P);                   // P is a power of two
+    const GenDiv by_s(s);
+    for (int idx = tid; idx < nbf * P; idx += GEN_NT) {
+        const int p = idx & (P - 1), b = idx >> lgP, j = by_s.div(b), q = b - j * s;
+        cx<T> a[R];
+        const cx<T> *src = x + (q + s * j) * PP + p;
+        static_for<R>([&](auto rc) { constexpr int r = decltype(rc)::value; a[r] = src[r * istride]; });
+        if constexpr (R == 7 || R == 11 || R == 13) gen_dft_prime<T, R, INV>(a, tw, S / R);
+        else dft<T, R, INV>(a);
+        cx<T> *dst = y + (q + s * R * j) * PP + p;
+        dst[0] = a[0];
+        if (m == 1) {            // last stage: every w_n^{jk} is 1
+            static_for<R - 1>([&](auto kc) { constexpr int k = decltype(kc)::value + 1; dst[k * ostride] = a[k]; });
+        } else {
+            static_for<R - 1>([&](auto kc) {
+                constexpr int k = decltype(kc)::value + 1;
+                dst[k * ostride] = a[k] * gen_w(tw, wn * j * k, INV);        // j k < n, so wn j k < S
+            });
+        }
+    }
+}
+
+// Any other radix (primes from 17 up): one output per thread per step, the R-term sum read from shared memory.
+template <typename T>
+__device__ __noinline__ void gen_stage_any(const cx<T> *x, cx<T> *y, const cx<T> *tw, int S, int P, int n, int s, int R, bool inv, int tid) {
+    const int PP = gen_pitch(P), m = n / R, wr = S / R, wn = S / n;
+    const int lgP = 31 - __clz(P);
+    for (int idx = tid; idx < S * P; idx += GEN_NT) {
+        const int p = idx & (P - 1), e = idx >> lgP;   // output element e = q + s (R j + k)
+        const int q = e % s, t = e / s, k = t % R, j = t / R;
+        const cx<T> *src = x + (q + s * j) * PP + p;
+        const int stride = s * m * PP;
+        T ar = 0, ai = 0;
+        int wi = 0;
+        const int step = (int)(((long long)wr * k) % S);
+        for (int r = 0; r < R; ++r) {
+            const cx<T> a = src[r * stride], w = gen_w(tw, wi, inv);
+            ar += a.re * w.re - a.im * w.im;
+            ai += a.re * w.im + a.im * w.re;
+            wi += step; if (wi >= S) wi -= S;
+        }
+        const cx<T> w = gen_w(tw, wn * j * k, inv);     // j k < n, so wn j k < S
+        y[e * PP + p] = mk<T>(ar * w.re - ai * w.im, ar * w.im + ai * w.re);
+    }
+}
+
+template <typename T, bool INV>
+PF_HD void gen_stage_dispatch(const cx<T> *x, cx<T> *y, const cx<T> *tw, int S, int P, int n, int s, int R, int tid) {
+    switch (R) {
+        case 2: gen_stage<T, 2, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 3: gen_stage<T, 3, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 4: gen_stage<T, 4, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 5: gen_stage<T, 5, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 6: gen_stage<T, 6, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 7: gen_stage<T, 7, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 8: gen_stage<T, 8, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 10: gen_stage<T, 10, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 11: gen_stage<T, 11, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 12: gen_stage<T, 12, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 13: gen_stage<T, 13, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 16: gen_stage<T, 16, INV>(x, y, tw, S, P, n, s, tid); break;
+        default: gen_stage_any<T>(x, y, tw, S, P, n, s, R, INV, tid); break;
+    }
+}
+
+// The Stockham pass sequence over the tile in x (the function returns the buffer that holds the result).
 template <typename T>
 PF_HD cx<T> *gen_fft(cx<T> *x, cx<T> *y, const cx<T> *tw, const PassParams &prm, bool inv, int tid) {
-    const int S = prm.gen_S, P = prm.gen_P, PP = gen_pitch(P);
+    const int S = prm.gen_S, P = prm.gen_P;
     int n = S, s = 1;
     for (int f = 0; f < prm.gen_nfac; ++f) {
-        const int R = prm.gen_fac[f], m = n / R, wr = S / R, wn = S / n;
-        for (int idx = tid; idx < S * P; idx += GEN_NT) {
-            const int p = idx % P, e = idx / P;            // output element e = q + s (R j + k)
-            const int q = e % s, t = e / s, k = t % R, j = t / R;
-            const cx<T> *src = x + (q + s * j) * PP + p;
-            const int stride = s * m * PP;
-            T ar = 0, ai = 0;
-            int wi = 0;
-            const int step = (int)(((long long)wr * k) % S);
-            for (int r = 0; r < R; ++r) {
-                const cx<T> a = src[r * stride], w = gen_w(tw, wi, inv);
-                ar += a.re * w.re - a.im * w.im;
-                ai += a.re * w.im + a.im * w.re;
-                wi += step; if (wi >= S) wi -= S;
-            }
-            const cx<T> w = gen_w(tw, wn * j * k, inv);     // j k < n, so wn j k < S
-            y[e * PP + p] = mk<T>(ar * w.re - ai * w.im, ar * w.im + ai * w.re);
-        }
+        const int R = prm.gen_fac[f];
+        if (inv) gen_stage_dispatch<T, true>(x, y, tw, S, P, n, s, R, tid);
+        else gen_stage_dispatch<T, false>(x, y, tw, S, P, n, s, R, tid);
         __syncthreads();
         cx<T> *tmp = x; x = y; y = tmp;
-        n = m; s *= R;
+        n /= R; s *= R;
     }
     return x;
 }
 
 template <typename T, int KIND>
-__global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams prm) {
+__global__ void __launch_bounds__(GEN_NT, 2) generic_pass_kernel(const PassParams prm) {
     extern __shared__ __align__(16) unsigned char pf_smem[];
     const int S = prm.gen_S, P = prm.gen_P, PP = gen_pitch(P), tid = threadIdx.x;
     const int H = S / 2 + 1;
@@ -76,6 +159,8 @@ __global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams p
     pdl_wait_prior_grid();
     __syncthreads();
     const int n_half = pruned ? S / 2 : S;      // points that exist on the un-padded side of this pass
+    const int lgP = 31 - __clz(P);              // P is a power of two
+    const GenDiv by_S(S), by_half(n_half);
 
     for (int tile = blockIdx.x; tile < prm.n_tiles; tile += gridDim.x) {
         const int bi = tile / prm.n_tiles1, tl = tile - bi * prm.n_tiles1;
@@ -87,7 +172,7 @@ __global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams p
         if constexpr (KIND == KIND_F1) {            // two real pencils adjacent in x -> one complex pencil
             const T *src = (prm.use_list == 1 ? reinterpret_cast<const T *>(prm.blist[bi]) : reinterpret_cast<const T *>(prm.in) + bi * prm.bs_in) + g * prm.gs_in;
             for (int idx = tid; idx < S * P; idx += GEN_NT) {
-                const int q = idx % P, n = idx / P;
+                const int q = idx & (P - 1), n = idx >> lgP;
                 cx<T> v = mk<T>((T)0, (T)0);
                 if (n < n_half && q < ncols) {
                     const long long xr = 2LL * (p0 + q);
@@ -99,7 +184,7 @@ __global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams p
         } else if constexpr (KIND == KIND_I1) {     // Z_k = A_k + i B_k,  Z_{S-k} = conj A_k + i conj B_k
             const cx<T> *src = pass_in<T>(prm, bi) + g * prm.gs_in;
             for (int idx = tid; idx < H * P; idx += GEN_NT) {
-                const int q = idx % P, k = idx / P;
+                const int q = idx & (P - 1), k = idx >> lgP;
                 cx<T> a = mk<T>((T)0, (T)0), b = a;
                 if (q < ncols) {
                     const long long xr = 2LL * (p0 + q);
@@ -115,7 +200,7 @@ __global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams p
             const bool lanes_p = prm.gen_lanes_p != 0;
             for (int idx = tid; idx < S * P; idx += GEN_NT) {
                 int n, p;
-                if (lanes_p) { p = idx % P; n = idx / P; } else { n = idx % S; p = idx / S; }
+                if (lanes_p) { p = idx & (P - 1); n = idx >> lgP; } else { p = by_S.div(idx); n = idx - p * S; }
                 x[n * PP + p] = (n < n_in && p < ncols) ? src[n * prm.ns_in + p * prm.ps_in] : mk<T>((T)0, (T)0);
             }
         }
@@ -131,7 +216,7 @@ __global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams p
             const long long kbase = lanes_p ? gk * S * prm.n_p + p0 : (gk * prm.n_p + p0) * S;
             for (int idx = tid; idx < S * P; idx += GEN_NT) {
                 int k, p;
-                if (lanes_p) { p = idx % P; k = idx / P; } else { k = idx % S; p = idx / S; }
+                if (lanes_p) { p = idx & (P - 1); k = idx >> lgP; } else { p = by_S.div(idx); k = idx - p * S; }
                 if (p < ncols) {
                     const long long ki = kbase + (lanes_p ? (long long)k * prm.n_p + p : (long long)p * S + k);
                     const cx<T> v = r[k * PP + p];
@@ -147,7 +232,7 @@ __global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams p
         if constexpr (KIND == KIND_F1) {            // A = (Z_k + conj Z_{S-k}) / 2,  B = -i (Z_k - conj Z_{S-k}) / 2,  k <= S/2
             cx<T> *dst = pass_out<T>(prm, bi) + g * prm.gs_out;
             for (int idx = tid; idx < H * P; idx += GEN_NT) {
-                const int q = idx % P, k = idx / P;
+                const int q = idx & (P - 1), k = idx >> lgP;
                 if (q < ncols) {
                     const cx<T> zk = r[k * PP + q], zp = r[((S - k) % S) * PP + q];
                     const T hf = (T)0.5;
@@ -159,7 +244,7 @@ __global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams p
         } else if constexpr (KIND == KIND_I1) {     // real part -> pencil 2q, imaginary part -> pencil 2q + 1
             T *dst = (prm.use_list == 2 ? reinterpret_cast<T *>(const_cast<void *>(prm.blist[bi])) : reinterpret_cast<T *>(prm.out) + bi * prm.bs_out) + g * prm.gs_out;
             for (int idx = tid; idx < n_half * P; idx += GEN_NT) {
-                const int q = idx % P, n = idx / P;
+                const int q = idx & (P - 1), n = idx >> lgP;
                 if (q < ncols) {
                     const cx<T> v = r[n * PP + q];
                     const long long xr = 2LL * (p0 + q);
@@ -173,7 +258,7 @@ __global__ void __launch_bounds__(GEN_NT) generic_pass_kernel(const PassParams p
             const bool lanes_p = prm.gen_lanes_p != 0;
             for (int idx = tid; idx < n_out * P; idx += GEN_NT) {
                 int n, p;
-                if (lanes_p) { p = idx % P; n = idx / P; } else { n = idx % n_out; p = idx / n_out; }
+                if (lanes_p) { p = idx & (P - 1); n = idx >> lgP; } else { p = (n_out == S ? by_S : by_half).div(idx); n = idx - p * n_out; }
                 if (p < ncols) dst[n * prm.ns_out + p * prm.ps_out] = r[n * PP + p];
             }
         }

@@ -99,24 +99,46 @@ static int generic_factors(int S, int fac[16]) {
     return n;
 }
 
+static int largest_prime_factor(int S) {
+    int best = 1;
+    for (int p = 2; (long long)p * p <= S; ++p) while (S % p == 0) { best = p; S /= p; }
+    return S > 1 ? S : best;
+}
+
+// Bluestein (generic_pass.cuh: gen_transform) for lengths with a prime factor >= 17, up to S = 1024: convolution length
+// M = the smallest of {2^a, 3 2^a, 5 2^a} that is >= 2S - 1.  0: the length runs the Stockham passes directly.
+static int bluestein_length(int S) {
+    if (S > 1024 || largest_prime_factor(S) < 17) return 0;
+    int best = 0;
+    for (int base : {1, 3, 5})
+        for (int m = base; m <= 4096; m *= 2)
+            if (m >= 2 * S - 1) { if (!best || m < best) best = m; break; }
+    return best;
+}
+
 // false: the length does not fit the any-length kernel (shared memory, or more than 16 radices)
 static bool make_generic_entry(KernelEntry &e, int kind, int S, int pruned, int lanes_p, int prec) {
     e = KernelEntry{};
     e.kind = kind; e.S = S; e.pruned = pruned; e.lanes_p = lanes_p; e.prec = prec; e.generic = 1;
     e.nbuf = 2; e.NT = GEN_NT; e.TPP = 0; e.V = 0; e.RA = S; e.RB = 1;
-    e.gen_nfac = generic_factors(S, e.gen_fac);
-    if (e.gen_nfac < 0 || S > GEN_MAX_S) return false;
+    if (S > GEN_MAX_S) return false;
+    const int M = bluestein_length(S);
+    e.gen_blue = M ? 1 : 0;
+    e.gen_L = M ? M : S;
+    const int L = e.gen_L;
+    e.gen_nfac = generic_factors(L, e.gen_fac);
+    if (e.gen_nfac < 0) return false;
     const size_t cplx = prec == POISSON_FP64 ? 16 : 8;
     // widest tile (whole 128-byte rows first) that fits the 227 KB of shared memory a CTA may use
     int P = (int)(128 / cplx);
-    while (P > 1 && gen_smem_bytes(S, P, cplx) > (size_t)227 * 1024) P /= 2;
-    if (gen_smem_bytes(S, P, cplx) > (size_t)227 * 1024) return false;
+    while (P > 1 && gen_smem_bytes(L, P, cplx) > (size_t)227 * 1024) P /= 2;
+    if (gen_smem_bytes(L, P, cplx) > (size_t)227 * 1024) return false;
     // two resident CTAs (16 warps) per SM matter more than whole 128-byte rows: halve the tile once if that makes room
-    if (P * cplx >= 128 && gen_smem_bytes(S, P, cplx) > (size_t)112 * 1024 && gen_smem_bytes(S, P / 2, cplx) <= (size_t)112 * 1024) P /= 2;
-    // small transforms: enough pencils per tile to give every thread work (S * P >= 2 * NT), still whole rows
-    while (S * P < 2 * GEN_NT && P < 64 && gen_smem_bytes(S, 2 * P, cplx) <= (size_t)48 * 1024) P *= 2;
+    if (P * cplx >= 128 && gen_smem_bytes(L, P, cplx) > (size_t)112 * 1024 && gen_smem_bytes(L, P / 2, cplx) <= (size_t)112 * 1024) P /= 2;
+    // small transforms: enough pencils per tile to give every thread work (L * P >= 2 * NT), still whole rows
+    while (L * P < 2 * GEN_NT && P < 64 && gen_smem_bytes(L, 2 * P, cplx) <= (size_t)48 * 1024) P *= 2;
     e.P = P;
-    e.smem_bytes = gen_smem_bytes(S, P, cplx);
+    e.smem_bytes = gen_smem_bytes(L, P, cplx);
     e.func = prec == POISSON_FP64 ? generic_func<double>(kind) : generic_func<float>(kind);
     return true;
 }
@@ -218,7 +240,8 @@ struct poisson_plan {
     void *wide_a1, *wide_a2;   // intermediates of wide_w densities (several small solves per launch), allocated on first use
     int wide_w;
     void *a1, *a2, *kint;
-    void *tw[3];          // per axis id
+    void *tw[3];          // per axis id: exp(-2 pi i m / S) (Bluestein axes: exp(-2 pi i m / M) of the convolution length)
+    void *chirp[3], *bspec[3];   // Bluestein axes only (generic_pass.cuh: gen_transform)
     void *rho_stage, *v_stage;
     const FusedEntry *fused;   // one-launch solve kernel compiled for this combination of axes, or NULL
     bool use_fused;            // launch mode picked for poisson_solve: fused kernel, else 5 launches (with or without PDL)
@@ -256,10 +279,43 @@ static void fill_twiddles(std::vector<unsigned char> &buf, int S, int prec) {
     }
 }
 
+// Bluestein tables of one axis (host, long double): chirp[n] = exp(-i pi n^2 / S), n < S (angle from n^2 mod 2S, exact), and
+// bspec = DFT_M(b) / M of b[0] = 1, b[n] = b[M - n] = conj(chirp[n]) for 0 < n < S, 0 elsewhere (the 1/M of the inner inverse
+// transform folded in).  The DFT is the O(M^2) definition: M <= 2048, a few tens of milliseconds once per plan.
+static void fill_bluestein(std::vector<unsigned char> &chirp, std::vector<unsigned char> &bspec, int S, int M, int prec) {
+    const long double pi = 3.141592653589793238462643383279502884L;
+    std::vector<long double> cr(S), ci(S), br(M, 0.0L), bi(M, 0.0L);
+    for (int n = 0; n < S; ++n) {
+        const long long m = ((long long)n * n) % (2LL * S);
+        const long double ang = pi * (long double)m / (long double)S;
+        cr[n] = cosl(ang); ci[n] = -sinl(ang);
+        br[n] = cr[n]; bi[n] = -ci[n];
+        if (n) { br[M - n] = br[n]; bi[M - n] = bi[n]; }
+    }
+    std::vector<long double> wr(M), wi(M);
+    for (int m = 0; m < M; ++m) { const long double a = 2.0L * pi * (long double)m / (long double)M; wr[m] = cosl(a); wi[m] = -sinl(a); }
+    const size_t el = prec == POISSON_FP64 ? 16 : 8;
+    chirp.resize((size_t)S * el); bspec.resize((size_t)M * el);
+    auto put = [&](std::vector<unsigned char> &buf, int i, long double re, long double im) {
+        if (prec == POISSON_FP64) { double *o = reinterpret_cast<double *>(buf.data()) + 2 * i; o[0] = (double)re; o[1] = (double)im; }
+        else { float *o = reinterpret_cast<float *>(buf.data()) + 2 * i; o[0] = (float)re; o[1] = (float)im; }
+    };
+    for (int n = 0; n < S; ++n) put(chirp, n, cr[n], ci[n]);
+    for (int k = 0; k < M; ++k) {
+        long double sr = 0.0L, si = 0.0L;
+        long long idx = 0;
+        for (int n = 0; n < M; ++n) {
+            if (br[n] != 0.0L || bi[n] != 0.0L) { sr += br[n] * wr[idx] - bi[n] * wi[idx]; si += br[n] * wi[idx] + bi[n] * wr[idx]; }
+            idx += k; if (idx >= M) idx -= M;
+        }
+        put(bspec, k, sr / M, si / M);
+    }
+}
+
 static void free_plan(poisson_plan *pl) {
     if (!pl) return;
     cudaFree(pl->a1); cudaFree(pl->a2); cudaFree(pl->kint);
-    for (int q = 0; q < 3; ++q) cudaFree(pl->tw[q]);
+    for (int q = 0; q < 3; ++q) { cudaFree(pl->tw[q]); cudaFree(pl->chirp[q]); cudaFree(pl->bspec[q]); }
     cudaFree(pl->rho_stage); cudaFree(pl->v_stage); cudaFree(pl->fused_sync);
     cudaFree(pl->wide_a1); cudaFree(pl->wide_a2);
     for (GraphSolve *g : {&pl->gs, &pl->gs_pdl}) { if (g->exec) cudaGraphExecDestroy(g->exec); if (g->graph) cudaGraphDestroy(g->graph); }
@@ -506,11 +562,24 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     if (ce == cudaSuccess) { ce = cudaMalloc(&pl->a2, (size_t)pl->a2_alloc_elems * cplx); ws += (size_t)pl->a2_alloc_elems * cplx; }
     if (ce == cudaSuccess) { ce = cudaMalloc(&pl->kint, (size_t)pl->kint_elems * pl->elem_real); ws += (size_t)pl->kint_elems * pl->elem_real; }
     for (int q = 0; q < 3 && ce == cudaSuccess; ++q) {
+        // a Bluestein axis (all passes of an axis agree: same length, any-length kernel) carries the table of its
+        // convolution length M plus the chirp and its spectrum
+        int M = 0;
+        for (int ps = 0; ps < 5; ++ps) if (d.pass[ps].axis == q && pl->k[ps]->generic && pl->k[ps]->gen_blue) M = pl->k[ps]->gen_L;
         std::vector<unsigned char> host;
-        fill_twiddles(host, d.s[q], precision);
+        fill_twiddles(host, M ? M : d.s[q], precision);
         ce = cudaMalloc(&pl->tw[q], host.size());
         if (ce == cudaSuccess) ce = cudaMemcpy(pl->tw[q], host.data(), host.size(), cudaMemcpyHostToDevice);
         ws += host.size();
+        if (M && ce == cudaSuccess) {
+            std::vector<unsigned char> hc, hb;
+            fill_bluestein(hc, hb, d.s[q], M, precision);
+            ce = cudaMalloc(&pl->chirp[q], hc.size());
+            if (ce == cudaSuccess) ce = cudaMemcpy(pl->chirp[q], hc.data(), hc.size(), cudaMemcpyHostToDevice);
+            if (ce == cudaSuccess) ce = cudaMalloc(&pl->bspec[q], hb.size());
+            if (ce == cudaSuccess) ce = cudaMemcpy(pl->bspec[q], hb.data(), hb.size(), cudaMemcpyHostToDevice);
+            ws += hc.size() + hb.size();
+        }
     }
     if (ce != cudaSuccess) {
         free_plan(pl);
@@ -707,6 +776,7 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
         const KernelEntry *e = pl->k[q];
         prm.gen_S = e->S; prm.gen_P = e->P; prm.gen_nfac = e->gen_nfac; prm.gen_pruned = e->pruned;
         prm.gen_nreal = ps.n_real; prm.gen_kcplx = pl->kcplx ? 1 : 0; prm.gen_lanes_p = ps.lanes_p;
+        prm.gen_L = e->gen_L; prm.gen_blue = e->gen_blue; prm.chirp = pl->chirp[ps.axis]; prm.bspec = pl->bspec[ps.axis];
         for (int i = 0; i < e->gen_nfac; ++i) prm.gen_fac[i] = e->gen_fac[i];
     }
     // L2 prefetch of the next tile only where the pass's input cannot be sitting in L2 already (measured: a few

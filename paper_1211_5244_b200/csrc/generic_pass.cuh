@@ -14,8 +14,8 @@
 // (natural order in, natural order out, no bit reversal).  The radices are chosen by the plan from {16, 12, 10, 8, 6, 5, 4,
 // 3, 2} (the in-register DFTs of fft_core.cuh: a thread holds a whole butterfly), 7 / 11 / 13 (the R-term sums written
 // out in registers) and, for any other prime factor p, a fallback that forms one output per thread per step -- O(p) per
-// point, so a prime length degenerates to the O(S^2) DFT (where a Bluestein chirp-z would be the asymptotically better
-// choice) and every smooth length is O(S log S) with as few passes over the tile as its factors allow.  Twiddles come from the plan's
+// point.  Lengths up to 1024 with a prime factor >= 17 instead take Bluestein's chirp-z (gen_transform below): two smooth
+// transforms of length M >= 2S - 1, so that every length is O(S log S).  Twiddles come from the plan's
 // table exp(-2 pi i m / S) in shared memory.  The paper's spread / compactification are the zero fill of
 // the tile's upper half on load and the store of the lower half only; R2C / C2R pack two real pencils
 // adjacent in x into one complex transform exactly as passes.cuh does, with an unpaired last pencil when N_x is odd.
@@ -31,7 +31,7 @@ constexpr int GEN_MAX_S = 4096;      // longest generic transform (three S-point
 
 // tile pitch: odd number of elements, so that both "lanes along pencils" and "lanes along the transform" spread over banks
 PF_CE int gen_pitch(int P) { return (P % 2 == 0) ? P + 1 : P; }
-PF_CE size_t gen_smem_bytes(int S, int P, size_t cplx_bytes) { return ((size_t)2 * S * gen_pitch(P) + S) * cplx_bytes; }
+PF_CE size_t gen_smem_bytes(int L, int P, size_t cplx_bytes) { return ((size_t)2 * L * gen_pitch(P) + L) * cplx_bytes; }   // L: buffer length (S, or Bluestein's M)
 
 // floor(n / d) for the index ranges of a tile (n d < 2^32) without an integer division: n * ceil(2^32 / d) >> 32
 struct GenDiv {
@@ -131,15 +131,16 @@ PF_HD void gen_stage_dispatch(const cx<T> *x, cx<T> *y, const cx<T> *tw, int S, 
     }
 }
 
-// The Stockham pass sequence over the tile in x (the function returns the buffer that holds the result).
+// The Stockham pass sequence over the tile in x (the function returns the buffer that holds the result); the transform
+// length is gen_L (= gen_S, or the convolution length M of the Bluestein path).
 template <typename T>
 PF_HD cx<T> *gen_fft(cx<T> *x, cx<T> *y, const cx<T> *tw, const PassParams &prm, bool inv, int tid) {
-    const int S = prm.gen_S, P = prm.gen_P;
-    int n = S, s = 1;
+    const int L = prm.gen_L, P = prm.gen_P;
+    int n = L, s = 1;
     for (int f = 0; f < prm.gen_nfac; ++f) {
         const int R = prm.gen_fac[f];
-        if (inv) gen_stage_dispatch<T, true>(x, y, tw, S, P, n, s, R, tid);
-        else gen_stage_dispatch<T, false>(x, y, tw, S, P, n, s, R, tid);
+        if (inv) gen_stage_dispatch<T, true>(x, y, tw, L, P, n, s, R, tid);
+        else gen_stage_dispatch<T, false>(x, y, tw, L, P, n, s, R, tid);
         __syncthreads();
         cx<T> *tmp = x; x = y; y = tmp;
         n /= R; s *= R;
@@ -147,15 +148,50 @@ PF_HD cx<T> *gen_fft(cx<T> *x, cx<T> *y, const cx<T> *tw, const PassParams &prm,
     return x;
 }
 
+// Length-S DFT of every pencil of the tile.  Smooth lengths: the Stockham passes directly.  Lengths with a prime factor
+// >= 17 (gen_blue): Bluestein's chirp-z -- with c_n = exp(-i pi n^2 / S),  n k = (n^2 + k^2 - (k - n)^2) / 2 gives
+//     X_k = c_k  sum_n (x_n c_n) conj(c_{k-n}),
+// a cyclic convolution of length M >= 2S - 1 done with two smooth length-M transforms: chirp[n] = c_n and
+// bspec = FFT_M(conj c, wrapped) / M come from the plan (host, long double); the inverse DFT conjugates both.
+template <typename T>
+PF_HD cx<T> *gen_transform(cx<T> *x, cx<T> *y, const cx<T> *tw, const PassParams &prm, bool inv, int tid) {
+    if (!prm.gen_blue) return gen_fft<T>(x, y, tw, prm, inv, tid);
+    const int S = prm.gen_S, L = prm.gen_L, P = prm.gen_P, PP = gen_pitch(P), lgP = 31 - __clz(P);
+    const cx<T> *chirp = reinterpret_cast<const cx<T> *>(prm.chirp), *bspec = reinterpret_cast<const cx<T> *>(prm.bspec);
+    for (int idx = tid; idx < L * P; idx += GEN_NT) {
+        const int p = idx & (P - 1), n = idx >> lgP;
+        cx<T> v = mk<T>((T)0, (T)0);
+        if (n < S) { const cx<T> c = chirp[n]; v = x[n * PP + p] * (inv ? conj(c) : c); }
+        x[n * PP + p] = v;
+    }
+    __syncthreads();
+    cx<T> *r = gen_fft<T>(x, y, tw, prm, false, tid);
+    cx<T> *o = (r == x) ? y : x;
+    for (int idx = tid; idx < L * P; idx += GEN_NT) {
+        const int p = idx & (P - 1), k = idx >> lgP;
+        const cx<T> b = bspec[k];
+        r[k * PP + p] = r[k * PP + p] * (inv ? conj(b) : b);
+    }
+    __syncthreads();
+    r = gen_fft<T>(r, o, tw, prm, true, tid);
+    for (int idx = tid; idx < S * P; idx += GEN_NT) {
+        const int p = idx & (P - 1), k = idx >> lgP;
+        const cx<T> c = chirp[k];
+        r[k * PP + p] = r[k * PP + p] * (inv ? conj(c) : c);
+    }
+    __syncthreads();
+    return r;
+}
+
 template <typename T, int KIND>
 __global__ void __launch_bounds__(GEN_NT, 2) generic_pass_kernel(const PassParams prm) {
     extern __shared__ __align__(16) unsigned char pf_smem[];
-    const int S = prm.gen_S, P = prm.gen_P, PP = gen_pitch(P), tid = threadIdx.x;
+    const int S = prm.gen_S, L = prm.gen_L, P = prm.gen_P, PP = gen_pitch(P), tid = threadIdx.x;
     const int H = S / 2 + 1;
     const bool pruned = prm.gen_pruned != 0;
-    cx<T> *b0 = reinterpret_cast<cx<T> *>(pf_smem), *b1 = b0 + (size_t)S * PP, *tw = b1 + (size_t)S * PP;
+    cx<T> *b0 = reinterpret_cast<cx<T> *>(pf_smem), *b1 = b0 + (size_t)L * PP, *tw = b1 + (size_t)L * PP;
     pdl_launch_dependents();
-    { const cx<T> *tab = reinterpret_cast<const cx<T> *>(prm.tw); for (int i = tid; i < S; i += GEN_NT) tw[i] = tab[i]; }
+    { const cx<T> *tab = reinterpret_cast<const cx<T> *>(prm.tw); for (int i = tid; i < L; i += GEN_NT) tw[i] = tab[i]; }
     pdl_wait_prior_grid();
     __syncthreads();
     const int n_half = pruned ? S / 2 : S;      // points that exist on the un-padded side of this pass
@@ -208,7 +244,7 @@ __global__ void __launch_bounds__(GEN_NT, 2) generic_pass_kernel(const PassParam
 
         // ---------------- transform(s)
         constexpr bool FIRST_INV = KIND == KIND_I2 || KIND == KIND_I1;
-        cx<T> *r = gen_fft<T>(x, y, tw, prm, FIRST_INV, tid);
+        cx<T> *r = gen_transform<T>(x, y, tw, prm, FIRST_INV, tid);
         cx<T> *o = (r == b0) ? b1 : b0;
         if constexpr (KIND == KIND_F3) {            // V^F = K^F rho^F (Eq. 3), then straight back
             const bool lanes_p = prm.gen_lanes_p != 0;
@@ -225,7 +261,7 @@ __global__ void __launch_bounds__(GEN_NT, 2) generic_pass_kernel(const PassParam
                 }
             }
             __syncthreads();
-            r = gen_fft<T>(r, o, tw, prm, true, tid);
+            r = gen_transform<T>(r, o, tw, prm, true, tid);
         }
 
         // ---------------- store (compactification: only the lower half leaves the chip)

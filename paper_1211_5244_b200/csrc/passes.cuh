@@ -117,6 +117,8 @@ struct PassParams {
     // any-length kernel only (generic_pass.cuh): transform length, pencils per tile, radices (product = gen_S), zero-padded axis,
     // real pencils along x of the R2C / C2R pass, complex K^F
     int gen_S, gen_P, gen_nfac, gen_pruned, gen_nreal, gen_kcplx, gen_lanes_p;
+    int gen_L, gen_blue;           // buffer / transform length (gen_S, or Bluestein's convolution length M) and the Bluestein flag
+    const void *chirp, *bspec;     // Bluestein: exp(-i pi n^2 / S), n < S;  FFT_M of the wrapped conjugate chirp, / M
     int gen_fac[16];
 };
 

@@ -24,6 +24,7 @@ struct KernelEntry {
     // any-length kernel (generic_pass.cuh): a per-plan entry with run-time length, tile width and radix list
     int generic;       // 0 for the compiled register-engine kernels
     int gen_nfac, gen_fac[16];
+    int gen_L, gen_blue;   // transform / buffer length (S, or Bluestein's M) and the Bluestein flag
 };
 
 // A fused solve kernel (solve_kernel.cuh): all five passes of one (axis a, axis b, axis c) combination.

@@ -76,10 +76,12 @@ def test_general_sizes_all_bc_vs_oracle(pk, n, prec):
         assert err <= TOL[prec], (n, bc, prec, err)
 
 
-@pytest.mark.parametrize("n,bc", [((251, 6, 4), (1, 0, 0)), ((4, 6, 300), (0, 0, 0)), ((6, 360, 4), (0, 1, 0)), ((450, 4, 2), (0, 0, 1))])
+@pytest.mark.parametrize("n,bc", [((251, 6, 4), (1, 0, 0)), ((4, 6, 300), (0, 0, 0)), ((6, 360, 4), (0, 1, 0)), ((450, 4, 2), (0, 0, 1)),
+                                  ((127, 4, 6), (0, 0, 0)), ((4, 6, 521), (0, 0, 1)), ((4, 6, 521), (0, 0, 0)), ((509, 3, 2), (1, 1, 1))])
 def test_long_awkward_lengths_vs_oracle(pk, n, bc):
-    """A prime length (251), 2 * 3 * 4 * 5 * 5 = 600, 360 = 4 * 2 * 3 * 3 * 5 and 900 = 4 * 3 * 3 * 5 * 5: the lengths DESIGN.md
-    (round 1) named as needing a three-pass engine."""
+    """600, 360 and 900 (the lengths DESIGN.md, round 1, named as needing a three-pass engine); prime and 2 * prime lengths up to
+    1024 through Bluestein's chirp-z (251, 254 = 2 * 127, 521, 509 with odd N_x in the R2C pass next to it); 1042 = 2 * 521, above the
+    Bluestein limit, through the O(p) fallback butterfly."""
     rng = np.random.default_rng(77 + sum(n))
     s = gen.padded_shape(n, bc)
     rho = rng.standard_normal((n[2], n[1], n[0]))

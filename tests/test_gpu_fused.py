@@ -196,3 +196,40 @@ def test_plane_chunked_middle_passes(pk, monkeypatch, n, bc, prec, mode):
         assert ei.value.status == 2                                # A2 is never whole in memory on a chunked plan
     finally:
         plan.close()
+
+
+MODE_ENV = {"five": {"POISSON_TUNE": "0"}, "five_pdl": {"POISSON_PDL": "1"}, "graph": {"POISSON_GRAPH": "1"},
+            "graph_pdl": {"POISSON_GRAPH": "1", "POISSON_PDL": "1"}, "fused": {"POISSON_FUSED": "1"}}
+
+
+@pytest.mark.parametrize("mode", list(MODE_ENV))
+@pytest.mark.parametrize("n", [(16, 8, 4), (24, 16, 32), (32, 32, 32), (20, 40, 36), (7, 12, 10)], ids=lambda n: "x".join(map(str, n)))
+def test_every_launch_mode_all_bc_vs_oracle(pk, monkeypatch, n, mode):
+    """poisson_plan_create normally keeps whichever launch mode its timing run found fastest, so a sweep only exercises the
+    winner.  Here every mode is FORCED in turn (all 8 BC combinations per size, compiled and any-length kernels) and compared
+    with the oracle; the mode actually used is asserted (the fused kernel exists only for the combinations of csrc/fused.def
+    and falls back to five launches elsewhere)."""
+    import itertools
+    import torch
+    for k, v in MODE_ENV[mode].items():
+        monkeypatch.setenv(k, v)
+    rng = np.random.default_rng(2024 + sum(n))
+    used = set()
+    for bc in itertools.product((0, 1), repeat=3):
+        s = gen.padded_shape(n, bc)
+        rho = rng.standard_normal((n[2], n[1], n[0]))
+        Kf = oracle.kernel_spectrum(_even_kernel(rng, s))
+        plan = pk.PoissonPlan(n, bc, 0.25, pk.FP64)
+        try:
+            got_mode = plan.launch_mode()[0]
+            used.add(got_mode)
+            assert got_mode == mode or (mode == "fused" and got_mode == "five")
+            plan.set_kernel(torch.from_numpy(Kf).cuda())
+            r = torch.from_numpy(rho).cuda()
+            V1 = plan.solve(r).cpu().numpy()
+            V2 = plan.solve(r).cpu().numpy()              # a second solve on the same plan (counters / graph nodes re-armed)
+        finally:
+            plan.close()
+        assert np.array_equal(V1, V2)
+        assert rel_l2(V1, oracle.solve(rho, Kf, bc)) <= 1e-12, (n, bc, mode)
+    print(n, mode, "modes used:", sorted(used))

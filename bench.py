@@ -378,7 +378,7 @@ def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, wi
     mode, tune_ms = plan.launch_mode()
     res = {"key": key, "single": single, "batch": batch, "batch_size": bsz,
            "info": info, "nbuf": nbuf, "rho_bytes": rho_bytes,
-           "launch_mode": mode, "tune_ms": tune_ms, "lanes": plan.batch_lanes(bsz),
+           "launch_mode": mode, "tune_ms": tune_ms, "graph_shape": list(plan.graph_shape()), "lanes": plan.batch_lanes(bsz),
            "width": plan.batch_width(bsz), "launches_per_solve": plan.launches_per_solve()}
     if pass_ms is not None:
         res["pass_ms"] = pass_ms
@@ -517,8 +517,11 @@ def run_ours(args):
                      "algorithmic_bytes_per_launch": dom_bytes, "peak_source": peak_src,
                      "duration_us": dom_us, "duration_source": "CUDA events around the kernel's stream launch (pass_us)"},
         "launch_mode": {"chosen": res["launch_mode"], "ms_per_solve_at_plan_creation": res["tune_ms"],
+                        "graph_shape": {"plane_chains": res["graph_shape"][0], "x_chains": res["graph_shape"][1]},
                         "note": "poisson_plan_create times {five launches, five + programmatic dependent launch, one fused "
-                                "cooperative launch, the five launches as one CUDA graph, that graph with PDL edges} and keeps the fastest"},
+                                "cooperative launch, the five passes as one CUDA graph, that graph with PDL edges} and keeps the fastest; "
+                                "the graph's passes are split into parallel chains over ranges of k_a planes and of x "
+                                "(poisson_plan_graph_shape): the same tiles by the same kernels, only the dependencies are finer"},
         "e2e": {"value": world * 1e3 / res["e2e_ms_per_step"], "unit": UNIT, "h2d_bytes_per_step": res["rho_bytes"],
                 "d2h_bytes_per_step": res["rho_bytes"], "ms_per_step": res["e2e_ms_per_step"], "steps": res["e2e_steps"],
                 "api": (f"poisson_solve_batch_host, {res['e2e_batch']} pinned host densities per call: every rho copied H2D, five passes, "
@@ -547,7 +550,7 @@ def run_ours(args):
                            "hbm_frac": i2.bytes_total / (r["single"]["ms"] * 1e-3) / 1e9 / peak,
                            "batched_ms_per_step": r["batch"]["ms"],
                            "batched_hbm_frac": i2.bytes_total / (r["batch"]["ms"] * 1e-3) / 1e9 / peak,
-                           "e2e_ms_per_step": r["e2e_ms_per_step"], "launch_mode": r["launch_mode"],
+                           "e2e_ms_per_step": r["e2e_ms_per_step"], "launch_mode": r["launch_mode"], "graph_shape": r["graph_shape"],
                            "pass_us": {pk.PASS_NAMES[q]: r["pass_ms"][q] * 1e3 for q in range(5)}}
         line["other_configs"] = others
         if "c4a" in others and "c4p" in others:

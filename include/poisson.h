@@ -199,8 +199,10 @@ POISSON_API int poisson_profile_read(poisson_plan *plan, double ms_sum[5] /* hos
 
 /* How poisson_solve launches the 13 steps of PAPER.md:57-71:
  *   FIVE      five fused passes, one launch each;
- *   FIVE_PDL  the same five launches with programmatic dependent launch (the next pass becomes resident
- *             while the previous one drains; pays on launch-bound grids);
+ *   FIVE_PDL  the same five launches with programmatic dependent launch: a CTA that has issued the loads of its last tile
+ *             lets the next pass launch, whose CTAs take the freed SM slots, build their tables and wait for the
+ *             previous pass to complete (triggering at the START of a pass instead costs 10 % on the 256^3 / 512^3
+ *             grids, measured: POISSON_PDL_TRIGGER=0);
  *   FUSED     ONE persistent cooperative launch: F1 | grid barrier | F2 -> F3 -> I2 as a per-plane dataflow
  *             through L2 | grid barrier | I1 (compiled for the combinations in csrc/fused_*.cu).
  *   GRAPH     the five launches as kernel nodes of one instantiated CUDA graph (one cudaGraphLaunch per solve; rho / V
@@ -214,8 +216,20 @@ POISSON_API int poisson_profile_read(poisson_plan *plan, double ms_sum[5] /* hos
 enum { POISSON_LAUNCH_FIVE = 0, POISSON_LAUNCH_FIVE_PDL = 1, POISSON_LAUNCH_FUSED = 2, POISSON_LAUNCH_GRAPH = 3, POISSON_LAUNCH_GRAPH_PDL = 4 };
 POISSON_API int poisson_plan_launch_mode(const poisson_plan *plan, int *mode /* host, out */, double ms_per_solve[5] /* host, out */);
 
+/* Shape of the GRAPH / GRAPH_PDL solve graph.  The five passes only couple along the axis they transform, so the graph
+ * need not be a chain: with J ranges of k_a planes and R ranges of x it is
+ *     F1_r -> F2_{r,j} -> F3_j -> I2_{r,j} -> I1_r          (r < R, j < J)
+ * (F1 / F2 / I2 / I1 tiles of different x never exchange data, F2 / F3 / I2 tiles of different k_a neither; PAPER.md:53's
+ * transposes are the only coupling), 2R + 2RJ + J kernel nodes in all.  A kernel whose successor needs only part of the
+ * grid hands its SM slots to that successor while its siblings still run, which hides the ramp-up and tail of the
+ * passes inside ONE solve (128^3 -> 256^3 fp64 on B200: 98.4 us as a chain, 92.3 with J = 4, 90.6 with J = R = 2).
+ * poisson_plan_create times a few shapes together with the launch modes; POISSON_BRANCHES=J / POISSON_XCHAINS=R fix one.
+ * x ranges need x as the last-processed axis and whole tiles per range, else R = 1.  Outputs 1, 1 in the other modes.
+ * Errors: EINVAL. */
+POISSON_API int poisson_plan_graph_shape(const poisson_plan *plan, int *plane_chains /* host, out */, int *x_chains /* host, out */);
+
 /* Number of kernel launches one poisson_solve enqueues (bench.py's gpu_launches): 5, 2 + 3 * chunks on a chunked plan, or 1
- * in FUSED mode. */
+ * in FUSED mode, 2R + 2RJ + J kernel nodes for a shaped graph (poisson_plan_graph_shape). */
 POISSON_API int poisson_plan_launches_per_solve(const poisson_plan *plan);
 
 /* Measures the plain-ALU fused-multiply-add peak of the current device for the given precision

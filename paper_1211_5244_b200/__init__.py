@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "poisson_plan_describe", "poisson_plan_create", "poisson_plan_kernel_dims", "poisson_plan_get_info",
     "poisson_set_kernel", "poisson_set_kernel_complex", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
     "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_measure_fma_peak", "poisson_plan_workspace_bytes",
-    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes", "poisson_plan_batch_width",
+    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_plan_graph_shape", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes", "poisson_plan_batch_width",
 )
 
 _PKG = Path(__file__).resolve().parent
@@ -93,6 +93,7 @@ def load_library():
     lib.poisson_solve_batch.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), i, vp]
     lib.poisson_solve_batch_host.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), i, vp]
     lib.poisson_plan_launch_mode.argtypes = [vp, ctypes.POINTER(i), ctypes.c_double * 5]
+    lib.poisson_plan_graph_shape.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i)]
     lib.poisson_plan_workspace_bytes.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.restype = ctypes.c_size_t
     lib.poisson_plan_destroy.argtypes = [vp]
@@ -285,6 +286,12 @@ class PoissonPlan:
         _check(load_library().poisson_plan_launch_mode(self._h, ctypes.byref(mode), ms), "poisson_plan_launch_mode")
         names = ("five", "five_pdl", "fused", "graph", "graph_pdl")
         return names[mode.value], {names[k]: ms[k] for k in range(5) if ms[k] > 0}
+
+    def graph_shape(self):
+        """(chains over k_a plane ranges, chains over x ranges) of the solve graph -- see poisson_plan_graph_shape."""
+        j, r = ctypes.c_int(), ctypes.c_int()
+        _check(load_library().poisson_plan_graph_shape(self._h, ctypes.byref(j), ctypes.byref(r)), "poisson_plan_graph_shape")
+        return j.value, r.value
 
     def workspace_bytes(self) -> int:
         return load_library().poisson_plan_workspace_bytes(self._h)

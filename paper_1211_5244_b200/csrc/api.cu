@@ -210,6 +210,7 @@ struct Lane {
 // The launches of one solve as an instantiated CUDA graph (kernel nodes F1 -> F2 -> F3 -> I2 -> I1, the middle three once per
 // plane chunk): one graph launch per solve; rho / V of the call are patched into the F1 / I1 nodes when they differ from the
 // previous call.
+#define PF_MAX_XR 8
 struct GraphSolve {
     cudaGraph_t graph;
     cudaGraphExec_t exec;
@@ -217,6 +218,10 @@ struct GraphSolve {
     PassParams prm_f1, prm_i1;
     const void *rho;
     void *V;
+    int xr;                             // > 1: F1 / I1 are split into xr kernels over ranges of x (x chains)
+    cudaGraphNode_t node_f1x[PF_MAX_XR], node_i1x[PF_MAX_XR];
+    PassParams prm_f1x[PF_MAX_XR], prm_i1x[PF_MAX_XR];
+    long long off_rho[PF_MAX_XR], off_V[PF_MAX_XR];   // byte offsets of the ranges in rho / V
 };
 
 struct poisson_plan {
@@ -235,6 +240,12 @@ struct poisson_plan {
     int chunk_planes, n_chunks; // middle passes F2 -> F3 -> I2 run chunk by chunk of k_a planes through a chunk-sized A2 (1 chunk: whole grid)
     long long a2_alloc_elems;   // complex elements of the A2 buffer actually allocated (one chunk when chunked)
     int late_tw;               // PassParams::late_tw for every pass (POISSON_LATE_TW, default 1; 0 under programmatic dependent launch)
+    int pdl_trigger;           // PassParams::pdl_trigger (POISSON_PDL_TRIGGER: 0 start of the pass, 1 last tile of each CTA, 2 exit)
+    bool env_lane_shape;       // POISSON_LANE_SHAPE=1: the batch lanes' graphs take the plan's graph shape too (experiments)
+    bool env_shape;            // POISSON_BRANCHES / POISSON_XCHAINS given: the tuner keeps that graph shape
+    int xchains;               // graph mode: F1 / F2 / I2 / I1 split over this many ranges of x (POISSON_XCHAINS)
+    int branch_serial, branch_grid;   // experiments: order the chains' kernels of one kind; cap the grid of a chain's kernels
+    int branches;              // graph mode: the middle passes as this many parallel chains over ranges of k_a planes (POISSON_BRANCHES)
     int env_lanes, env_wide;   // POISSON_LANES / POISSON_WIDE as read at plan creation (-1: not set)
     bool env_lane_graph;       // POISSON_LANE_GRAPH=0 at plan creation: plain launches on the batch lanes (experiments)
     void *wide_a1, *wide_a2;   // intermediates of wide_w densities (several small solves per launch), allocated on first use
@@ -504,6 +515,13 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     for (int q = 0; q < 5; ++q) pl->pf_force[q] = env_pass_value("POISSON_PREFETCH", q, -1);
     // every environment knob is read HERE, once; the solve path never calls getenv
     { const char *env = std::getenv("POISSON_LATE_TW"); pl->late_tw = env ? std::atoi(env) : 1; }
+    { const char *env = std::getenv("POISSON_PDL_TRIGGER"); pl->pdl_trigger = env ? std::atoi(env) : 1; }
+    { const char *env = std::getenv("POISSON_BRANCHES"); pl->branches = env ? std::atoi(env) : 1; }
+    { const char *env = std::getenv("POISSON_XCHAINS"); pl->xchains = env ? std::atoi(env) : 1; if (pl->xchains > PF_MAX_XR) pl->xchains = PF_MAX_XR; }
+    pl->env_shape = std::getenv("POISSON_BRANCHES") || std::getenv("POISSON_XCHAINS");
+    { const char *env = std::getenv("POISSON_LANE_SHAPE"); pl->env_lane_shape = env && env[0] == '1'; }
+    { const char *env = std::getenv("POISSON_BRANCH_SERIAL"); pl->branch_serial = env ? std::atoi(env) : 0; }
+    { const char *env = std::getenv("POISSON_BRANCH_GRID"); pl->branch_grid = env ? std::atoi(env) : 0; }
     { const char *env = std::getenv("POISSON_LANES"); pl->env_lanes = env ? std::atoi(env) : -1; }
     { const char *env = std::getenv("POISSON_WIDE"); pl->env_wide = env ? std::atoi(env) : -1; }
     { const char *env = std::getenv("POISSON_LANE_GRAPH"); pl->env_lane_graph = !(env && env[0] == '0'); }
@@ -639,7 +657,14 @@ int poisson_plan_get_info(const poisson_plan *pl, poisson_plan_info *info) {
 
 size_t poisson_plan_workspace_bytes(const poisson_plan *pl) { return pl ? pl->workspace_bytes : 0; }
 
-int poisson_plan_launches_per_solve(const poisson_plan *pl) { return pl ? (pl->fused && pl->use_fused ? 1 : launches_per_solve(pl)) : 0; }   // kernels per solve (graph mode: that many kernel nodes)
+// kernels per solve (graph mode: that many kernel nodes; a shaped graph has R F1 + R J F2 + J F3 + R J I2 + R I1 of them)
+int poisson_plan_launches_per_solve(const poisson_plan *pl) {
+    if (!pl) return 0;
+    if (pl->fused && pl->use_fused) return 1;
+    int J = 1, R = 1;
+    if (poisson_plan_graph_shape(pl, &J, &R) == POISSON_OK && (J > 1 || R > 1)) return 2 * R + 2 * R * J + J;
+    return launches_per_solve(pl);
+}
 
 int poisson_plan_launch_mode(const poisson_plan *pl, int *mode, double ms_per_solve[5]) {
     if (!pl || !mode || !ms_per_solve) return POISSON_EINVAL;
@@ -647,6 +672,14 @@ int poisson_plan_launch_mode(const poisson_plan *pl, int *mode, double ms_per_so
           : (pl->use_graph && active_graph(pl) ? (pl->use_pdl ? POISSON_LAUNCH_GRAPH_PDL : POISSON_LAUNCH_GRAPH)
                                                : (pl->use_pdl ? POISSON_LAUNCH_FIVE_PDL : POISSON_LAUNCH_FIVE));
     for (int m = 0; m < 5; ++m) ms_per_solve[m] = (double)pl->tune_ms[m];
+    return POISSON_OK;
+}
+
+int poisson_plan_graph_shape(const poisson_plan *pl, int *plane_chains, int *x_chains) {
+    if (!pl || !plane_chains || !x_chains) return POISSON_EINVAL;
+    const GraphSolve *g = (pl->use_graph && !(pl->fused && pl->use_fused)) ? active_graph(pl) : nullptr;
+    *plane_chains = g && pl->n_chunks <= 1 && pl->branches > 1 ? (pl->branches < pl->d.H ? pl->branches : pl->d.H) : 1;
+    *x_chains = g && g->xr > 1 ? g->xr : 1;
     return POISSON_OK;
 }
 
@@ -771,7 +804,8 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
     prm.n_tiles1 = pl->n_tiles[q];   // one density per launch
     // twiddle tables under the first tile's load latency; with programmatic dependent launch they are built BEFORE the wait
     // on the previous pass instead (that is the part of a pass PDL overlaps with its predecessor's tail)
-    prm.late_tw = (pl->late_tw && !pl->use_pdl) ? 1 : 0;
+    prm.late_tw = (pl->late_tw == 2 || (pl->late_tw && !pl->use_pdl)) ? 1 : 0;   // POISSON_LATE_TW=2: late also under PDL (experiments)
+    prm.pdl_trigger = pl->pdl_trigger;
     if (pl->k[q]->generic) {
         const KernelEntry *e = pl->k[q];
         prm.gen_S = e->S; prm.gen_P = e->P; prm.gen_nfac = e->gen_nfac; prm.gen_pruned = e->pruned;
@@ -883,29 +917,158 @@ static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t s
 }
 
 // Builds the graph of one solve on the plan's own intermediates (explicit kernel nodes, plain dependencies).
+// Parameters of pass q restricted to the k_a planes [g0, g0 + ng) (middle passes F2, F3, I2) and / or to the pencils
+// x in [x0, x0 + nx) (F1, F2, I2, I1 when their pencil index is the x axis; nx = 0: all) of the full-size arrays.
+static PassParams range_params(const poisson_plan *pl, int q, const Lane *ln, int g0, int ng, int x0 = 0, int nx = 0) {
+    const size_t cplx = 2 * pl->elem_real;
+    PassParams prm = pass_params(pl, q, nullptr, nullptr, ln);
+    const bool ends = q == POISSON_PASS_F1 || q == POISSON_PASS_I1;
+    long long off_in = 0, off_out = 0;
+    if (!ends) {
+        prm.k_g0 = g0;                                     // K^F is indexed by the plane's position in the whole grid
+        off_in += (long long)g0 * prm.gs_in; off_out += (long long)g0 * prm.gs_out;
+    } else {
+        ng = (int)pl->d.pass[q].n_g;
+    }
+    if (nx > 0) {
+        const int e = pl->k[q]->P;
+        if (ends) {   // pencils are x-pairs: rho / V in pairs, A1 in complex numbers (two per pair)
+            const int x0p = x0 / 2, nxp = nx / 2;
+            prm.n_p = nxp; prm.tiles_per_g = (nxp + e - 1) / e;
+            if (q == POISSON_PASS_F1) { off_in += (long long)x0p * prm.ps_in; off_out += 2LL * x0p * prm.ps_out; }
+            else { off_in += 2LL * x0p * prm.ps_in; off_out += (long long)x0p * prm.ps_out; }
+        } else {
+            prm.n_p = nx; prm.tiles_per_g = (nx + e - 1) / e;
+            off_in += (long long)x0 * prm.ps_in; off_out += (long long)x0 * prm.ps_out;
+        }
+    }
+    prm.n_tiles = ng * prm.tiles_per_g;
+    prm.n_tiles1 = prm.n_tiles;
+    prm.in = static_cast<const char *>(prm.in) + (size_t)off_in * cplx;
+    prm.out = static_cast<char *>(prm.out) + (size_t)off_out * cplx;
+    return prm;
+}
+
 static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
     if (g.exec) return POISSON_OK;
     PF_CUDA(cudaGraphCreate(&g.graph, 0));
-    cudaGraphNode_t prev = nullptr;
-    bool have_prev = false;
-    const int rc = for_each_launch(pl, nullptr, nullptr, ln, 0, 4, [&](int q, const PassParams &prm_in, int grid) -> int {
+    auto add_node = [&](int q, PassParams prm, int grid, cudaGraphNode_t *node) -> int {
         const KernelEntry *e = pl->k[q];
-        PassParams prm = prm_in;
-        if (q == POISSON_PASS_F1) g.prm_f1 = prm;
-        if (q == POISSON_PASS_I1) g.prm_i1 = prm;
         void *args[] = {&prm};
         cudaKernelNodeParams kp{};
         kp.func = const_cast<void *>(e->func);
         kp.gridDim = dim3(grid); kp.blockDim = dim3(e->NT);
         kp.sharedMemBytes = (unsigned)e->smem_bytes;
         kp.kernelParams = args; kp.extra = nullptr;
-        cudaGraphNode_t node;
-        PF_CUDA(cudaGraphAddKernelNode(&node, g.graph, have_prev ? &prev : nullptr, have_prev ? 1 : 0, &kp));
-        if (q == POISSON_PASS_F1) g.node_f1 = node;
-        if (q == POISSON_PASS_I1) g.node_i1 = node;
-        prev = node; have_prev = true;
+        PF_CUDA(cudaGraphAddKernelNode(node, g.graph, nullptr, 0, &kp));
         return POISSON_OK;
-    });
+    };
+    // data dependency from -> to; programmatic (the dependent may launch when `from` triggers, and waits inside the kernel) when asked
+    const bool prog = pl->use_pdl;
+    auto add_edge = [&](cudaGraphNode_t from, cudaGraphNode_t to, bool programmatic) -> int {
+        if (programmatic) {
+            cudaGraphEdgeData ed{};
+            ed.type = cudaGraphDependencyTypeProgrammatic; ed.from_port = cudaGraphKernelNodePortProgrammatic;
+            PF_CUDA(cudaGraphAddDependencies_v2(g.graph, &from, &to, &ed, 1));
+        } else {
+            PF_CUDA(cudaGraphAddDependencies(g.graph, &from, &to, 1));
+        }
+        return POISSON_OK;
+    };
+    int rc = POISSON_OK;
+    const bool shaped = pl->n_chunks <= 1 && (!ln || pl->env_lane_shape);   // batch lanes already overlap each other: plain chains there
+    const int B = shaped ? (pl->branches < pl->d.H ? pl->branches : pl->d.H) : 1;
+    int R = shaped ? pl->xchains : 1;
+    {   // x chains need: no plane chunks, the register engine everywhere, x as the pencil index of F1 / F2 / I2 / I1, whole tiles per range
+        bool ok = R > 1 && pl->n_chunks <= 1 && pl->d.order[2] == 0;
+        for (int q = 0; q < 5 && ok; ++q) ok = !pl->k[q]->generic;
+        if (ok) ok = pl->d.n[0] % (R * 2 * pl->k[0]->P) == 0 && pl->d.n[0] % (R * pl->k[1]->P) == 0;
+        if (!ok) R = 1;
+    }
+    if (R > 1) {
+        // F1_r -> F2_{r,j} -> F3_j -> I2_{r,j} -> I1_r: r = range of x (F1 / F2 / I2 / I1 tiles only couple along y resp. k_a),
+        // j = range of k_a planes (F3 couples along x).  Every kernel except F3 has a successor that only needs part of the grid.
+        const int J = B > 1 ? B : 1, nxr = pl->d.n[0] / R;
+        std::vector<cudaGraphNode_t> f1(R), i1(R), f2(R * J), f3(J), i2(R * J);
+        g.node_f1 = nullptr; g.node_i1 = nullptr;   // rho / V are patched into R nodes each: see run_graph
+        g.xr = R;
+        for (int r = 0; r < R && rc == POISSON_OK; ++r) {
+            g.prm_f1x[r] = range_params(pl, POISSON_PASS_F1, ln, 0, 0, r * nxr, nxr);
+            rc = add_node(POISSON_PASS_F1, g.prm_f1x[r], g.prm_f1x[r].n_tiles < pl->grid[0] ? g.prm_f1x[r].n_tiles : pl->grid[0], &f1[r]);
+            g.node_f1x[r] = f1[r];
+            g.off_rho[r] = (long long)reinterpret_cast<size_t>(g.prm_f1x[r].in);    // built on a NULL rho: the pointer IS the range's offset
+        }
+        auto pr = [&](int j, int &g0, int &ng) { g0 = (int)((long long)pl->d.H * j / J); ng = (int)((long long)pl->d.H * (j + 1) / J) - g0; };
+        for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2 && rc == POISSON_OK; ++q)
+            for (int j = 0; j < J && rc == POISSON_OK; ++j) {
+                int g0, ng; pr(j, g0, ng);
+                if (q == POISSON_PASS_F3) {
+                    const PassParams prm = range_params(pl, q, ln, g0, ng);
+                    rc = add_node(q, prm, prm.n_tiles < pl->grid[q] ? prm.n_tiles : pl->grid[q], &f3[j]);
+                    for (int r = 0; r < R && rc == POISSON_OK; ++r) rc = add_edge(f2[r * J + j], f3[j], prog && r == 0);
+                } else {
+                    for (int r = 0; r < R && rc == POISSON_OK; ++r) {
+                        const PassParams prm = range_params(pl, q, ln, g0, ng, r * nxr, nxr);
+                        cudaGraphNode_t &node = q == POISSON_PASS_F2 ? f2[r * J + j] : i2[r * J + j];
+                        rc = add_node(q, prm, prm.n_tiles < pl->grid[q] ? prm.n_tiles : pl->grid[q], &node);
+                        if (rc == POISSON_OK) rc = add_edge(q == POISSON_PASS_F2 ? f1[r] : f3[j], node, prog);
+                    }
+                }
+            }
+        for (int r = 0; r < R && rc == POISSON_OK; ++r) {
+            g.prm_i1x[r] = range_params(pl, POISSON_PASS_I1, ln, 0, 0, r * nxr, nxr);
+            rc = add_node(POISSON_PASS_I1, g.prm_i1x[r], g.prm_i1x[r].n_tiles < pl->grid[4] ? g.prm_i1x[r].n_tiles : pl->grid[4], &i1[r]);
+            g.node_i1x[r] = i1[r];
+            g.off_V[r] = (long long)reinterpret_cast<size_t>(g.prm_i1x[r].out);
+            for (int j = 0; j < J && rc == POISSON_OK; ++j) rc = add_edge(i2[r * J + j], i1[r], prog && j == 0);
+        }
+    } else if (B > 1) {
+        // F1 -> B parallel chains (F2 -> F3 -> I2 over a range of k_a planes: the middle passes work plane by plane) -> I1.
+        // A chain's next kernel is ready while the other chains still run, so its CTAs fill the slots a draining kernel frees:
+        // the ramp-up / tail of the middle passes overlaps other work, as it does between the lanes of a batch.
+        g.prm_f1 = pass_params(pl, POISSON_PASS_F1, nullptr, nullptr, ln);
+        g.prm_i1 = pass_params(pl, POISSON_PASS_I1, nullptr, nullptr, ln);
+        rc = add_node(POISSON_PASS_F1, g.prm_f1, pl->grid[0], &g.node_f1);
+        cudaGraphNode_t last[3] = {nullptr, nullptr, nullptr};   // the previous chain's F2 / F3 / I2 (serial ordering experiment)
+        std::vector<cudaGraphNode_t> tails(B, g.node_f1);
+        auto add_chain_node = [&](int j, int q) -> int {
+            const int g0 = (int)((long long)pl->d.H * j / B), g1 = (int)((long long)pl->d.H * (j + 1) / B);
+            const PassParams prm = range_params(pl, q, ln, g0, g1 - g0);
+            int grid = prm.n_tiles < pl->grid[q] ? prm.n_tiles : pl->grid[q];
+            if (pl->branch_grid > 0 && grid > pl->branch_grid) grid = pl->branch_grid;
+            cudaGraphNode_t node;
+            int rc1 = add_node(q, prm, grid, &node);
+            if (rc1 == POISSON_OK) rc1 = add_edge(tails[j], node, prog);
+            if (rc1 == POISSON_OK && pl->branch_serial == 1 && last[q - 1]) rc1 = add_edge(last[q - 1], node, false);
+            last[q - 1] = node;
+            tails[j] = node;
+            return rc1;
+        };
+        if (pl->branch_serial == 2) {   // node creation order: pass by pass
+            for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2; ++q)
+                for (int j = 0; j < B && rc == POISSON_OK; ++j) rc = add_chain_node(j, q);
+        } else {                        // chain by chain
+            for (int j = 0; j < B; ++j)
+                for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2 && rc == POISSON_OK; ++q) rc = add_chain_node(j, q);
+        }
+        if (rc == POISSON_OK) rc = add_node(POISSON_PASS_I1, g.prm_i1, pl->grid[4], &g.node_i1);
+        for (size_t j = 0; j < tails.size() && rc == POISSON_OK; ++j) rc = add_edge(tails[j], g.node_i1, prog && j == 0);   // one programmatic edge into I1, the rest plain
+    } else {
+        cudaGraphNode_t prev = nullptr;
+        bool have_prev = false;
+        rc = for_each_launch(pl, nullptr, nullptr, ln, 0, 4, [&](int q, const PassParams &prm, int grid) -> int {
+            if (q == POISSON_PASS_F1) g.prm_f1 = prm;
+            if (q == POISSON_PASS_I1) g.prm_i1 = prm;
+            cudaGraphNode_t node;
+            int rc1 = add_node(q, prm, grid, &node);
+            if (rc1 == POISSON_OK && have_prev) rc1 = add_edge(prev, node, false);
+            if (rc1 != POISSON_OK) return rc1;
+            if (q == POISSON_PASS_F1) g.node_f1 = node;
+            if (q == POISSON_PASS_I1) g.node_i1 = node;
+            prev = node; have_prev = true;
+            return POISSON_OK;
+        });
+    }
     if (rc != POISSON_OK) { cudaGraphDestroy(g.graph); g.graph = nullptr; return rc; }
     PF_CUDA(cudaGraphInstantiate(&g.exec, g.graph, 0));
     g.rho = nullptr; g.V = nullptr;
@@ -916,6 +1079,13 @@ static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
 // the launch attribute into programmatic edges); the F1 / I1 kernel nodes are identified by their function.
 static int build_graph_pdl(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
     if (g.exec) return POISSON_OK;
+    if ((pl->branches > 1 || pl->xchains > 1) && pl->n_chunks <= 1 && (!ln || pl->env_lane_shape)) {   // parallel chains: explicit nodes with programmatic edges
+        const bool saved = pl->use_pdl;
+        pl->use_pdl = true;
+        const int rc = build_graph(pl, g, ln);
+        pl->use_pdl = saved;
+        return rc;
+    }
     cudaStream_t cs = nullptr;
     PF_CUDA(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
     const bool saved = pl->use_pdl;
@@ -954,15 +1124,20 @@ static int run_graph(poisson_plan *pl, GraphSolve &g, const void *rho, void *V, 
         const bool stale = q == 0 ? g.rho != rho : g.V != V;
         if (!stale) continue;
         const KernelEntry *e = pl->k[q];
-        PassParams &prm = q == 0 ? g.prm_f1 : g.prm_i1;
-        if (q == 0) prm.in = rho; else prm.out = V;
-        void *args[] = {&prm};
-        cudaKernelNodeParams kp{};
-        kp.func = const_cast<void *>(e->func);
-        kp.gridDim = dim3(pl->grid[q]); kp.blockDim = dim3(e->NT);
-        kp.sharedMemBytes = (unsigned)e->smem_bytes;
-        kp.kernelParams = args; kp.extra = nullptr;
-        PF_CUDA(cudaGraphExecKernelNodeSetParams(g.exec, q == 0 ? g.node_f1 : g.node_i1, &kp));   // launch attributes (PDL edges) stay as built
+        const int parts = g.xr > 1 ? g.xr : 1;
+        for (int r = 0; r < parts; ++r) {
+            PassParams &prm = g.xr > 1 ? (q == 0 ? g.prm_f1x[r] : g.prm_i1x[r]) : (q == 0 ? g.prm_f1 : g.prm_i1);
+            const long long off = g.xr > 1 ? (q == 0 ? g.off_rho[r] : g.off_V[r]) : 0;
+            if (q == 0) prm.in = static_cast<const char *>(rho) + off; else prm.out = static_cast<char *>(V) + off;
+            void *args[] = {&prm};
+            cudaKernelNodeParams kp{};
+            kp.func = const_cast<void *>(e->func);
+            kp.gridDim = dim3(prm.n_tiles < pl->grid[q] ? prm.n_tiles : pl->grid[q]); kp.blockDim = dim3(e->NT);
+            kp.sharedMemBytes = (unsigned)e->smem_bytes;
+            kp.kernelParams = args; kp.extra = nullptr;
+            const cudaGraphNode_t node = g.xr > 1 ? (q == 0 ? g.node_f1x[r] : g.node_i1x[r]) : (q == 0 ? g.node_f1 : g.node_i1);
+            PF_CUDA(cudaGraphExecKernelNodeSetParams(g.exec, node, &kp));   // launch attributes (PDL edges) stay as built
+        }
     }
     g.rho = rho; g.V = V;
     PF_CUDA(cudaGraphLaunch(g.exec, st));
@@ -1048,23 +1223,49 @@ static int tune_plan(poisson_plan *pl) {
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { cudaGetLastError(); cleanup(); return POISSON_OK; }
     const bool modes[5][3] = {{false, false, false}, {true, false, false}, {false, true, false}, {false, false, true}, {true, false, true}};   // {pdl, fused, graph}
     int best = 0; float best_ms = 1e30f;
-    if (build_graph(pl, pl->gs, nullptr) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }      // no graph: that mode is skipped
-    if (build_graph_pdl(pl, pl->gs_pdl, nullptr) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }
-    for (int m = 0; m < 5 && rc == POISSON_OK; ++m) {
-        if (modes[m][1] && !pl->fused) continue;
-        if (modes[m][2] && !(modes[m][0] ? pl->gs_pdl.exec : pl->gs.exec)) continue;
-        pl->use_pdl = modes[m][0]; pl->use_fused = modes[m][1]; pl->use_graph = modes[m][2];
+    // ms per solve of the launch mode currently set in the plan (0: failed)
+    auto time_mode = [&]() -> float {
         int reps = 3;
+        float ms = 0.f;
         for (int round = 0; round < 2 && rc == POISSON_OK; ++round) {   // round 0: warm-up + pick the repeat count
             cudaEventRecord(e0, ts);
             for (int i = 0; i < reps && rc == POISSON_OK; ++i) rc = run_solve(pl, rho, V, ts);
             cudaEventRecord(e1, ts);
-            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = cuda_fail(cudaGetLastError(), "tuning solve"); break; }
-            float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = cuda_fail(cudaGetLastError(), "tuning solve"); return 0.f; }
+            cudaEventElapsedTime(&ms, e0, e1);
             ms /= (float)reps;
             if (round == 0) { reps = (int)(2.0f / (ms > 1e-4f ? ms : 1e-4f)); reps = reps < 3 ? 3 : (reps > 64 ? 64 : reps); }
-            else { pl->tune_ms[m] = ms; if (ms < best_ms) { best_ms = ms; best = m; } }
         }
+        return ms;
+    };
+    // Graph shape: {chains over ranges of k_a planes, chains over ranges of x} (build_graph).  Which shape wins depends on the
+    // grid (measured on B200: 128^3 -> 256^3 fp64 98.4 us plain, 92.3 with 4 plane chains, 90.6 with 2 x 2; 32^3 -> 64^3
+    // loses 2 us with any), so the shapes are timed like the launch modes; POISSON_BRANCHES / POISSON_XCHAINS fix one.
+    static const int shapes[][2] = {{1, 1}, {2, 1}, {4, 1}, {2, 2}, {2, 4}};
+    int shape_best[2] = {pl->branches, pl->xchains};
+    if (!pl->env_shape && pl->n_chunks <= 1) {
+        float sb = 1e30f;
+        pl->use_pdl = false; pl->use_fused = false; pl->use_graph = true;
+        for (const auto &sh : shapes) {
+            if (rc != POISSON_OK) break;
+            destroy_graph(pl->gs);
+            pl->branches = sh[0]; pl->xchains = sh[1];
+            if (build_graph(pl, pl->gs, nullptr) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); continue; }
+            if (sh[1] > 1 && pl->gs.xr <= 1) continue;   // x chains do not apply to this plan: same graph as {sh[0], 1}
+            const float ms = time_mode();
+            if (rc == POISSON_OK && ms > 0.f && ms < 0.995f * sb) { sb = ms; shape_best[0] = sh[0]; shape_best[1] = sh[1]; }
+        }
+        destroy_graph(pl->gs);
+        pl->branches = shape_best[0]; pl->xchains = shape_best[1];
+    }
+    if (rc == POISSON_OK && build_graph(pl, pl->gs, nullptr) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }      // no graph: that mode is skipped
+    if (rc == POISSON_OK && build_graph_pdl(pl, pl->gs_pdl, nullptr) != POISSON_OK) { cudaGetLastError(); g_last_error.clear(); }
+    for (int m = 0; m < 5 && rc == POISSON_OK; ++m) {
+        if (modes[m][1] && !pl->fused) continue;
+        if (modes[m][2] && !(modes[m][0] ? pl->gs_pdl.exec : pl->gs.exec)) continue;
+        pl->use_pdl = modes[m][0]; pl->use_fused = modes[m][1]; pl->use_graph = modes[m][2];
+        const float ms = time_mode();
+        if (rc == POISSON_OK) { pl->tune_ms[m] = ms; if (ms < 0.99f * best_ms) { best_ms = ms; best = m; } }   // a later mode must win by more than the timing noise
     }
     pl->use_pdl = modes[best][0]; pl->use_fused = modes[best][1]; pl->use_graph = modes[best][2];
     cleanup();

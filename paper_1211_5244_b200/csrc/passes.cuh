@@ -107,6 +107,8 @@ struct PassParams {
     int tiles_per_g;   // ceil(n_p / P)
     int n_tiles;       // n_g * tiles_per_g
     int late_tw;       // 1: build the twiddle tables after the first tile's loads have been issued (else before: the PDL order)
+    int pdl_trigger;   // programmatic dependent launch: 0 = the next pass may launch from the start of this one, 1 = once this CTA is
+                       // past its last tile's loads, 2 = only when this pass exits (the implicit trigger)
     int k_g0;          // F3 of a plane chunk: first plane of the chunk (K^F is indexed by the plane's position in the whole grid)
     int prefetch;      // bit 0: prefetch the next tile's inputs into L2 (unstaged tile loops); bit 1: F3 prefetches its K^F lines
     // several densities per launch (small grids, poisson_solve_batch): tile = bi * n_tiles1 + tile of density bi
@@ -476,7 +478,7 @@ PF_HD void stage_issue(cx<typename G::T> *stage, const cx<typename G::T> *src, l
 // WAITN = copy groups that may still be pending when a tile's inputs are needed.
 struct NoPrefetch { PF_HD void operator()(int) const {} };
 template <class G, class Buf, bool STAGED, int WAITN, class Issue, class After, class Fetch, class Process, class Pf = NoPrefetch>
-PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_first, Fetch &&fetch, Process &&process,
+PF_HD void tile_loop(int bid, int nb, int n_tiles, bool trig_late, Issue &&issue, After &&after_first, Fetch &&fetch, Process &&process,
                      Pf &&prefetch_next = Pf()) {
     if constexpr (STAGED) {
         int tile = bid;
@@ -490,6 +492,7 @@ PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_
             fetch(cur, tile);
             G::xsync();                       // stage free again
             if (tile + nb < n_tiles) issue(tile + nb);
+            else if (trig_late) pdl_launch_dependents();   // last tile of this CTA: its inputs are in registers
             cp_async_commit();
             process(cur, tile);
         }
@@ -502,6 +505,7 @@ PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_
             Buf nxt;
             const bool more = tile + nb < n_tiles;
             if (more) fetch(nxt, tile + nb);
+            else if (trig_late) pdl_launch_dependents();
             process(cur, tile);
             if (more) cur = nxt;
         }
@@ -512,16 +516,18 @@ PF_HD void tile_loop(int bid, int nb, int n_tiles, Issue &&issue, After &&after_
             fetch(cur, tile);
             if (first) { after_first(); first = false; }           // the first tile's loads are in flight: run the hook under them
             if (tile + nb < n_tiles) prefetch_next(tile + nb);   // unstaged: at least start the next tile DRAM -> L2
+            else if (trig_late) pdl_launch_dependents();         // last tile of this CTA: its loads have been issued
             process(cur, tile);
         }
         if (first) after_first();
+        if (trig_late && bid >= n_tiles) pdl_launch_dependents();
     }
 }
 
 // Exchange buffer as the stage: process(buf, tile, after_read) calls after_read() once the thread has read its last
 // exchange value of the tile; a barrier later the buffer is idle and takes the next tile's copies.
 template <class G, class Buf, class Issue, class After, class Fetch, class Process>
-PF_HD void tile_loop_x(int bid, int nb, int n_tiles, Issue &&issue, After &&after_first, Fetch &&fetch, Process &&process) {
+PF_HD void tile_loop_x(int bid, int nb, int n_tiles, bool trig_late, Issue &&issue, After &&after_first, Fetch &&fetch, Process &&process) {
     int tile = bid;
     if (tile < n_tiles) issue(tile);
     cp_async_commit();
@@ -532,6 +538,7 @@ PF_HD void tile_loop_x(int bid, int nb, int n_tiles, Issue &&issue, After &&afte
         G::xsync();                       // every copy of the scope has landed
         fetch(cur, tile);
         G::xsync();                       // buffer free: the transform may write it
+        if (trig_late && tile + nb >= n_tiles) pdl_launch_dependents();
         process(cur, tile, [&] {
             G::xsync();                   // every thread of the scope is done reading the exchange
             if (tile + nb < n_tiles) issue(tile + nb);
@@ -776,7 +783,7 @@ PF_HD void process_i1(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c
     cx<T> *stage = smem_c + G::NBUF * G::XELEMS + G::tw_elems(KIND);                                       \
     const unsigned long long pol = (St::ON || St::XON) ? evict_first_policy() : 0ull;                              \
     (void)stage; (void)pol; (void)t; (void)p;                                               \
-    pdl_launch_dependents();                                                                          \
+    if (prm.pdl_trigger == 0) pdl_launch_dependents();                                                \
     auto init_tw = [&] { c.tw.template init<NEED_A, NEED_B>(reinterpret_cast<const cx<T> *>(prm.tw), smem_c + G::NBUF * G::XELEMS, tid, c.t); }; \
     if (!prm.late_tw) init_tw();           /* tables first, then wait for the previous pass (the PDL order) */ \
     pdl_wait_prior_grid();                                                                            \
@@ -786,7 +793,7 @@ template <class G, bool PRUNED>
 PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     PF_BODY_PROLOGUE(true, false, KIND_F2)
     using Buf = BufA<G, PRUNED>;
-    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
+    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles, prm.pdl_trigger == 1,
         [&](int tile) {
             PF_TILE_COORDS
             stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
@@ -811,7 +818,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     PF_BODY_PROLOGUE(false, true, KIND_I2)
     using Buf = BufB<G>;
     if constexpr (St::XON) {   // the exchange buffer doubles as the stage
-        tile_loop_x<G, Buf>(bid, nb, prm.n_tiles,
+        tile_loop_x<G, Buf>(bid, nb, prm.n_tiles, prm.pdl_trigger == 1,
             [&](int tile) {
                 PF_TILE_COORDS
                 stage_issue<G, St, true, true>(smem_c, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
@@ -840,7 +847,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             });
         return;
     }
-    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
+    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles, prm.pdl_trigger == 1,
         [&](int tile) {
             PF_TILE_COORDS
             stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);  // last read of A2
@@ -886,7 +893,7 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1 + prm.k_g0 * prm.tiles_per_g) * NKV * G::NT + tid;
         static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; cp_async_vec16(kstage + q * G::NT + tid, kp + (size_t)q * G::NT, pol); });
     };
-    tile_loop<G, Buf, St::ON, (St::KON ? 1 : 0)>(bid, nb, prm.n_tiles,
+    tile_loop<G, Buf, St::ON, (St::KON ? 1 : 0)>(bid, nb, prm.n_tiles, prm.pdl_trigger == 1,
         [&](int tile) {
             PF_TILE_COORDS
             stage_issue<G, St, false>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
@@ -928,7 +935,7 @@ template <class G, bool PRUNED>
 PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     PF_BODY_PROLOGUE(true, false, KIND_F1)
     using Buf = BufA<G, PRUNED>;
-    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
+    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles, prm.pdl_trigger == 1,
         [&](int tile) {
             PF_TILE_COORDS
             stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + p0 * prm.ps_in, prm.ns_in, prm.ps_in, prm.n_p - p0, tid, pol);
@@ -953,7 +960,7 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     PF_BODY_PROLOGUE(false, true, KIND_I1)
     using Buf = BufB<G>;
     if constexpr (St::XON) {   // the exchange buffer doubles as the stage
-        tile_loop_x<G, Buf>(bid, nb, prm.n_tiles,
+        tile_loop_x<G, Buf>(bid, nb, prm.n_tiles, prm.pdl_trigger == 1,
             [&](int tile) {
                 PF_TILE_COORDS
                 stage_issue<G, St, true, true>(smem_c, pass_in<T>(prm, bi) + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);
@@ -969,7 +976,7 @@ PF_HD void body_i1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             });
         return;
     }
-    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles,
+    tile_loop<G, Buf, St::ON, 0>(bid, nb, prm.n_tiles, prm.pdl_trigger == 1,
         [&](int tile) {
             PF_TILE_COORDS   // stage rows: kk = 0..S/2, columns: the 2 P complex pencils of the P pairs
             stage_issue<G, St, true>(stage, pass_in<T>(prm, bi) + g * prm.gs_in + 2 * p0 * prm.ps_in, prm.ns_in, prm.ps_in, 2 * (prm.n_p - p0), tid, pol);

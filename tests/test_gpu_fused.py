@@ -47,7 +47,8 @@ def _solve(pk, rho, Kf, n, bc, prec, fused, repeats=1):
         else:
             os.environ["POISSON_FUSED"] = old
     try:
-        assert plan.launches_per_solve() == (1 if fused else 5)
+        J, R = plan.graph_shape()      # the tuner may keep a shaped graph (parallel chains) when not fused
+        assert plan.launches_per_solve() == (1 if fused else (5 if (J, R) == (1, 1) else 2 * R + 2 * R * J + J))
         plan.set_kernel(torch.from_numpy(np.ascontiguousarray(Kf.astype(dt))).cuda())
         r = torch.from_numpy(np.ascontiguousarray(rho.astype(dt))).cuda()
         outs = []
@@ -233,3 +234,89 @@ def test_every_launch_mode_all_bc_vs_oracle(pk, monkeypatch, n, mode):
         assert np.array_equal(V1, V2)
         assert rel_l2(V1, oracle.solve(rho, Kf, bc)) <= 1e-12, (n, bc, mode)
     print(n, mode, "modes used:", sorted(used))
+
+
+SHAPES = [(2, 1), (3, 1), (4, 1), (1, 2), (2, 2), (2, 4), (3, 2)]
+
+
+@pytest.mark.parametrize("pdl", [False, True], ids=["graph", "graph_pdl"])
+@pytest.mark.parametrize("shape", SHAPES, ids=lambda s: f"J{s[0]}R{s[1]}")
+def test_shaped_graph_bitwise_and_vs_oracle(pk, monkeypatch, shape, pdl):
+    """The solve graph as parallel chains (poisson_plan_graph_shape: J ranges of k_a planes, R ranges of x), FORCED with
+    POISSON_BRANCHES / POISSON_XCHAINS: same kernels on the same tiles, so the result is bitwise the five stream launches';
+    it is also compared with the oracle.  Grids: x last-processed with whole tiles per x range (R applies), surface
+    boundary conditions and an odd N_x (R must fall back to 1), rho / V changing between calls, rho == V, another stream."""
+    import torch
+    J, R = shape
+    # x ranges need whole tiles: 128 x values = 4 ranges of 2 P = 32 reals in F1 / I1 (S = 64: 8 threads per pencil, P = 16)
+    cases = [((128, 32, 32), (0, 0, 0), True), ((128, 32, 64), (0, 0, 1), True), ((32, 24, 16), (1, 1, 0), False), ((15, 12, 10), (0, 1, 0), False)]
+    for n, bc, x_ok in cases:
+        rng = np.random.default_rng(77 + sum(n) + J + 10 * R)
+        s = gen.padded_shape(n, bc)
+        Kf_np = oracle.kernel_spectrum(_even_kernel(rng, s))
+        rhos_np = [rng.standard_normal((n[2], n[1], n[0])) for _ in range(3)]
+        Kf = torch.from_numpy(Kf_np).cuda()
+        rhos = [torch.from_numpy(r).cuda() for r in rhos_np]
+        for k in ("POISSON_GRAPH", "POISSON_PDL", "POISSON_BRANCHES", "POISSON_XCHAINS"):
+            monkeypatch.delenv(k, raising=False)
+        monkeypatch.setenv("POISSON_TUNE", "0")
+        ref_plan = pk.PoissonPlan(n, bc, 0.3, pk.FP64)
+        ref_plan.set_kernel(Kf)
+        assert ref_plan.launch_mode()[0] == "five" and ref_plan.graph_shape() == (1, 1)
+        refs = [ref_plan.solve(r).clone() for r in rhos]
+        ref_plan.close()
+        monkeypatch.setenv("POISSON_GRAPH", "1")
+        monkeypatch.setenv("POISSON_BRANCHES", str(J))
+        monkeypatch.setenv("POISSON_XCHAINS", str(R))
+        if pdl:
+            monkeypatch.setenv("POISSON_PDL", "1")
+        plan = pk.PoissonPlan(n, bc, 0.3, pk.FP64)
+        try:
+            plan.set_kernel(Kf)
+            assert plan.launch_mode()[0] == ("graph_pdl" if pdl else "graph")
+            want_r = R if x_ok else 1
+            assert plan.graph_shape() == (J, want_r), (n, bc, plan.graph_shape())
+            if J > 1 or want_r > 1:
+                assert plan.launches_per_solve() == 2 * want_r + 2 * want_r * J + J
+            outs = [torch.empty_like(r) for r in rhos]
+            for rep in range(2):
+                for r, o, ref in zip(rhos, outs, refs):
+                    plan.solve(r, o)
+                    assert torch.equal(o, ref), (n, bc, shape)
+            w = rhos[1].clone()
+            plan.solve(w, w)                                   # in place
+            assert torch.equal(w, refs[1])
+            s2 = torch.cuda.Stream()
+            with torch.cuda.stream(s2):
+                plan.solve(rhos[2], outs[0], stream=s2)
+            s2.synchronize()
+            assert torch.equal(outs[0], refs[2])
+            for v, ref in zip(plan.solve_batch(rhos), refs):   # the batch lanes keep plain chains
+                torch.cuda.synchronize()
+                assert torch.equal(v, ref)
+        finally:
+            plan.close()
+        assert rel_l2(refs[0].cpu().numpy(), oracle.solve(rhos_np[0], Kf_np, bc)) <= 1e-12
+
+
+def test_tuner_reports_graph_shape(pk):
+    """poisson_plan_create times a few graph shapes with the launch modes; whatever it keeps is reported consistently."""
+    import torch
+    plan = pk.PoissonPlan((64, 64, 64), (0, 0, 0), 0.2, pk.FP64)
+    try:
+        mode, ms = plan.launch_mode()
+        J, R = plan.graph_shape()
+        print("launch mode", mode, "graph shape", (J, R), ms)
+        assert J >= 1 and R >= 1
+        if mode not in ("graph", "graph_pdl"):
+            assert (J, R) == (1, 1)
+        if (J, R) != (1, 1):
+            assert plan.launches_per_solve() == 2 * R + 2 * R * J + J
+        rng = np.random.default_rng(5)
+        Kf = oracle.kernel_spectrum(_even_kernel(rng, (128, 128, 128)))
+        rho = rng.standard_normal((64, 64, 64))
+        plan.set_kernel(torch.from_numpy(Kf).cuda())
+        V = plan.solve(torch.from_numpy(rho).cuda()).cpu().numpy()
+    finally:
+        plan.close()
+    assert rel_l2(V, oracle.solve(rho, Kf, (0, 0, 0))) <= 1e-12

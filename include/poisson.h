@@ -241,6 +241,61 @@ POISSON_API int poisson_measure_fma_peak(int precision, double *tflops /* host, 
 POISSON_API size_t poisson_plan_workspace_bytes(const poisson_plan *plan);
 POISSON_API int poisson_plan_destroy(poisson_plan *plan);
 
+/* ---- One solve sharded over several GPUs.
+ * The paper's transposes act on the reduced data set and it names direct GPU-to-GPU transfers as the way to
+ * scale.  Here rho / V are distributed in slabs along the axis o (the non-x axis that is not the first
+ * processed axis a: y for fully free / wire / periodic grids, z for the surface grid).  F1 transforms axis a on a rank's own
+ * slab; the half spectrum then changes hands ONCE per direction, on the smallest intermediate of the pipeline (A1:
+ * H x N_o x N_x complex, 33.8 MB for 128^3 -> 256^3 against 67.6 MB for A2):
+ *     F1 (own slab of o)  --stores-->  every rank's plane slab  [k_a in its range][all o][x]        exchange 1
+ *     F2, F3, I2 on the rank's own k_a planes (its share of K^F only)
+ *     I2                  --stores-->  every rank's slab        [all k_a][its range of o][x]         exchange 2
+ *     I1 (own slab of o)  ->  V
+ * The exchanges are not separate copies or collectives: passes F1 and I2 store every element straight into the slab of
+ * the GPU that owns it, through peer-mapped pointers (NVLink / NVSwitch peer memory), so the transfer overlaps the
+ * transform tile by tile.  The caller provides the slabs (memory every peer can address: CUDA IPC / VMM / symmetric
+ * memory; on one GPU any device memory) and the two cross-rank barriers:
+ *     poisson_shard_forward(rho)  |  barrier A (all ranks' forward done)  |  poisson_shard_middle
+ *                                 |  barrier B (all ranks' middle done)   |  poisson_shard_inverse(V)
+ * each barrier ordered on `stream` (e.g. a one-element NCCL all-reduce enqueued on it).  Barrier B also protects the
+ * next solve: its forward overwrites the plane slabs the middle pass has consumed by then, and its middle pass
+ * overwrites the slabs pass I1 reads only after the next barrier A, which every rank enqueues after its own I1.
+ * Partition: rank s of R owns [floor(T s / R), floor(T (s + 1) / R)) of T = N_o points resp. T = H planes.
+ * Supported: grids whose five passes all run the compiled register-engine kernels, even N_x, R <= min(N_o, H, 32);
+ * else POISSON_EUNSUPPORTED.  Results are bitwise those of poisson_solve (same kernels, same arithmetic per pencil). */
+typedef struct poisson_shard_info {
+    int rank, nranks;
+    int split_axis;         /* o: rho / V are distributed along this axis (1 = y, 2 = z)                          */
+    int plane_axis;         /* a: between the exchanges the half spectrum k_a = 0 .. H-1 of this axis is distributed */
+    int o0, o1;             /* this rank's slab: o0 <= o < o1                                                       */
+    int k0, k1;             /* its planes: k0 <= k_a < k1                                                           */
+    long long local_dims[3];   /* shape of the rank's rho / V, C order [z][y][x]                                    */
+    long long mid_dims[3];     /* shape of its exchange slab 1 (complex), C order: A1 with axis a -> k1 - k0        */
+    long long back_dims[3];    /* shape of its exchange slab 2 (complex), C order: A1 with axis o -> o1 - o0        */
+    long long mid_bytes, back_bytes;   /* sizes of the two slabs the caller must provide for this rank              */
+    long long sent_bytes[2];   /* bytes this rank stores into OTHER ranks' slabs in exchange 1 / exchange 2          */
+    long long workspace_bytes; /* device memory the plan itself owns (A2 of its planes, its share of K^F, tables)   */
+} poisson_shard_info;
+
+/* Planner only (no device needed).  Errors: EINVAL, EUNSUPPORTED. */
+POISSON_API int poisson_shard_describe(int nx, int ny, int nz, const int bc[3], int precision, int rank, int nranks,
+                                       poisson_shard_info *info /* host, out */);
+/* Plan of rank `rank` of `nranks` for the GLOBAL grid nx, ny, nz on the current device.  A shard plan only takes the
+ * poisson_shard_* calls (plus poisson_plan_kernel_dims / _destroy); poisson_solve on it returns EINVAL. */
+POISSON_API int poisson_shard_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc[3], double h, int precision,
+                                          int rank, int nranks);
+POISSON_API int poisson_shard_get_info(const poisson_plan *plan, poisson_shard_info *info /* host, out */);
+/* mid_of_rank[s] / back_of_rank[s]: device pointers, valid on THIS device, to rank s's exchange slabs (host arrays of
+ * nranks pointers; entry [rank] is the rank's own slab).  16-byte aligned.  The plan keeps the pointers, not the memory. */
+POISSON_API int poisson_shard_set_slabs(poisson_plan *plan, void *const *mid_of_rank /* host */, void *const *back_of_rank /* host */);
+/* K_f_dev: the WHOLE spectrum [S_z][S_y][S_x/2+1] as for poisson_set_kernel; only the rank's planes are kept. */
+POISSON_API int poisson_shard_set_kernel(poisson_plan *plan, const void *K_f_dev, void *stream);
+/* The three stages of one sharded solve (asynchronous on `stream`; the caller enqueues the barriers between them).
+ * rho_local_dev / V_local_dev: the rank's slab, plan precision, C order local_dims.  Errors: EINVAL, ENOKERNEL, ECUDA. */
+POISSON_API int poisson_shard_forward(poisson_plan *plan, const void *rho_local_dev, void *stream);
+POISSON_API int poisson_shard_middle(poisson_plan *plan, void *stream);
+POISSON_API int poisson_shard_inverse(poisson_plan *plan, void *V_local_dev, void *stream);
+
 POISSON_API const char *poisson_status_string(int status);
 /* Text of the last CUDA error seen by this thread's most recent failing call ("" if none). */
 POISSON_API const char *poisson_last_error(void);

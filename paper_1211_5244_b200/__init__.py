@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "poisson_plan_describe", "poisson_plan_create", "poisson_plan_kernel_dims", "poisson_plan_get_info",
     "poisson_set_kernel", "poisson_set_kernel_complex", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
     "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_measure_fma_peak", "poisson_plan_workspace_bytes",
-    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_plan_graph_shape", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes", "poisson_plan_batch_width",
+    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_plan_graph_shape", "poisson_shard_describe", "poisson_shard_plan_create", "poisson_shard_get_info", "poisson_shard_set_slabs", "poisson_shard_set_kernel", "poisson_shard_forward", "poisson_shard_middle", "poisson_shard_inverse", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes", "poisson_plan_batch_width",
 )
 
 _PKG = Path(__file__).resolve().parent
@@ -55,6 +55,20 @@ class PlanInfo(ctypes.Structure):
             "length": list(self.length), "bytes": list(self.bytes), "bytes_total": self.bytes_total,
             "workspace_bytes": self.workspace_bytes, "fft_fraction": self.fft_fraction,
         }
+
+
+class ShardInfo(ctypes.Structure):
+    """Mirror of `poisson_shard_info` (include/poisson.h)."""
+    _fields_ = [
+        ("rank", ctypes.c_int), ("nranks", ctypes.c_int), ("split_axis", ctypes.c_int), ("plane_axis", ctypes.c_int),
+        ("o0", ctypes.c_int), ("o1", ctypes.c_int), ("k0", ctypes.c_int), ("k1", ctypes.c_int),
+        ("local_dims", ctypes.c_longlong * 3), ("mid_dims", ctypes.c_longlong * 3), ("back_dims", ctypes.c_longlong * 3),
+        ("mid_bytes", ctypes.c_longlong), ("back_bytes", ctypes.c_longlong), ("sent_bytes", ctypes.c_longlong * 2),
+        ("workspace_bytes", ctypes.c_longlong),
+    ]
+
+    def as_dict(self):
+        return {k: (list(getattr(self, k)) if hasattr(getattr(self, k), "__len__") else getattr(self, k)) for k, _ in self._fields_}
 
 
 def lib_path() -> Path:
@@ -94,6 +108,14 @@ def load_library():
     lib.poisson_solve_batch_host.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), i, vp]
     lib.poisson_plan_launch_mode.argtypes = [vp, ctypes.POINTER(i), ctypes.c_double * 5]
     lib.poisson_plan_graph_shape.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i)]
+    lib.poisson_shard_describe.argtypes = [i, i, i, i3, i, i, i, ctypes.POINTER(ShardInfo)]
+    lib.poisson_shard_plan_create.argtypes = [ctypes.POINTER(vp), i, i, i, i3, ctypes.c_double, i, i, i]
+    lib.poisson_shard_get_info.argtypes = [vp, ctypes.POINTER(ShardInfo)]
+    lib.poisson_shard_set_slabs.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp)]
+    lib.poisson_shard_set_kernel.argtypes = [vp, vp, vp]
+    lib.poisson_shard_forward.argtypes = [vp, vp, vp]
+    lib.poisson_shard_middle.argtypes = [vp, vp]
+    lib.poisson_shard_inverse.argtypes = [vp, vp, vp]
     lib.poisson_plan_workspace_bytes.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.restype = ctypes.c_size_t
     lib.poisson_plan_destroy.argtypes = [vp]
@@ -154,6 +176,13 @@ def poisson_measure_fma_peak(precision: int = FP64) -> float:
 
 def poisson_plan_destroy(plan: int) -> None:
     _check(load_library().poisson_plan_destroy(plan), "poisson_plan_destroy")
+
+
+def poisson_shard_describe(nx: int, ny: int, nz: int, bc, precision: int, rank: int, nranks: int) -> ShardInfo:
+    info = ShardInfo()
+    _check(load_library().poisson_shard_describe(nx, ny, nz, (ctypes.c_int * 3)(*bc), precision, rank, nranks, ctypes.byref(info)),
+           "poisson_shard_describe")
+    return info
 
 
 # ------------------------------------------------------------------ small convenience wrapper over torch tensors
@@ -318,3 +347,114 @@ class PoissonPlan:
             self.close()
         except Exception:
             pass
+
+
+class ShardPlan:
+    """One rank of a solve sharded over several GPUs (include/poisson.h: poisson_shard_*).  Marshalling only: the caller
+    owns the exchange slabs and enqueues the two cross-rank barriers (see ShardedSolver for the torch.distributed plumbing)."""
+
+    def __init__(self, n, bc, h: float, precision: int, rank: int, nranks: int):
+        self.n = tuple(int(v) for v in n)
+        self.bc = tuple(int(v) for v in bc)
+        self.precision = precision
+        handle = ctypes.c_void_p()
+        _check(load_library().poisson_shard_plan_create(ctypes.byref(handle), self.n[0], self.n[1], self.n[2], (ctypes.c_int * 3)(*self.bc),
+                                                        float(h), precision, rank, nranks), "poisson_shard_plan_create")
+        self._h = handle.value
+        self.info = ShardInfo()
+        _check(load_library().poisson_shard_get_info(self._h, ctypes.byref(self.info)), "poisson_shard_get_info")
+        dims = (ctypes.c_longlong * 3)()
+        _check(load_library().poisson_plan_kernel_dims(self._h, dims), "poisson_plan_kernel_dims")
+        self.kernel_dims = tuple(dims)
+        self._keep = None
+
+    @property
+    def local_shape(self):
+        return tuple(self.info.local_dims)
+
+    def set_slabs(self, mid_ptrs, back_ptrs, keep=None):
+        """mid_ptrs / back_ptrs: one device pointer per rank (as THIS device addresses that rank's slab)."""
+        n = self.info.nranks
+        assert len(mid_ptrs) == n and len(back_ptrs) == n
+        m = (ctypes.c_void_p * n)(*[int(p) for p in mid_ptrs])
+        b = (ctypes.c_void_p * n)(*[int(p) for p in back_ptrs])
+        _check(load_library().poisson_shard_set_slabs(self._h, m, b), "poisson_shard_set_slabs")
+        self._keep = keep     # whatever owns the memory
+
+    def set_kernel(self, K_f, stream=None):
+        assert K_f.is_cuda and K_f.is_contiguous() and tuple(K_f.shape) == self.kernel_dims
+        _check(load_library().poisson_shard_set_kernel(self._h, K_f.data_ptr(), PoissonPlan._stream(stream)), "poisson_shard_set_kernel")
+
+    def forward(self, rho_local, stream=None):
+        assert rho_local.is_cuda and rho_local.is_contiguous() and tuple(rho_local.shape) == self.local_shape
+        _check(load_library().poisson_shard_forward(self._h, rho_local.data_ptr(), PoissonPlan._stream(stream)), "poisson_shard_forward")
+
+    def middle(self, stream=None):
+        _check(load_library().poisson_shard_middle(self._h, PoissonPlan._stream(stream)), "poisson_shard_middle")
+
+    def inverse(self, V_local, stream=None):
+        assert V_local.is_cuda and V_local.is_contiguous() and tuple(V_local.shape) == self.local_shape
+        _check(load_library().poisson_shard_inverse(self._h, V_local.data_ptr(), PoissonPlan._stream(stream)), "poisson_shard_inverse")
+
+    def close(self):
+        if self._h:
+            poisson_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class ShardedSolver:
+    """One solve over the GPUs of a torch.distributed process group (one process per GPU, NCCL): this rank's ShardPlan, its two
+    exchange slabs in symmetric memory (every peer's slab mapped into this process over NVLink), and the two barriers as
+    one-element all-reduces on the compute stream.  torch supplies memory, peer mapping and the barrier; every step of the
+    path runs in the library's kernels, which store straight into the peers' slabs."""
+
+    def __init__(self, n, bc, h: float, precision: int = FP64, group=None):
+        import torch
+        import torch.distributed as dist
+        self.group = group
+        self.rank = dist.get_rank(group) if dist.is_initialized() else 0
+        self.world = dist.get_world_size(group) if dist.is_initialized() else 1
+        self.plan = ShardPlan(n, bc, h, precision, self.rank, self.world)
+        info = self.plan.info
+        if self.world == 1:
+            self._mid = torch.empty(info.mid_bytes, dtype=torch.uint8, device="cuda")
+            self._back = torch.empty(info.back_bytes, dtype=torch.uint8, device="cuda")
+            mids, backs = [self._mid.data_ptr()], [self._back.data_ptr()]
+        else:
+            import torch.distributed._symmetric_memory as symm
+            # symmetric allocations have one size on every rank: the largest slab of any rank
+            sizes = torch.tensor([info.mid_bytes, info.back_bytes], dtype=torch.int64, device="cuda")
+            dist.all_reduce(sizes, op=dist.ReduceOp.MAX, group=group)
+            mid_b, back_b = (int(v) for v in sizes.tolist())
+            gname = (group or dist.group.WORLD).group_name
+            self._mid = symm.empty(mid_b, dtype=torch.uint8, device="cuda")
+            self._back = symm.empty(back_b, dtype=torch.uint8, device="cuda")
+            hm, hb = symm.rendezvous(self._mid, gname), symm.rendezvous(self._back, gname)
+            mids, backs = list(hm.buffer_ptrs), list(hb.buffer_ptrs)
+        self.plan.set_slabs(mids, backs, keep=(self._mid, self._back))
+        self._flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+
+    def _barrier(self):
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.all_reduce(self._flag, group=self.group)     # stream-ordered: enqueued on the current stream
+
+    def set_kernel(self, K_f):
+        self.plan.set_kernel(K_f)
+
+    def solve(self, rho_local, V_local=None):
+        import torch
+        if V_local is None:
+            V_local = torch.empty_like(rho_local)
+        self.plan.forward(rho_local)
+        self._barrier()
+        self.plan.middle()
+        self._barrier()
+        self.plan.inverse(V_local)
+        return V_local

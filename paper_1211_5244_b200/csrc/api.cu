@@ -225,6 +225,9 @@ struct GraphSolve {
 };
 
 struct poisson_plan {
+    ShardDesc *shard;          // non-NULL: plan of one rank of a sharded solve (poisson_shard_*); only those calls apply
+    void *sh_mid[PF_MAX_WIDE], *sh_back[PF_MAX_WIDE];   // every rank's exchange slabs as this device addresses them
+    bool sh_slabs_set;
     PlanDesc d;
     double h;
     int device;
@@ -325,6 +328,7 @@ static void fill_bluestein(std::vector<unsigned char> &chirp, std::vector<unsign
 
 static void free_plan(poisson_plan *pl) {
     if (!pl) return;
+    delete pl->shard;
     cudaFree(pl->a1); cudaFree(pl->a2); cudaFree(pl->kint);
     for (int q = 0; q < 3; ++q) { cudaFree(pl->tw[q]); cudaFree(pl->chirp[q]); cudaFree(pl->bspec[q]); }
     cudaFree(pl->rho_stage); cudaFree(pl->v_stage); cudaFree(pl->fused_sync);
@@ -348,7 +352,11 @@ static void free_plan(poisson_plan *pl) {
     delete pl;
 }
 
-static int check_device(const poisson_plan *pl) {
+static int check_device(const poisson_plan *pl, bool want_shard = false) {
+    if ((pl->shard != nullptr) != want_shard) {
+        g_last_error = want_shard ? "not a shard plan (poisson_shard_plan_create)" : "a shard plan only takes the poisson_shard_* calls";
+        return POISSON_EINVAL;
+    }
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess || dev != pl->device) {
         cudaGetLastError();
@@ -719,6 +727,7 @@ static int relayout_kernel_spectrum(poisson_plan *pl, const void *K_f_dev, bool 
             generic_relayout_kernel<float><<<(int)blocks, threads, 0, st>>>(static_cast<const float *>(K_f_dev), static_cast<float *>(pl->kint), q);
     } else {
         RelayoutParams q;
+        q.g0 = pl->shard ? pl->shard->k0 : 0;
         q.RA = e->RA; q.RB = e->RB; q.TPP = e->TPP; q.P = e->P; q.V = e->V; q.NT = e->NT; q.lanes_p = e->lanes_p;
         q.tiles_per_g = pl->tiles_per_g[2]; q.n_p = (int)d.pass[2].n_p;
         q.a_axis = d.order[0]; q.c_axis = d.order[2];
@@ -1321,7 +1330,7 @@ int poisson_profile_read(poisson_plan *pl, double ms_sum[5], int *n_solves) {
 }
 
 int poisson_debug_run_passes(poisson_plan *pl, const void *rho_dev, void *V_dev, void *stream, int first, int last) {
-    if (!pl || first < 0 || last > 4 || first > last) return POISSON_EINVAL;
+    if (!pl || pl->shard || first < 0 || last > 4 || first > last) return POISSON_EINVAL;
     if (first == 0 && !rho_dev) return POISSON_EINVAL;
     if (last == 4 && !V_dev) return POISSON_EINVAL;
     if (first <= 2 && last >= 2 && !pl->kernel_set) return POISSON_ENOKERNEL;
@@ -1330,7 +1339,7 @@ int poisson_debug_run_passes(poisson_plan *pl, const void *rho_dev, void *V_dev,
 }
 
 int poisson_debug_workspace(const poisson_plan *pl, int which, void **ptr, long long dims[3]) {
-    if (!pl || !ptr || !dims || (which != 0 && which != 1)) return POISSON_EINVAL;
+    if (!pl || pl->shard || !ptr || !dims || (which != 0 && which != 1)) return POISSON_EINVAL;
     if (which == 1 && pl->n_chunks > 1) return POISSON_EUNSUPPORTED;   // chunked plan: A2 is never whole in memory
     const long long *ext = which == 0 ? pl->d.ext1 : pl->d.ext2;
     *ptr = which == 0 ? pl->a1 : pl->a2;
@@ -1512,6 +1521,208 @@ int poisson_solve_host(poisson_plan *pl, const void *rho_host, void *V_host, voi
     PF_CUDA(cudaMemcpyAsync(V_host, pl->v_stage, bytes, cudaMemcpyDeviceToHost, st));
     PF_CUDA(cudaStreamSynchronize(st));
     return POISSON_OK;
+}
+
+// ------------------------------------------------------------------ one solve sharded over several GPUs
+static void fill_shard_info(const PlanDesc &d, const ShardDesc &sh, poisson_shard_info *I) {
+    std::memset(I, 0, sizeof(*I));
+    const long long cplx = d.prec == POISSON_FP64 ? 16 : 8;
+    I->rank = sh.rank; I->nranks = sh.R; I->split_axis = sh.o; I->plane_axis = sh.a;
+    I->o0 = sh.o0; I->o1 = sh.o1; I->k0 = sh.k0; I->k1 = sh.k1;
+    for (int q = 0; q < 3; ++q) { I->local_dims[q] = sh.ext_rho[2 - q]; I->mid_dims[q] = sh.ext_mid[2 - q]; I->back_dims[q] = sh.ext_back[2 - q]; }
+    I->mid_bytes = sh.mid_elems * cplx; I->back_bytes = sh.back_elems * cplx;
+    // exchange 1: this rank's F1 output (H planes x its o slab x N_x) minus the planes it owns itself;
+    // exchange 2: its I2 output (its planes x all o x N_x) minus its own o slab
+    const long long no = sh.o1 - sh.o0, ng = sh.k1 - sh.k0, nx = d.ext1[0];
+    I->sent_bytes[0] = (d.H - ng) * no * nx * cplx;
+    I->sent_bytes[1] = ng * (d.n[sh.o] - no) * nx * cplx;
+}
+
+int poisson_shard_describe(int nx, int ny, int nz, const int bc[3], int precision, int rank, int nranks, poisson_shard_info *info) {
+    if (!info) return POISSON_EINVAL;
+    PlanDesc d;
+    int st = plan_build(nx, ny, nz, bc, precision, d);
+    if (st != POISSON_OK) return st;
+    ShardDesc sh;
+    st = shard_build(d, rank, nranks, sh);
+    if (st != POISSON_OK) return st;
+    static const int kinds[5] = {KIND_F1S, KIND_F2, KIND_F3, KIND_I2S, KIND_I1};
+    for (int q = 0; q < 5; ++q)
+        if (!find_kernel(kinds[q], sh.pass[q].S, sh.pass[q].pruned, sh.pass[q].lanes_p, precision, 0)) return POISSON_EUNSUPPORTED;
+    fill_shard_info(d, sh, info);
+    return POISSON_OK;
+}
+
+int poisson_shard_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc[3], double h, int precision, int rank, int nranks) {
+    if (!out) return POISSON_EINVAL;
+    *out = nullptr;
+    if (!(h > 0.0) || !std::isfinite(h)) return POISSON_EINVAL;
+    PlanDesc d;
+    int st = plan_build(nx, ny, nz, bc, precision, d);
+    if (st != POISSON_OK) return st;
+    ShardDesc sh;
+    st = shard_build(d, rank, nranks, sh);
+    if (st != POISSON_OK) return st;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); g_last_error = "no CUDA device"; return POISSON_EARCH; }
+    int dev = 0;
+    PF_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    PF_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) { g_last_error = "device is sm_" + std::to_string(prop.major * 10 + prop.minor) + ", kernels are sm_100a"; return POISSON_EARCH; }
+    poisson_plan *pl = new (std::nothrow) poisson_plan();
+    if (!pl) return POISSON_ENOMEM;
+    std::memset(static_cast<void *>(pl), 0, sizeof(*pl));
+    pl->shard = new (std::nothrow) ShardDesc(sh);
+    if (!pl->shard) { delete pl; return POISSON_ENOMEM; }
+    pl->d = d; pl->h = h; pl->device = dev; pl->num_sms = prop.multiProcessorCount;
+    pl->elem_real = precision == POISSON_FP64 ? 8 : 4;
+    pl->late_tw = 1; pl->pdl_trigger = 1; pl->branches = 1; pl->xchains = 1; pl->n_chunks = 1; pl->chunk_planes = d.H;
+    pl->env_lanes = pl->env_wide = -1;
+    for (int q = 0; q < 5; ++q) pl->pf_force[q] = -1;
+    pl->pf_min_bytes = (size_t)96 << 20;
+    static const int kinds[5] = {KIND_F1S, KIND_F2, KIND_F3, KIND_I2S, KIND_I1};
+    for (int q = 0; q < 5; ++q) {
+        const PassDesc &ps = sh.pass[q];
+        const KernelEntry *e = find_kernel(kinds[q], ps.S, ps.pruned, ps.lanes_p, precision, 0);
+        if (!e) { free_plan(pl); return POISSON_EUNSUPPORTED; }
+        pl->k[q] = e;
+        pl->tiles_per_g[q] = (int)((ps.n_p + e->P - 1) / e->P);
+        pl->n_tiles[q] = (int)(ps.n_g * pl->tiles_per_g[q]);
+        cudaError_t ce = cudaFuncSetAttribute(e->func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e->smem_bytes);
+        int occ = 0;
+        if (ce == cudaSuccess) ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, e->func, e->NT, e->smem_bytes);
+        if (ce != cudaSuccess || occ < 1) { free_plan(pl); return cuda_fail(ce, "shard kernel setup"); }
+        pl->resident[q] = occ * pl->num_sms;
+        pl->grid[q] = pl->n_tiles[q] < pl->resident[q] ? pl->n_tiles[q] : pl->resident[q];
+    }
+    const size_t cplx = 2 * pl->elem_real;
+    pl->a2_alloc_elems = sh.a2_elems;
+    pl->kint_elems = kint_reals(pl);
+    size_t ws = 0;
+    cudaError_t ce = cudaMalloc(&pl->a2, (size_t)sh.a2_elems * cplx); ws += (size_t)sh.a2_elems * cplx;
+    if (ce == cudaSuccess) { ce = cudaMalloc(&pl->kint, (size_t)pl->kint_elems * pl->elem_real); ws += (size_t)pl->kint_elems * pl->elem_real; }
+    for (int q = 0; q < 3 && ce == cudaSuccess; ++q) {
+        std::vector<unsigned char> host;
+        fill_twiddles(host, d.s[q], precision);
+        ce = cudaMalloc(&pl->tw[q], host.size());
+        if (ce == cudaSuccess) ce = cudaMemcpy(pl->tw[q], host.data(), host.size(), cudaMemcpyHostToDevice);
+        ws += host.size();
+    }
+    if (ce != cudaSuccess) {
+        free_plan(pl);
+        if (ce == cudaErrorMemoryAllocation) { cudaGetLastError(); return POISSON_ENOMEM; }
+        return cuda_fail(ce, "shard workspace allocation");
+    }
+    pl->workspace_bytes = ws;
+    pl->d.info.workspace_bytes = (long long)ws;
+    *out = pl;
+    return POISSON_OK;
+}
+
+int poisson_shard_get_info(const poisson_plan *pl, poisson_shard_info *info) {
+    if (!pl || !pl->shard || !info) return POISSON_EINVAL;
+    fill_shard_info(pl->d, *pl->shard, info);
+    info->workspace_bytes = (long long)pl->workspace_bytes;
+    return POISSON_OK;
+}
+
+int poisson_shard_set_slabs(poisson_plan *pl, void *const *mid_of_rank, void *const *back_of_rank) {
+    if (!pl || !pl->shard || !mid_of_rank || !back_of_rank) return POISSON_EINVAL;
+    for (int s = 0; s < pl->shard->R; ++s) {
+        if (!mid_of_rank[s] || !back_of_rank[s]) return POISSON_EINVAL;
+        if (reinterpret_cast<size_t>(mid_of_rank[s]) % 32 || reinterpret_cast<size_t>(back_of_rank[s]) % 32) return POISSON_EINVAL;   // 256-bit pair stores
+        pl->sh_mid[s] = mid_of_rank[s]; pl->sh_back[s] = back_of_rank[s];
+    }
+    pl->sh_slabs_set = true;
+    return POISSON_OK;
+}
+
+int poisson_shard_set_kernel(poisson_plan *pl, const void *K_f_dev, void *stream) {
+    if (!pl || !K_f_dev) return POISSON_EINVAL;
+    if (reinterpret_cast<size_t>(K_f_dev) % 16) return POISSON_EINVAL;
+    if (check_device(pl, true) != POISSON_OK) return POISSON_EINVAL;
+    const int rc = relayout_kernel_spectrum(pl, K_f_dev, false, reinterpret_cast<cudaStream_t>(stream));
+    if (rc != POISSON_OK) return rc;
+    pl->kernel_set = true;
+    return POISSON_OK;
+}
+
+// Parameters of pass q of a shard plan on the rank's local arrays.
+static PassParams shard_pass_params(const poisson_plan *pl, int q, const void *rho, void *V) {
+    const ShardDesc &sh = *pl->shard;
+    const PlanDesc &d = pl->d;
+    const PassDesc &ps = sh.pass[q];
+    PassParams prm{};
+    void *mid = pl->sh_mid[sh.rank], *back = pl->sh_back[sh.rank];
+    switch (q) {
+        case POISSON_PASS_F1: prm.in = rho; prm.out = nullptr; break;
+        case POISSON_PASS_F2: prm.in = mid; prm.out = pl->a2; break;
+        case POISSON_PASS_F3: prm.in = pl->a2; prm.out = pl->a2; break;
+        case POISSON_PASS_I2: prm.in = pl->a2; prm.out = nullptr; break;
+        default: prm.in = back; prm.out = V; break;
+    }
+    prm.kint = pl->kint;
+    prm.tw = pl->tw[ps.axis];
+    prm.gs_in = ps.gs_in; prm.ns_in = ps.ns_in; prm.ps_in = ps.ps_in;
+    prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;
+    prm.n_p = (int)ps.n_p; prm.tiles_per_g = pl->tiles_per_g[q]; prm.n_tiles = pl->n_tiles[q]; prm.n_tiles1 = pl->n_tiles[q];
+    prm.late_tw = 1; prm.pdl_trigger = 1;
+    prm.prefetch = q == POISSON_PASS_F3 && (size_t)pl->kint_elems * pl->elem_real >= pl->pf_min_bytes ? 2 : 0;
+    if (q == POISSON_PASS_F1 || q == POISSON_PASS_I2) {
+        const bool f1 = q == POISSON_PASS_F1;
+        const int T = f1 ? d.H : d.n[sh.o];                 // the distributed axis of the output: k_a planes resp. the split axis o
+        prm.sh_R = sh.R; prm.sh_total = T;
+        prm.sh_vslow = f1 ? (sh.a > sh.o) : (sh.o > sh.a);
+        prm.sh_nx = (int)d.ext1[0];
+        prm.sh_eu = f1 ? d.n[sh.o] : d.H;                    // whole extent of the other axis
+        prm.sh_u0 = f1 ? sh.o0 : sh.k0;
+        prm.sh_vp = (!f1 && d.order[1] == 0) ? 1 : 0;        // I2 along x: the split coordinate is the pencil index
+        for (int s = 0; s <= sh.R; ++s) prm.sh_lo[s] = shard_lo(T, s, sh.R);
+        for (int s = 0; s < sh.R; ++s) prm.blist[s] = f1 ? pl->sh_mid[s] : pl->sh_back[s];
+    }
+    return prm;
+}
+
+static int shard_launch(poisson_plan *pl, int q, const void *rho, void *V, cudaStream_t st) {
+    const KernelEntry *e = pl->k[q];
+    PassParams prm = shard_pass_params(pl, q, rho, V);
+    void *args[] = {&prm};
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(pl->grid[q]); cfg.blockDim = dim3(e->NT);
+    cfg.dynamicSmemBytes = e->smem_bytes; cfg.stream = st;
+    PF_CUDA(cudaLaunchKernelExC(&cfg, e->func, args));
+    return POISSON_OK;
+}
+
+static int shard_ready(const poisson_plan *pl) {
+    if (!pl) return POISSON_EINVAL;
+    if (check_device(pl, true) != POISSON_OK) return POISSON_EINVAL;
+    if (!pl->sh_slabs_set) { g_last_error = "poisson_shard_set_slabs has not been called"; return POISSON_EINVAL; }
+    return POISSON_OK;
+}
+
+int poisson_shard_forward(poisson_plan *pl, const void *rho_local_dev, void *stream) {
+    if (!rho_local_dev || reinterpret_cast<size_t>(rho_local_dev) % 16) return POISSON_EINVAL;
+    const int rc = shard_ready(pl);
+    if (rc != POISSON_OK) return rc;
+    return shard_launch(pl, POISSON_PASS_F1, rho_local_dev, nullptr, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int poisson_shard_middle(poisson_plan *pl, void *stream) {
+    int rc = shard_ready(pl);
+    if (rc != POISSON_OK) return rc;
+    if (!pl->kernel_set) return POISSON_ENOKERNEL;
+    for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2 && rc == POISSON_OK; ++q)
+        rc = shard_launch(pl, q, nullptr, nullptr, reinterpret_cast<cudaStream_t>(stream));
+    return rc;
+}
+
+int poisson_shard_inverse(poisson_plan *pl, void *V_local_dev, void *stream) {
+    if (!V_local_dev || reinterpret_cast<size_t>(V_local_dev) % 16) return POISSON_EINVAL;
+    const int rc = shard_ready(pl);
+    if (rc != POISSON_OK) return rc;
+    return shard_launch(pl, POISSON_PASS_I1, nullptr, V_local_dev, reinterpret_cast<cudaStream_t>(stream));
 }
 
 }  // extern "C"

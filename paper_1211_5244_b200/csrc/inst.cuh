@@ -16,6 +16,8 @@ __global__ void __launch_bounds__(G::NT, G::MINB) pass_kernel(const PassParams p
     else if constexpr (KIND == KIND_F2) body_f2<G, PRUNED>(prm, bid, nb, tid, pf_smem);
     else if constexpr (KIND == KIND_F3) body_f3<G, PRUNED>(prm, bid, nb, tid, pf_smem);
     else if constexpr (KIND == KIND_I2) body_i2<G, PRUNED>(prm, bid, nb, tid, pf_smem);
+    else if constexpr (KIND == KIND_F1S) body_f1<G, PRUNED, true>(prm, bid, nb, tid, pf_smem);
+    else if constexpr (KIND == KIND_I2S) body_i2<G, PRUNED, true>(prm, bid, nb, tid, pf_smem);
     else body_i1<G, PRUNED>(prm, bid, nb, tid, pf_smem);
 }
 
@@ -25,7 +27,7 @@ static void reg_one(int prec, int variant) {
     e.kind = KIND; e.S = G::S; e.pruned = PRUNED ? 1 : 0; e.lanes_p = G::LANES_P ? 1 : 0; e.prec = prec;
     e.variant = variant; e.nbuf = G::NBUF; e.tws = G::TWS ? 1 : 0; e.minb = G::MINB; e.stg = G::STG;
     e.RA = G::RA; e.RB = G::RB;
-    e.P = G::P; e.TPP = G::TPP; e.V = G::V; e.NT = G::NT; e.smem_bytes = pass_smem_bytes<G, PRUNED, KIND>();
+    e.P = G::P; e.TPP = G::TPP; e.V = G::V; e.NT = G::NT; e.smem_bytes = pass_smem_bytes<G, PRUNED, base_kind(KIND)>();
     e.func = reinterpret_cast<const void *>(&pass_kernel<G, PRUNED, KIND>);
     kernel_registry().push_back(e);
 }
@@ -56,6 +58,11 @@ static void reg_length(int prec, int variant) {
     reg_one<GC, true, KIND_F2>(prec, variant);  reg_one<GC, false, KIND_F2>(prec, variant);
     reg_one<GC, true, KIND_I2>(prec, variant);  reg_one<GC, false, KIND_I2>(prec, variant);
     reg_one<GC, true, KIND_F3>(prec, variant);  reg_one<GC, false, KIND_F3>(prec, variant);
+    if (variant == 0) {   // sharded single solve: F1 / I2 with their stores scattered over the peer GPUs (default geometry only)
+        reg_one<GP, true, KIND_F1S>(prec, variant);  reg_one<GP, false, KIND_F1S>(prec, variant);
+        reg_one<GP, true, KIND_I2S>(prec, variant);  reg_one<GP, false, KIND_I2S>(prec, variant);
+        reg_one<GC, true, KIND_I2S>(prec, variant);  reg_one<GC, false, KIND_I2S>(prec, variant);
+    }
 }
 
 }  // namespace pfft

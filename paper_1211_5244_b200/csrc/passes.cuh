@@ -31,7 +31,10 @@ namespace pfft {
 PF_HD void cta_sync() { __syncthreads(); }
 PF_HD void warp_sync() { __syncwarp(); }
 
-enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4 };
+enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4,
+                // sharded single solve: F1 / I2 whose stores go straight into the A1 slabs of the peer GPUs
+                KIND_F1S = 5, KIND_I2S = 6 };
+PF_CE int base_kind(int kind) { return kind == KIND_F1S ? KIND_F1 : (kind == KIND_I2S ? KIND_I2 : kind); }
 
 // ------------------------------------------------------------------ geometry
 // NBUF_   : exchange buffers (2 = one barrier per exchange, 1 = half the shared memory, one more barrier)
@@ -115,7 +118,15 @@ struct PassParams {
     int n_tiles1;      // tiles of ONE density (n_tiles = nb * n_tiles1; nb = 1 for a single solve)
     int use_list;      // 0: in/out + bi * bs_in/bs_out; 1: inputs are blist[bi] (F1: rho); 2: outputs are blist[bi] (I1: V)
     long long bs_in, bs_out;   // elements between the intermediates of consecutive densities
-    const void *blist[PF_MAX_WIDE];
+    const void *blist[PF_MAX_WIDE];   // sharded stores (sh_R > 1): base of every rank's destination slab instead
+    // sharded single solve: the output array is distributed over sh_R GPUs along a "varying" axis v (F1S: axis a, the planes
+    // k_a; I2S: the split axis o of rho / V, sh_total = T points in all), rank s owning a contiguous range of it; the other
+    // non-x axis u is whole on every rank.  Destination of element (v, u, x): blist[s] + vl * st_v + u * st_u + x with the
+    // strides of a dense [.][.][N_x] array (sh_vslow: v is the slower of the two axes in memory)
+    int sh_R, sh_total, sh_vslow, sh_nx, sh_eu;
+    int sh_lo[PF_MAX_WIDE + 1];   // rank s owns v in [sh_lo[s], sh_lo[s + 1]) = [floor(T s / R), floor(T (s + 1) / R))
+    int sh_u0;         // global u coordinate of this rank's first g (F1S: first o of its slab; I2S: first k_a plane it owns)
+    int sh_vp;         // I2S: 1 = the split coordinate v is the pencil index pp and x the transform index n, 0 = the reverse
     // any-length kernel only (generic_pass.cuh): transform length, pencils per tile, radices (product = gen_S), zero-padded axis,
     // real pencils along x of the R2C / C2R pass, complex K^F
     int gen_S, gen_P, gen_nfac, gen_pruned, gen_nreal, gen_kcplx, gen_lanes_p;
@@ -129,6 +140,15 @@ template <typename T> PF_HD const cx<T> *pass_in(const PassParams &prm, int bi) 
 }
 template <typename T> PF_HD cx<T> *pass_out(const PassParams &prm, int bi) {
     return prm.use_list == 2 ? reinterpret_cast<cx<T> *>(const_cast<void *>(prm.blist[bi])) : reinterpret_cast<cx<T> *>(prm.out) + bi * prm.bs_out;
+}
+
+// Sharded stores: address of element (v, u, x) of the distributed output (see PassParams::sh_*).
+template <typename T> PF_HD cx<T> *shard_ptr(const PassParams &prm, int v, int u, int x) {
+    const int s = ((v + 1) * prm.sh_R - 1) / prm.sh_total;                                 // owner of v (planner.hpp: shard_owner)
+    const int lo = prm.sh_lo[s], es = prm.sh_lo[s + 1] - lo, vl = v - lo;                  // rank s holds es points of v
+    const long long st_v = prm.sh_vslow ? (long long)prm.sh_eu * prm.sh_nx : prm.sh_nx;
+    const long long st_u = prm.sh_vslow ? prm.sh_nx : (long long)es * prm.sh_nx;
+    return reinterpret_cast<cx<T> *>(const_cast<void *>(prm.blist[s])) + vl * st_v + u * st_u + x;
 }
 
 // ------------------------------------------------------------------ programmatic dependent launch
@@ -677,13 +697,26 @@ PF_HD void process_f2(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
     store_B<G>(v, pass_out<T>(prm, bi) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
 }
 // I2: inverse 1D FFT along axis b + compactification (+ transpose)
-template <class G, bool PRUNED, class Hook = NoHook>
+template <class G, bool PRUNED, bool SHARD = false, class Hook = NoHook>
 PF_HD void process_i2(BufB<G> &b, const PassParams &prm, int tile, TileCtx<G> &c, Hook &&after_read = Hook()) {
     using T = typename G::T;
     const int t = c.t, p = c.p;
     PF_TILE_COORDS
     inv_BtoA<G, PRUNED>(b.x, c.tw, c.xbufs.next(), t, p, after_read);
-    store_A<G, PRUNED>(b.x, pass_out<T>(prm, bi) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+    if constexpr (SHARD) {   // every element goes to the GPU that owns its point of the split axis
+        constexpr int NA2 = PRUNED ? G::RA / 2 : G::RA;
+        if (valid)
+            static_for<G::CA>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                static_for<NA2>([&](auto nc) {
+                    constexpr int n2 = decltype(nc)::value;
+                    const int n = (t + G::TPP * i) + G::RB * n2;
+                    *shard_ptr<T>(prm, prm.sh_vp ? pp : n, prm.sh_u0 + g, prm.sh_vp ? n : pp) = b.x[i * G::RA + n2];
+                });
+            });
+    } else {
+        store_A<G, PRUNED>(b.x, pass_out<T>(prm, bi) + g * prm.gs_out + pp * prm.ps_out, prm.ns_out, t, valid);
+    }
 }
 // F3: spread + 1D FFT along axis c, K^F multiply (Eq. 3), inverse 1D FFT along c,
 // compactification; in place over the tile it read.  kmul(v) multiplies the V
@@ -727,7 +760,7 @@ PF_HD void kmul_global(cx<typename G::T> *v, const void *kint, int tile, int tid
 // Two real pencils adjacent along x are transformed as ONE complex pencil z = rho(2q) + i rho(2q+1)
 // (the real array read as complex IS that packing) and separated with the Hermitian symmetry
 // F_{S-k} = conj(F_k) of PAPER.md:55; only k = 0..S/2 is kept.  in: pairs, out: complex.
-template <class G, bool PRUNED>
+template <class G, bool PRUNED, bool SHARD = false>
 PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileCtx<G> &c) {
     static_assert(G::LANES_P, "the R2C pass runs on a strided axis");
     using T = typename G::T;
@@ -756,7 +789,8 @@ PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
             const T hf = (T)0.5;
             // A = (Z_k + conj Z_{S-k})/2 ; B = -i (Z_k - conj Z_{S-k})/2
             const cx<T> fa = mk<T>(hf * (zk.re + zp.re), hf * (zk.im - zp.im)), fb = mk<T>(hf * (zk.im + zp.im), hf * (zp.re - zk.re));
-            if (pair_store) st_pair(dst + k * prm.ns_out, fa, fb);   // adjacent pencils: one access (256-bit in fp64)
+            if constexpr (SHARD) st_pair(shard_ptr<T>(prm, k, prm.sh_u0 + g, 2 * pp), fa, fb);   // to the GPU that owns plane k
+            else if (pair_store) st_pair(dst + k * prm.ns_out, fa, fb);   // adjacent pencils: one access (256-bit in fp64)
             else { dst[k * prm.ns_out] = fa; dst[k * prm.ns_out + prm.ps_out] = fb; }
         }
     });
@@ -813,7 +847,7 @@ PF_HD void body_f2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         });
 }
 
-template <class G, bool PRUNED>
+template <class G, bool PRUNED, bool SHARD = false>
 PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     PF_BODY_PROLOGUE(false, true, KIND_I2)
     using Buf = BufB<G>;
@@ -843,7 +877,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             },
             [&](Buf &b, int tile, auto &&after_read) {
                 c.xbufs.dirty = false;   // the loop's barriers already separate the tiles
-                process_i2<G, PRUNED>(b, prm, tile, c, after_read);
+                process_i2<G, PRUNED, SHARD>(b, prm, tile, c, after_read);
             });
         return;
     }
@@ -870,7 +904,7 @@ PF_HD void body_i2(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](Buf &b, int tile) {
             if constexpr (St::ON) c.xbufs.dirty = false;
-            process_i2<G, PRUNED>(b, prm, tile, c);
+            process_i2<G, PRUNED, SHARD>(b, prm, tile, c);
         },
         [&](int tile) {
             PF_TILE_COORDS
@@ -931,7 +965,7 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         });   // no next-tile prefetch here: measured slower (512^3 fp32 F3 182 -> 196 us), it competes with the K^F prefetch
 }
 
-template <class G, bool PRUNED>
+template <class G, bool PRUNED, bool SHARD = false>
 PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) {
     PF_BODY_PROLOGUE(true, false, KIND_F1)
     using Buf = BufA<G, PRUNED>;
@@ -947,7 +981,7 @@ PF_HD void body_f1(const PassParams &prm, int bid, int nb, int tid, void *smem) 
         },
         [&](Buf &b, int tile) {
             if constexpr (St::ON) c.xbufs.dirty = false;
-            process_f1<G, PRUNED>(b, prm, tile, c);
+            process_f1<G, PRUNED, SHARD>(b, prm, tile, c);
         },
         [&](int tile) {
             PF_TILE_COORDS

@@ -156,4 +156,73 @@ inline int plan_build(int nx, int ny, int nz, const int bc_in[3], int prec, Plan
     return POISSON_OK;
 }
 
+// ---- sharded single solve ("transposes on the reduced data set", PAPER.md:89 GPU-to-GPU transfers)
+// rho / V are distributed along the axis o (the non-x axis that is not a); between F1 and F2, and between I2 and I1, the
+// half spectrum A1 changes hands once: distributed along o <-> distributed along k_a.  Both partitions are balanced:
+// rank s owns [floor(T s / R), floor(T (s + 1) / R)) of T points, and v belongs to rank floor(((v + 1) R - 1) / T).
+inline int shard_lo(int total, int s, int R) { return (int)((long long)total * s / R); }
+inline int shard_owner(int total, int v, int R) { return (int)((((long long)v + 1) * R - 1) / total); }
+
+struct ShardDesc {
+    int rank, R;
+    int a, o;                 // plane axis, split axis
+    int o0, o1, k0, k1;       // this rank's slab of rho / V along o, and its planes k_a
+    long long ext_rho[3];     // local rho / V extents per axis id (o -> o1 - o0)
+    long long ext_mid[3];     // this rank's exchange slab 1: A1 with a -> k1 - k0 (o whole)
+    long long ext_a2[3];      // its A2: a -> k1 - k0, b -> S_b
+    long long ext_back[3];    // its exchange slab 2: A1 with o -> o1 - o0 (a whole: H)
+    long long mid_elems, back_elems, a2_elems;
+    PassDesc pass[5];         // F1S (in strides only), F2, F3, I2S (in strides only), I1 on the local arrays
+};
+
+inline int shard_build(const PlanDesc &d, int rank, int R, ShardDesc &sh) {
+    if (R < 1 || rank < 0 || rank >= R) return POISSON_EINVAL;
+    std::memset(&sh, 0, sizeof(sh));
+    const int a = d.order[0], b = d.order[1], c = d.order[2], o = 3 - a;
+    if (R > d.n[o] || R > d.H || R > 32) return POISSON_EUNSUPPORTED;    // every rank holds a non-empty slab and plane range
+    if (d.n[0] % 2 != 0) return POISSON_EUNSUPPORTED;                     // the register-engine R2C pass reads x-pairs
+    for (int q = 0; q < 5; ++q) if (d.pass[q].generic) return POISSON_EUNSUPPORTED;
+    sh.rank = rank; sh.R = R; sh.a = a; sh.o = o;
+    sh.o0 = shard_lo(d.n[o], rank, R); sh.o1 = shard_lo(d.n[o], rank + 1, R);
+    sh.k0 = shard_lo(d.H, rank, R);    sh.k1 = shard_lo(d.H, rank + 1, R);
+    const long long no = sh.o1 - sh.o0, ng = sh.k1 - sh.k0;
+    for (int q = 0; q < 3; ++q) { sh.ext_rho[q] = d.n[q]; sh.ext_mid[q] = d.ext1[q]; sh.ext_a2[q] = d.ext2[q]; sh.ext_back[q] = d.ext1[q]; }
+    sh.ext_rho[o] = no; sh.ext_mid[a] = ng; sh.ext_a2[a] = ng; sh.ext_back[o] = no;
+    sh.mid_elems = sh.ext_mid[0] * sh.ext_mid[1] * sh.ext_mid[2];
+    sh.back_elems = sh.ext_back[0] * sh.ext_back[1] * sh.ext_back[2];
+    sh.a2_elems = sh.ext_a2[0] * sh.ext_a2[1] * sh.ext_a2[2];
+    auto stride = [](const long long ext[3], int q) -> long long { return q == 0 ? 1 : (q == 1 ? ext[0] : ext[0] * ext[1]); };
+    const long long extp[3] = {sh.ext_rho[0] / 2, sh.ext_rho[1], sh.ext_rho[2]};   // rho / V read as x-pairs
+
+    PassDesc f1 = d.pass[0];   // kind, axis, S, pruned, lanes_p as in the global plan
+    f1.n_g = no; f1.n_p = d.n[0] / 2;
+    f1.gs_in = stride(extp, o); f1.ns_in = stride(extp, a); f1.ps_in = 1;
+    f1.gs_out = f1.ns_out = f1.ps_out = 0;                                        // scattered over the ranks' slabs (PassParams::sh_*)
+    PassDesc i1 = d.pass[4];
+    i1.n_g = no; i1.n_p = d.n[0] / 2;
+    i1.gs_in = stride(sh.ext_back, o); i1.ns_in = stride(sh.ext_back, a); i1.ps_in = 1;
+    i1.gs_out = f1.gs_in; i1.ns_out = f1.ns_in; i1.ps_out = 1;
+
+    PassDesc f2 = d.pass[1];
+    f2.n_g = ng;
+    if (b == 0) { f2.n_p = sh.ext_mid[c];
+        f2.gs_in = stride(sh.ext_mid, a); f2.ns_in = 1; f2.ps_in = stride(sh.ext_mid, c);
+        f2.gs_out = stride(sh.ext_a2, a); f2.ns_out = 1; f2.ps_out = stride(sh.ext_a2, c);
+    } else { f2.n_p = sh.ext_mid[0];
+        f2.gs_in = stride(sh.ext_mid, a); f2.ns_in = stride(sh.ext_mid, b); f2.ps_in = 1;
+        f2.gs_out = stride(sh.ext_a2, a); f2.ns_out = stride(sh.ext_a2, b); f2.ps_out = 1;
+    }
+    PassDesc i2 = d.pass[3];
+    i2.n_g = ng; i2.n_p = f2.n_p;
+    i2.gs_in = f2.gs_out; i2.ns_in = f2.ns_out; i2.ps_in = f2.ps_out;
+    i2.gs_out = i2.ns_out = i2.ps_out = 0;                                        // scattered
+    PassDesc f3 = d.pass[2];
+    f3.n_g = ng;
+    if (c == 0) { f3.n_p = sh.ext_a2[b]; f3.gs_in = stride(sh.ext_a2, a); f3.ns_in = 1; f3.ps_in = stride(sh.ext_a2, b); }
+    else { f3.n_p = sh.ext_a2[0]; f3.gs_in = stride(sh.ext_a2, a); f3.ns_in = stride(sh.ext_a2, c); f3.ps_in = 1; }
+    f3.gs_out = f3.gs_in; f3.ns_out = f3.ns_in; f3.ps_out = f3.ps_in;
+    sh.pass[0] = f1; sh.pass[1] = f2; sh.pass[2] = f3; sh.pass[3] = i2; sh.pass[4] = i1;
+    return POISSON_OK;
+}
+
 }  // namespace pfft

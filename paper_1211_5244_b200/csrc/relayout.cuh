@@ -12,6 +12,7 @@ namespace pfft {
 struct RelayoutParams {
     int RA, RB, TPP, P, V, NT, lanes_p;
     int tiles_per_g, n_p;
+    int g0;               // first k_a plane held (sharded plans keep only their own planes; else 0)
     int a_axis, c_axis;   // the pencil index pp runs along the remaining axis
     int sx, sy, sz;
     long long total;
@@ -26,7 +27,7 @@ PF_HD T relayout_value(const T *kuser, const RelayoutParams &q, long long idx) {
     const long long tile = idx / ((long long)q.NT * q.V);
     int t, p;
     if (q.lanes_p) { p = tid % q.P; t = tid / q.P; } else { t = tid % q.TPP; p = tid / q.TPP; }
-    const long long g = tile / q.tiles_per_g;
+    const long long g = tile / q.tiles_per_g + q.g0;
     const long long pp = (tile % q.tiles_per_g) * q.P + p;
     if (pp >= q.n_p) return (T)0;
     const int i = r / q.RB, k1 = r % q.RB;

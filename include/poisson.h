@@ -94,7 +94,8 @@ POISSON_API int poisson_plan_describe(int nx, int ny, int nz, const int bc[3] /*
  * metadata only.  *out is set to NULL on failure.  Problem statement: PAPER.md:51.
  * Supported grids: every N_i >= 1 with padded length S_i = N_i * B_i <= 4096, odd N included ("various grid sizes",
  * PAPER.md:89).  A pass whose length is one of
- *   4 8 12 16 20 24 32 36 40 48 60 64 72 80 96 100 120 128 144 160 192 200 240 256 288 320 384 400 480 512 576 640 768 1024
+ *   4 8 12 16 20 24 28 32 36 40 48 56 60 64 72 80 96 100 112 120 128 140 144 160 168 192 200 224 240 256 280 288 320 336 384 400
+ *   448 480 512 576 640 768 896 1024
  * (csrc/sizes.def) runs the compiled register-engine kernel for that length; every other length (odd, factors 7, 11, ...,
  * three or more radices, primes), and the R2C / C2R pass of a grid with odd N_x, runs the any-length shared-memory
  * Stockham kernel (csrc/generic_pass.cuh) -- correct for every length, slower.  Only S_i > 4096 is refused with

@@ -1,5 +1,5 @@
 // fft_core.cuh -- in-register building blocks of the customised FFT:
-// complex arithmetic, compile-time twiddles, small DFTs of radix 2..32 held entirely in one
+// complex arithmetic, compile-time twiddles, small DFTs of radix 2..32 (factors 2, 3, 5, 7) held entirely in one
 // thread's registers, and the two "pruned" variants that implement the paper's spread /
 // compactification without ever touching the zero half:
 //   * dft_pruned_in  : DFT of a length-R sequence whose upper half is zero   (spread,  PAPER.md:53)
@@ -115,14 +115,35 @@ PF_CE double sin480(int j) {  // j in [0, 480)
     return neg ? -v : v;
 }
 PF_CE bool divides480(int R) { return R > 0 && 480 % R == 0; }
+// cos/sin(2 pi m / R) for R | 28 (radices 7, 14, 28), reduced to the first quadrant of an 8-entry literal table.
+PF_CE double q28_cos(int j) { constexpr double t[8] = {PFFT_R28_COS_LIST}; return t[j]; }
+PF_CE double q28_sin(int j) { constexpr double t[8] = {PFFT_R28_SIN_LIST}; return t[j]; }
+PF_CE double cos28(int j) {  // j in [0, 28)
+    if (j > 14) j = 28 - j;
+    return j <= 7 ? q28_cos(j) : -q28_cos(14 - j);
+}
+PF_CE double sin28(int j) {  // j in [0, 28)
+    bool neg = false;
+    if (j > 14) { j = 28 - j; neg = true; }
+    const double v = j <= 7 ? q28_sin(j) : q28_sin(14 - j);
+    return neg ? -v : v;
+}
+PF_CE bool divides28(int R) { return R > 0 && 28 % R == 0; }
+PF_CE bool literal_radix(int R) { return divides480(R) || divides28(R); }
 // real / imaginary part of exp(-2 pi i m / R)   (forward sign)
-PF_CE double tw_re(int m, int R) { return cos480((((m % R) + R) % R) * (480 / R)); }
-PF_CE double tw_im(int m, int R) { return -sin480((((m % R) + R) % R) * (480 / R)); }
+PF_CE double tw_re(int m, int R) {
+    const int j = ((m % R) + R) % R;
+    return divides480(R) ? cos480(j * (480 / R)) : cos28(j * (28 / R));
+}
+PF_CE double tw_im(int m, int R) {
+    const int j = ((m % R) + R) % R;
+    return divides480(R) ? -sin480(j * (480 / R)) : -sin28(j * (28 / R));
+}
 
 // a * exp(-/+ 2 pi i M / R) with M, R compile-time: trivial cases cost no multiply.
 template <int M_, int R, bool INV, typename T>
 PF_HD cx<T> mul_tw(cx<T> a) {
-    static_assert(divides480(R), "radix must divide 480");
+    static_assert(literal_radix(R), "radix must divide 480 or 28");
     constexpr int M = ((M_ % R) + R) % R;
     if constexpr (M == 0) {
         return a;
@@ -201,10 +222,36 @@ template <typename T, bool INV> struct Dft<T, 5, INV> {
     }
 };
 
+// radix 7: a_j = x_j + x_{7-j}, b_j = x_j - x_{7-j};  X_k, X_{7-k} = x_0 + sum_j cos(2 pi jk/7) a_j  -/+  i sum_j sin(2 pi jk/7) b_j
+template <typename T, bool INV> struct Dft<T, 7, INV> {
+    static PF_HD void run(cx<T> *x) {
+        constexpr T c1 = (T)0.6234898018587335305250048840042398106323;    // cos(2 pi/7)
+        constexpr T c2 = (T)-0.2225209339563144042889025644967947594664;   // cos(4 pi/7)
+        constexpr T c3 = (T)-0.9009688679024191262361023195074450511659;   // cos(6 pi/7)
+        constexpr T s1 = (T)0.7818314824680298087084445266740577502323;    // sin(2 pi/7)
+        constexpr T s2 = (T)0.9749279121818236070181316829939312172328;    // sin(4 pi/7)
+        constexpr T s3 = (T)0.43388373911755812047576833284835875461;      // sin(6 pi/7)
+        const cx<T> a1 = x[1] + x[6], b1 = x[1] - x[6], a2 = x[2] + x[5], b2 = x[2] - x[5], a3 = x[3] + x[4], b3 = x[3] - x[4];
+        // cos(2 pi jk/7): k = 1: c1 c2 c3;  k = 2: c2 c3 c1;  k = 3: c3 c1 c2.   sin: k = 1: s1 s2 s3;  k = 2: s2 -s3 -s1;  k = 3: s3 -s1 s2
+        const cx<T> m1 = mk<T>(x[0].re + c1 * a1.re + c2 * a2.re + c3 * a3.re, x[0].im + c1 * a1.im + c2 * a2.im + c3 * a3.im);
+        const cx<T> m2 = mk<T>(x[0].re + c2 * a1.re + c3 * a2.re + c1 * a3.re, x[0].im + c2 * a1.im + c3 * a2.im + c1 * a3.im);
+        const cx<T> m3 = mk<T>(x[0].re + c3 * a1.re + c1 * a2.re + c2 * a3.re, x[0].im + c3 * a1.im + c1 * a2.im + c2 * a3.im);
+        const cx<T> u1 = mk<T>(s1 * b1.re + s2 * b2.re + s3 * b3.re, s1 * b1.im + s2 * b2.im + s3 * b3.im);
+        const cx<T> u2 = mk<T>(s2 * b1.re - s3 * b2.re - s1 * b3.re, s2 * b1.im - s3 * b2.im - s1 * b3.im);
+        const cx<T> u3 = mk<T>(s3 * b1.re - s1 * b2.re + s2 * b3.re, s3 * b1.im - s1 * b2.im + s2 * b3.im);
+        // forward: X_k = m_k - i u_k, X_{7-k} = m_k + i u_k
+        const cx<T> v1 = INV ? mul_pi(u1) : mul_mi(u1);
+        const cx<T> v2 = INV ? mul_pi(u2) : mul_mi(u2);
+        const cx<T> v3 = INV ? mul_pi(u3) : mul_mi(u3);
+        x[0] = x[0] + a1 + a2 + a3;
+        x[1] = m1 + v1; x[6] = m1 - v1; x[2] = m2 + v2; x[5] = m2 - v2; x[3] = m3 + v3; x[4] = m3 - v3;
+    }
+};
+
 // first factor A of the Cooley-Tukey split R = A * B used for composite radices
 PF_CE int split_a(int R) {
-    return R == 6 ? 2 : R == 8 ? 2 : R == 10 ? 2 : R == 12 ? 3 : R == 16 ? 4 : R == 20 ? 4
-         : R == 24 ? 3 : R == 32 ? 4 : 0;
+    return R == 6 ? 2 : R == 8 ? 2 : R == 10 ? 2 : R == 12 ? 3 : R == 14 ? 2 : R == 16 ? 4 : R == 20 ? 4
+         : R == 24 ? 3 : R == 28 ? 4 : R == 32 ? 4 : 0;
 }
 
 // Composite: n = n1 + B n2, k = k2 + A k1;  X[k2 + A k1] = sum_n1 w_B^{n1 k1} [ w_R^{n1 k2} sum_n2 x[n1 + B n2] w_A^{n2 k2} ]

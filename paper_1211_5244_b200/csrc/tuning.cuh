@@ -26,6 +26,31 @@
     PF_VARIANT(7, 1, true, 0, 3, true) PF_VARIANT(8, 1, true, 3, 3, true) PF_VARIANT(10, 1, false, 3, 0, true) PF_VARIANT(11, 1, false, 4, 0, true)
 #endif
 
+#if PF_S == 28 && defined(PF_ONLY_F64)
+// one thread per pencil, 28 complex fp64 values in registers (radix 28): no 128-register cap (it spills 256 bytes)
+#define PF_MINB 2
+#endif
+
+#if PF_S == 448 && defined(PF_ONLY_F64)
+// 32 complex fp64 values per thread (28 x 16, two columns of the second pass per thread): as 384 / 512
+#define PF_MINB 2
+#define PF_STG 1
+#endif
+
+#if PF_S == 336 && defined(PF_ONLY_F64)
+// 24 complex fp64 values per thread, 192 threads per CTA: as 576
+#define PF_MINB 2
+#define PF_STG 1
+#endif
+
+#if PF_S == 896
+// as 1024: one CTA per SM (fp64: 32 complex values per thread, next tile staged)
+#define PF_MINB 1
+#if defined(PF_ONLY_F64)
+#define PF_STG 1
+#endif
+#endif
+
 #if PF_S == 384 && defined(PF_ONLY_F64)
 // 32 complex fp64 values per thread: the full register file, 2 CTAs of 128 threads per SM
 #define PF_MINB 2

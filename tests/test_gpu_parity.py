@@ -65,13 +65,16 @@ SWEEP_SIZES = [(4, 4, 4), (8, 4, 16), (16, 8, 4), (12, 24, 6), (32, 6, 8), (6, 4
                # lengths with factors 5 and 9, and 1024 (sizes.def, second block)
                (20, 40, 36), (72, 20, 40), (100, 36, 20), (144, 8, 20), (200, 4, 8), (4, 288, 8), (8, 4, 512),
                # lengths whose second-pass columns are ragged (sizes.def, third block)
-               (60, 8, 4), (120, 4, 8), (4, 160, 8), (8, 4, 240), (320, 4, 4), (4, 384, 4), (80, 192, 4)]
+               (60, 8, 4), (120, 4, 8), (4, 160, 8), (8, 4, 240), (320, 4, 4), (4, 384, 4), (80, 192, 4),
+               # lengths with a factor 7: radix 7 / 14 / 28 in registers (sizes.def, fourth block), on every axis position
+               (28, 8, 4), (4, 56, 8), (8, 4, 112), (140, 4, 4), (4, 168, 4), (224, 4, 8), (8, 224, 4), (4, 8, 336),
+               (4, 4, 448), (448, 4, 4), (56, 28, 12)]
 
 
 @pytest.mark.parametrize("prec", ["fp64", "fp32"])
 @pytest.mark.parametrize("n", SWEEP_SIZES, ids=lambda n: "x".join(map(str, n)))
 def test_sweep_all_bc_vs_oracle(pk, n, prec):
-    """Lengths 2^a, 3*2^a and the 5- and 9-smooth ones of sizes.def, several tiles and ragged tails, all 8 BC
+    """Lengths 2^a, 3*2^a and the 5-, 7- and 9-smooth ones of sizes.def, several tiles and ragged tails, all 8 BC
     combinations per size."""
     rng = np.random.default_rng(1000 + sum(n))
     ran = 0

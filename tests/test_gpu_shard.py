@@ -165,7 +165,7 @@ def test_shard_plan_refuses_plain_calls_and_bad_arguments(pk):
         pk.ShardPlan((32, 32, 32), (0, 0, 0), 0.2, pk.FP64, 2, 2)          # rank out of range
     assert ei.value.status == 1
     with pytest.raises(pk.PoissonError) as ei:
-        pk.ShardPlan((30, 14, 12), (0, 0, 0), 0.2, pk.FP64, 0, 2)          # S = 28: no register-engine kernel
+        pk.ShardPlan((30, 22, 12), (0, 0, 0), 0.2, pk.FP64, 0, 2)          # S = 44: no register-engine kernel
     assert ei.value.status == 2
     p = pk.ShardPlan((32, 32, 32), (0, 0, 0), 0.2, pk.FP64, 0, 2)
     try:

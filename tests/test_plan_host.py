@@ -119,8 +119,17 @@ def test_plan_create_fails_loudly_without_a_b200(lib):
         pk.PoissonPlan((8, 8, 8), (0, 0, 0), 0.1)
 
 
-SUPPORTED_LENGTHS = [4, 8, 12, 16, 20, 24, 32, 36, 40, 48, 60, 64, 72, 80, 96, 100, 120, 128, 144, 160, 192, 200, 240,
-                     256, 288, 320, 384, 400, 480, 512, 576, 640, 768, 1024]
+SUPPORTED_LENGTHS = [4, 8, 12, 16, 20, 24, 28, 32, 36, 40, 48, 56, 60, 64, 72, 80, 96, 100, 112, 120, 128, 140, 144, 160, 168, 192,
+                     200, 224, 240, 256, 280, 288, 320, 336, 384, 400, 448, 480, 512, 576, 640, 768, 896, 1024]
+
+
+def test_compiled_lengths_are_those_of_sizes_def():
+    text = (ROOT / "paper_1211_5244_b200" / "csrc" / "sizes.def").read_text()
+    listed = sorted(int(m) for m in re.findall(r"^PF_SIZE\((\d+),", text, flags=re.M))
+    assert listed == SUPPORTED_LENGTHS
+    header = (ROOT / "include" / "poisson.h").read_text()
+    for v in SUPPORTED_LENGTHS:
+        assert re.search(rf"\b{v}\b", header), f"{v} missing from the list in poisson.h"
 
 
 def test_every_length_is_planned_up_to_the_any_length_limit():

@@ -74,7 +74,7 @@ def test_exchange_is_on_the_smallest_intermediate():
 def test_unsupported_and_invalid():
     for args, status in [(((30, 32, 32), (0, 0, 0), 0, 2), None),            # fine: S = 60 is compiled
                          (((31, 32, 32), (0, 0, 0), 0, 2), 2),               # odd N_x
-                         (((32, 14, 32), (0, 0, 0), 0, 2), 2),               # S_y = 28: any-length kernel only
+                         (((32, 22, 32), (0, 0, 0), 0, 2), 2),               # S_y = 44: any-length kernel only
                          (((32, 4, 32), (0, 1, 0), 0, 5), 2),                # more ranks than points of the split axis
                          (((32, 32, 32), (0, 0, 0), 2, 2), 1),               # rank out of range
                          (((32, 32, 32), (0, 0, 0), 0, 0), 1)]:

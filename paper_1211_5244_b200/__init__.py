@@ -432,10 +432,10 @@ class ShardedSolver:
             sizes = torch.tensor([info.mid_bytes, info.back_bytes], dtype=torch.int64, device="cuda")
             dist.all_reduce(sizes, op=dist.ReduceOp.MAX, group=group)
             mid_b, back_b = (int(v) for v in sizes.tolist())
-            gname = (group or dist.group.WORLD).group_name
+            pg = group or dist.group.WORLD
             self._mid = symm.empty(mid_b, dtype=torch.uint8, device="cuda")
             self._back = symm.empty(back_b, dtype=torch.uint8, device="cuda")
-            hm, hb = symm.rendezvous(self._mid, gname), symm.rendezvous(self._back, gname)
+            hm, hb = symm.rendezvous(self._mid, pg), symm.rendezvous(self._back, pg)
             mids, backs = list(hm.buffer_ptrs), list(hb.buffer_ptrs)
         self.plan.set_slabs(mids, backs, keep=(self._mid, self._back))
         self._flag = torch.zeros(1, dtype=torch.int32, device="cuda")

@@ -244,10 +244,8 @@ struct poisson_plan {
     long long a2_alloc_elems;   // complex elements of the A2 buffer actually allocated (one chunk when chunked)
     int late_tw;               // PassParams::late_tw for every pass (POISSON_LATE_TW, default 1; 0 under programmatic dependent launch)
     int pdl_trigger;           // PassParams::pdl_trigger (POISSON_PDL_TRIGGER: 0 start of the pass, 1 last tile of each CTA, 2 exit)
-    bool env_lane_shape;       // POISSON_LANE_SHAPE=1: the batch lanes' graphs take the plan's graph shape too (experiments)
     bool env_shape;            // POISSON_BRANCHES / POISSON_XCHAINS given: the tuner keeps that graph shape
     int xchains;               // graph mode: F1 / F2 / I2 / I1 split over this many ranges of x (POISSON_XCHAINS)
-    int branch_serial, branch_grid;   // experiments: order the chains' kernels of one kind; cap the grid of a chain's kernels
     int branches;              // graph mode: the middle passes as this many parallel chains over ranges of k_a planes (POISSON_BRANCHES)
     int env_lanes, env_wide;   // POISSON_LANES / POISSON_WIDE as read at plan creation (-1: not set)
     bool env_lane_graph;       // POISSON_LANE_GRAPH=0 at plan creation: plain launches on the batch lanes (experiments)
@@ -527,9 +525,6 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     { const char *env = std::getenv("POISSON_BRANCHES"); pl->branches = env ? std::atoi(env) : 1; }
     { const char *env = std::getenv("POISSON_XCHAINS"); pl->xchains = env ? std::atoi(env) : 1; if (pl->xchains > PF_MAX_XR) pl->xchains = PF_MAX_XR; }
     pl->env_shape = std::getenv("POISSON_BRANCHES") || std::getenv("POISSON_XCHAINS");
-    { const char *env = std::getenv("POISSON_LANE_SHAPE"); pl->env_lane_shape = env && env[0] == '1'; }
-    { const char *env = std::getenv("POISSON_BRANCH_SERIAL"); pl->branch_serial = env ? std::atoi(env) : 0; }
-    { const char *env = std::getenv("POISSON_BRANCH_GRID"); pl->branch_grid = env ? std::atoi(env) : 0; }
     { const char *env = std::getenv("POISSON_LANES"); pl->env_lanes = env ? std::atoi(env) : -1; }
     { const char *env = std::getenv("POISSON_WIDE"); pl->env_wide = env ? std::atoi(env) : -1; }
     { const char *env = std::getenv("POISSON_LANE_GRAPH"); pl->env_lane_graph = !(env && env[0] == '0'); }
@@ -985,7 +980,7 @@ static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
         return POISSON_OK;
     };
     int rc = POISSON_OK;
-    const bool shaped = pl->n_chunks <= 1 && (!ln || pl->env_lane_shape);   // batch lanes already overlap each other: plain chains there
+    const bool shaped = pl->n_chunks <= 1 && !ln;   // batch lanes already overlap each other: plain chains there (measured: 90.3 vs 92.8 us)
     const int B = shaped ? (pl->branches < pl->d.H ? pl->branches : pl->d.H) : 1;
     int R = shaped ? pl->xchains : 1;
     {   // x chains need: no plane chunks, the register engine everywhere, x as the pencil index of F1 / F2 / I2 / I1, whole tiles per range
@@ -1038,27 +1033,17 @@ static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
         g.prm_f1 = pass_params(pl, POISSON_PASS_F1, nullptr, nullptr, ln);
         g.prm_i1 = pass_params(pl, POISSON_PASS_I1, nullptr, nullptr, ln);
         rc = add_node(POISSON_PASS_F1, g.prm_f1, pl->grid[0], &g.node_f1);
-        cudaGraphNode_t last[3] = {nullptr, nullptr, nullptr};   // the previous chain's F2 / F3 / I2 (serial ordering experiment)
+        // node creation order matters: chain by chain, I1 last (creating I1 before the chains made the wire grid 50 % slower)
         std::vector<cudaGraphNode_t> tails(B, g.node_f1);
-        auto add_chain_node = [&](int j, int q) -> int {
+        for (int j = 0; j < B; ++j) {
             const int g0 = (int)((long long)pl->d.H * j / B), g1 = (int)((long long)pl->d.H * (j + 1) / B);
-            const PassParams prm = range_params(pl, q, ln, g0, g1 - g0);
-            int grid = prm.n_tiles < pl->grid[q] ? prm.n_tiles : pl->grid[q];
-            if (pl->branch_grid > 0 && grid > pl->branch_grid) grid = pl->branch_grid;
-            cudaGraphNode_t node;
-            int rc1 = add_node(q, prm, grid, &node);
-            if (rc1 == POISSON_OK) rc1 = add_edge(tails[j], node, prog);
-            if (rc1 == POISSON_OK && pl->branch_serial == 1 && last[q - 1]) rc1 = add_edge(last[q - 1], node, false);
-            last[q - 1] = node;
-            tails[j] = node;
-            return rc1;
-        };
-        if (pl->branch_serial == 2) {   // node creation order: pass by pass
-            for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2; ++q)
-                for (int j = 0; j < B && rc == POISSON_OK; ++j) rc = add_chain_node(j, q);
-        } else {                        // chain by chain
-            for (int j = 0; j < B; ++j)
-                for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2 && rc == POISSON_OK; ++q) rc = add_chain_node(j, q);
+            for (int q = POISSON_PASS_F2; q <= POISSON_PASS_I2 && rc == POISSON_OK; ++q) {
+                const PassParams prm = range_params(pl, q, ln, g0, g1 - g0);
+                cudaGraphNode_t node;
+                rc = add_node(q, prm, prm.n_tiles < pl->grid[q] ? prm.n_tiles : pl->grid[q], &node);
+                if (rc == POISSON_OK) rc = add_edge(tails[j], node, prog);
+                tails[j] = node;
+            }
         }
         if (rc == POISSON_OK) rc = add_node(POISSON_PASS_I1, g.prm_i1, pl->grid[4], &g.node_i1);
         for (size_t j = 0; j < tails.size() && rc == POISSON_OK; ++j) rc = add_edge(tails[j], g.node_i1, prog && j == 0);   // one programmatic edge into I1, the rest plain
@@ -1088,7 +1073,7 @@ static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
 // the launch attribute into programmatic edges); the F1 / I1 kernel nodes are identified by their function.
 static int build_graph_pdl(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
     if (g.exec) return POISSON_OK;
-    if ((pl->branches > 1 || pl->xchains > 1) && pl->n_chunks <= 1 && (!ln || pl->env_lane_shape)) {   // parallel chains: explicit nodes with programmatic edges
+    if ((pl->branches > 1 || pl->xchains > 1) && pl->n_chunks <= 1 && !ln) {   // parallel chains: explicit nodes with programmatic edges
         const bool saved = pl->use_pdl;
         pl->use_pdl = true;
         const int rc = build_graph(pl, g, ln);

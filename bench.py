@@ -313,13 +313,14 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------ GPU timing
-def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, with_profile=True, inputs=None):
+def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, with_profile=True, inputs=None, even_kernel=False):
     cfg, rho_np, kf_np = inputs if inputs is not None else build_inputs(key)
     prec = pk.FP64 if cfg.precision == "fp64" else pk.FP32
     np_dt = np.float64 if prec == pk.FP64 else np.float32
     plan = pk.PoissonPlan(cfg.n, cfg.bc, cfg.h, prec)
     info = plan.info
-    plan.set_kernel(torch.from_numpy(np.ascontiguousarray(kf_np.astype(np_dt))).cuda())
+    # even_kernel: the folded K^F copy (poisson_set_kernel_even; every BASELINE kernel is even along each axis)
+    (plan.set_kernel_even if even_kernel else plan.set_kernel)(torch.from_numpy(np.ascontiguousarray(kf_np.astype(np_dt))).cuda())
     rho_bytes = rho_np.size * np.dtype(np_dt).itemsize
     nbuf = max(2, int(math.ceil(1.1 * L2_BYTES / (2 * rho_bytes))))    # rho+V ring larger than L2
     nbuf = min(max(nbuf, min(BATCH, 8 if rho_bytes > 64e6 else BATCH)), 64)
@@ -379,7 +380,7 @@ def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, wi
     res = {"key": key, "single": single, "batch": batch, "batch_size": bsz,
            "info": info, "nbuf": nbuf, "rho_bytes": rho_bytes,
            "launch_mode": mode, "tune_ms": tune_ms, "graph_shape": list(plan.graph_shape()), "lanes": plan.batch_lanes(bsz),
-           "width": plan.batch_width(bsz), "launches_per_solve": plan.launches_per_solve()}
+           "width": plan.batch_width(bsz), "launches_per_solve": plan.launches_per_solve(), "workspace_bytes": plan.workspace_bytes()}
     if pass_ms is not None:
         res["pass_ms"] = pass_ms
 
@@ -444,7 +445,7 @@ def run_ours(args):
     inputs = build_inputs(args.config)
     sampler = ClockSampler(local)
     sampler.start()
-    res = time_config(pk, torch, args.config, steps, warmup, inputs=inputs)
+    res = time_config(pk, torch, args.config, steps, warmup, inputs=inputs, even_kernel=args.even_kernel)
     clocks = sampler.stop()
     if rank != 0:
         return 0
@@ -532,6 +533,15 @@ def run_ours(args):
         "gpu_launches_note": f"{res['launches_per_solve']} kernels per solve x {steps} solves in ONE timed region ({res['single']['regions']} regions were timed)",
         "clocks": clocks,
     }
+    if args.even_kernel:
+        line["config"]["kernel_storage"] = "folded: poisson_set_kernel_even (K^F kept for k_b <= S_b/2 only)"
+    elif world == 1:
+        # SURVEY.md 8f-2 (less K^F traffic): the same solves with the folded K^F copy, timed the same way
+        ev = time_config(pk, torch, args.config, steps, warmup, with_e2e=False, with_cold=False, with_profile=False, inputs=inputs,
+                         even_kernel=True)
+        line["even_kernel"] = {"ms_per_step": ev["single"]["ms"], "solves_per_sec": 1e3 / ev["single"]["ms"],
+                               "workspace_bytes": ev["workspace_bytes"], "workspace_bytes_full_kernel": res["workspace_bytes"],
+                               "api": "poisson_set_kernel_even + poisson_solve: K^F stored for k_b <= S_b/2 only (kernels even along every axis)"}
     if world == 1 and not args.no_cpu_baseline:
         sec, desc, threads, extrap, frac, ntimed = oracle_steps(cfg, inputs[1], inputs[2], 3, 0, 30.0)
         line["cpu_baseline"] = {"value": 1.0 / sec, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
@@ -569,6 +579,7 @@ def main():
     ap.add_argument("--config", default="c1", choices=sorted(WORKLOAD_TEXT))
     ap.add_argument("--headline-only", action="store_true", help="skip the other configs' timings")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--even-kernel", action="store_true", help="install K^F with poisson_set_kernel_even (folded storage) instead of poisson_set_kernel")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

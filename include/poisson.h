@@ -117,6 +117,17 @@ POISSON_API int poisson_plan_get_info(const poisson_plan *plan, poisson_plan_inf
  * Asynchronous on `stream`; K_f_dev may be freed once that work has completed. */
 POISSON_API int poisson_set_kernel(poisson_plan *plan, const void *K_f_dev, void *stream);
 
+/* The same for a kernel that is even along EVERY axis separately, K(+-x, +-y, +-z) all equal -- the free-space, wire and
+ * surface Green's functions and -1/|k|^2 are -- stored at half the size (less K^F traffic).
+ * Then K^F(k_a, S_b - k_b, k_c) = K^F(k_a, k_b, k_c) along the second-processed axis b, and the internal copy keeps only
+ * the pencils k_b = 0 .. S_b/2: H (S_b/2 + 1) S_c reals instead of H S_b S_c.  Pass F3 reads the K^F of pencil S_b - k_b for
+ * the upper half (same values, so results are bitwise those of poisson_set_kernel); its K^F traffic and the plan's largest
+ * buffer halve.  K_f_dev as for poisson_set_kernel (the whole array; only k_b <= S_b/2 of it is read).  The evenness is the
+ * CALLER's statement: it is not checked, and a kernel that is only inversion symmetric gives wrong results here.
+ * The first call re-allocates the internal copy (device synchronisation) and drops the one-launch FUSED mode; poisson_set_kernel
+ * switches back.  Register-engine F3 kernels only (else EUNSUPPORTED).  Errors: EINVAL, EUNSUPPORTED, ENOMEM, ECUDA. */
+POISSON_API int poisson_set_kernel_even(poisson_plan *plan, const void *K_f_dev, void *stream);
+
 /* The same for a real kernel K WITHOUT inversion symmetry (K(-r) != K(r): the general convolution of Eq. 2,
  * PAPER.md:37; screened / anisotropic kernels and the plane-wave local-potential convolution of PAPER.md:93), whose
  * spectrum is complex with K^F(-k) = conj K^F(k).

@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = (
     "poisson_plan_describe", "poisson_plan_create", "poisson_plan_kernel_dims", "poisson_plan_get_info",
     "poisson_set_kernel", "poisson_set_kernel_complex", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
     "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_measure_fma_peak", "poisson_plan_workspace_bytes",
-    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_plan_graph_shape", "poisson_shard_describe", "poisson_shard_plan_create", "poisson_shard_get_info", "poisson_shard_set_slabs", "poisson_shard_set_kernel", "poisson_shard_forward", "poisson_shard_middle", "poisson_shard_inverse", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes", "poisson_plan_batch_width",
+    "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_plan_graph_shape", "poisson_set_kernel_even", "poisson_shard_describe", "poisson_shard_plan_create", "poisson_shard_get_info", "poisson_shard_set_slabs", "poisson_shard_set_kernel", "poisson_shard_forward", "poisson_shard_middle", "poisson_shard_inverse", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes", "poisson_plan_batch_width",
 )
 
 _PKG = Path(__file__).resolve().parent
@@ -93,6 +93,7 @@ def load_library():
     lib.poisson_plan_get_info.argtypes = [vp, ctypes.POINTER(PlanInfo)]
     lib.poisson_set_kernel.argtypes = [vp, vp, vp]
     lib.poisson_set_kernel_complex.argtypes = [vp, vp, vp]
+    lib.poisson_set_kernel_even.argtypes = [vp, vp, vp]
     lib.poisson_solve.argtypes = [vp, vp, vp, vp]
     lib.poisson_solve_host.argtypes = [vp, vp, vp, vp]
     lib.poisson_debug_workspace.argtypes = [vp, i, ctypes.POINTER(vp), ll * 3]
@@ -153,6 +154,10 @@ def poisson_plan_create(nx: int, ny: int, nz: int, bc, h: float, precision: int 
 
 def poisson_set_kernel(plan: int, K_f_dev_ptr: int, stream: int = 0) -> None:
     _check(load_library().poisson_set_kernel(plan, K_f_dev_ptr, stream), "poisson_set_kernel")
+
+
+def poisson_set_kernel_even(plan: int, K_f_dev_ptr: int, stream: int = 0) -> None:
+    _check(load_library().poisson_set_kernel_even(plan, K_f_dev_ptr, stream), "poisson_set_kernel_even")
 
 
 def poisson_set_kernel_complex(plan: int, K_f_dev_ptr: int, stream: int = 0) -> None:
@@ -220,6 +225,12 @@ class PoissonPlan:
         assert K_f.is_cuda and K_f.is_contiguous() and K_f.dtype == self._dtype()
         assert tuple(K_f.shape) == self.kernel_dims, (tuple(K_f.shape), self.kernel_dims)
         poisson_set_kernel(self._h, K_f.data_ptr(), self._stream(stream))
+
+    def set_kernel_even(self, K_f, stream=None):
+        """K_f of a kernel that is even along every axis: stored folded, half the size (poisson_set_kernel_even)."""
+        assert K_f.is_cuda and K_f.is_contiguous() and K_f.dtype == self._dtype()
+        assert tuple(K_f.shape) == self.kernel_dims, (tuple(K_f.shape), self.kernel_dims)
+        poisson_set_kernel_even(self._h, K_f.data_ptr(), self._stream(stream))
 
     def set_kernel_complex(self, K_f, stream=None):
         """K_f: complex CUDA tensor [S_z][S_y][S_x/2+1] (rfftn of a real kernel without inversion symmetry)."""

@@ -235,6 +235,8 @@ struct poisson_plan {
     const KernelEntry *k[5];
     KernelEntry gen_entry[5];  // the passes that run the any-length kernel point here
     bool kcplx;                // the installed K^F is complex (poisson_set_kernel_complex)
+    bool keven;                // the installed K^F is stored folded along axis b (poisson_set_kernel_even): pencils 0 .. S_b / 2 only
+    int k_tpg;                 // ... in this many tiles per k_a plane
     int grid[5];
     int resident[5];      // co-resident CTAs of each pass kernel on this device
     int n_tiles[5], tiles_per_g[5];
@@ -377,6 +379,7 @@ static int launches_per_solve(const poisson_plan *pl) { return pl->n_chunks <= 1
 static long long kint_reals(const poisson_plan *pl) {
     const KernelEntry *e = pl->k[2];
     if (e->generic) return (long long)pl->d.pass[2].n_g * pl->d.pass[2].S * pl->d.pass[2].n_p * (pl->kcplx ? 2 : 1);
+    if (pl->keven) return (long long)pl->d.pass[2].n_g * pl->k_tpg * e->V * e->NT;
     return (long long)pl->n_tiles[2] * e->V * e->NT;
 }
 
@@ -724,7 +727,8 @@ static int relayout_kernel_spectrum(poisson_plan *pl, const void *K_f_dev, bool 
         RelayoutParams q;
         q.g0 = pl->shard ? pl->shard->k0 : 0;
         q.RA = e->RA; q.RB = e->RB; q.TPP = e->TPP; q.P = e->P; q.V = e->V; q.NT = e->NT; q.lanes_p = e->lanes_p;
-        q.tiles_per_g = pl->tiles_per_g[2]; q.n_p = (int)d.pass[2].n_p;
+        q.tiles_per_g = pl->keven ? pl->k_tpg : pl->tiles_per_g[2]; q.n_p = (int)d.pass[2].n_p;
+        q.fold = pl->keven ? (int)d.pass[2].n_p : 0;
         q.a_axis = d.order[0]; q.c_axis = d.order[2];
         q.sx = d.s[0]; q.sy = d.s[1]; q.sz = d.s[2];
         q.total = pl->kint_elems;
@@ -740,10 +744,50 @@ static int relayout_kernel_spectrum(poisson_plan *pl, const void *K_f_dev, bool 
     return POISSON_OK;
 }
 
+// Switches the internal K^F copy between the full and the folded layout (poisson_set_kernel_even): the buffer is re-allocated at
+// its new size and everything built around pass F3's parameters (graphs, the one-launch kernel's addressing) is dropped / rebuilt.
+static int switch_kernel_fold(poisson_plan *pl, bool even) {
+    if (pl->keven == even) return POISSON_OK;
+    PF_CUDA(cudaDeviceSynchronize());   // no solve of this plan may still be reading the buffer replaced below
+    const bool was = pl->keven;
+    pl->keven = even;
+    pl->k_tpg = (int)((pl->d.pass[2].n_p / 2 + 1 + pl->k[2]->P - 1) / pl->k[2]->P);
+    const long long need = kint_reals(pl);
+    void *fresh = nullptr;
+    cudaError_t ce = cudaMalloc(&fresh, (size_t)need * pl->elem_real);
+    if (ce != cudaSuccess) { cudaGetLastError(); pl->keven = was; return ce == cudaErrorMemoryAllocation ? POISSON_ENOMEM : cuda_fail(ce, "K^F allocation"); }
+    cudaFree(pl->kint);
+    pl->kint = fresh;
+    pl->workspace_bytes += (size_t)need * pl->elem_real;
+    pl->workspace_bytes -= (size_t)pl->kint_elems * pl->elem_real;
+    pl->d.info.workspace_bytes = (long long)pl->workspace_bytes;
+    pl->kint_elems = need;
+    pl->kernel_set = false;
+    destroy_graph(pl->gs); destroy_graph(pl->gs_pdl);
+    if (pl->lanes) for (Lane &ln : *pl->lanes) if (ln.gs) destroy_graph(*ln.gs);
+    if (even) { pl->fused = nullptr; pl->use_fused = false; }   // the one-launch kernel addresses the full layout
+    if (pl->use_graph) { if ((pl->use_pdl ? build_graph_pdl(pl, pl->gs_pdl, nullptr) : build_graph(pl, pl->gs, nullptr)) != POISSON_OK) cudaGetLastError(); }
+    return POISSON_OK;
+}
+
+int poisson_set_kernel_even(poisson_plan *pl, const void *K_f_dev, void *stream) {
+    if (!pl || !K_f_dev) return POISSON_EINVAL;
+    if (reinterpret_cast<size_t>(K_f_dev) % 16) return POISSON_EINVAL;
+    if (check_device(pl) != POISSON_OK) return POISSON_EINVAL;
+    if (pl->k[2]->generic || pl->kcplx) return POISSON_EUNSUPPORTED;   // the register-engine F3 kernels only
+    int rc = switch_kernel_fold(pl, true);
+    if (rc != POISSON_OK) return rc;
+    rc = relayout_kernel_spectrum(pl, K_f_dev, false, reinterpret_cast<cudaStream_t>(stream));
+    if (rc != POISSON_OK) return rc;
+    pl->kernel_set = true;
+    return POISSON_OK;
+}
+
 int poisson_set_kernel(poisson_plan *pl, const void *K_f_dev, void *stream) {
     if (!pl || !K_f_dev) return POISSON_EINVAL;
     if (reinterpret_cast<size_t>(K_f_dev) % 16) return POISSON_EINVAL;
     if (check_device(pl) != POISSON_OK) return POISSON_EINVAL;
+    if (pl->keven) { const int rc0 = switch_kernel_fold(pl, false); if (rc0 != POISSON_OK) return rc0; }
     if (pl->kcplx) {   // back from a complex kernel: the any-length F3 kernel stays, its K^F copy holds reals again
         pl->kcplx = false;
         destroy_graph(pl->gs); destroy_graph(pl->gs_pdl);
@@ -761,6 +805,7 @@ int poisson_set_kernel_complex(poisson_plan *pl, const void *K_f_dev, void *stre
     if (reinterpret_cast<size_t>(K_f_dev) % 16) return POISSON_EINVAL;
     if (check_device(pl) != POISSON_OK) return POISSON_EINVAL;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (pl->keven) { const int rc0 = switch_kernel_fold(pl, false); if (rc0 != POISSON_OK) return rc0; }
     if (!pl->kcplx) {
         // The complex multiply lives in the any-length F3 kernel: switch pass F3 to it (once), drop what was built
         // around the old kernel (graphs, the fused one-launch kernel), and size the internal K^F copy for complex values.
@@ -801,6 +846,7 @@ static PassParams pass_params(const poisson_plan *pl, int q, const void *rho, vo
         default: prm.in = a1; prm.out = V; break;
     }
     prm.kint = pl->kint;
+    if (q == POISSON_PASS_F3 && pl->keven) { prm.k_fold = (int)ps.n_p; prm.k_tpg = pl->k_tpg; }
     prm.tw = pl->tw[ps.axis];
     prm.gs_in = ps.gs_in; prm.ns_in = ps.ns_in; prm.ps_in = ps.ps_in;
     prm.gs_out = ps.gs_out; prm.ns_out = ps.ns_out; prm.ps_out = ps.ps_out;

@@ -113,6 +113,9 @@ struct PassParams {
     int pdl_trigger;   // programmatic dependent launch: 0 = the next pass may launch from the start of this one, 1 = once this CTA is
                        // past its last tile's loads, 2 = only when this pass exits (the implicit trigger)
     int k_g0;          // F3 of a plane chunk: first plane of the chunk (K^F is indexed by the plane's position in the whole grid)
+    int k_fold;        // F3, K^F even along axis b (poisson_set_kernel_even): S_b, the pencils pp > S_b / 2 read the K^F of pencil
+                       // S_b - pp and only pencils 0 .. S_b / 2 are stored (k_tpg tiles per plane); 0: every pencil is stored
+    int k_tpg;
     int prefetch;      // bit 0: prefetch the next tile's inputs into L2 (unstaged tile loops); bit 1: F3 prefetches its K^F lines
     // several densities per launch (small grids, poisson_solve_batch): tile = bi * n_tiles1 + tile of density bi
     int n_tiles1;      // tiles of ONE density (n_tiles = nb * n_tiles1; nb = 1 for a single solve)
@@ -617,6 +620,22 @@ PF_HD void unpack_A(cx<typename G::T> *v, const B &b) {
     });
 }
 
+// Where thread (t, p) of `tile` finds its K^F vectors: (tile of the internal copy, thread slot in it).  Plain storage: the
+// thread's own tile and slot.  Folded storage (PassParams::k_fold): the tile / slot of the mirror pencil S_b - pp.
+template <class G>
+PF_HD void kf_slot(const PassParams &prm, int tile, int tid, int t, int p, int &ktile, int &ktid) {
+    const int tl1 = tile % prm.n_tiles1;                       // tile within one density
+    ktile = tl1 + prm.k_g0 * prm.tiles_per_g; ktid = tid;
+    if (prm.k_fold) {
+        const int g = tl1 / prm.tiles_per_g, pp = (tl1 % prm.tiles_per_g) * G::P + p;
+        int ppk = pp <= prm.k_fold / 2 ? pp : prm.k_fold - pp;
+        if (ppk < 0) ppk = 0;                                  // pencils past the end of a ragged tile (never used)
+        const int pk = ppk % G::P;
+        ktile = (g + prm.k_g0) * prm.k_tpg + ppk / G::P;
+        ktid = G::LANES_P ? t * G::P + pk : pk * G::TPP + t;
+    }
+}
+
 #ifndef PF_KPREF
 #define PF_KPREF 1   // pass F3 prefetches its K^F lines into L2 at the top of the tile (where PassParams::prefetch bit 1 is set)
 #endif
@@ -923,8 +942,13 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
     const typename KV::V *kint = reinterpret_cast<const typename KV::V *>(prm.kint);
     typename KV::V *kstage = reinterpret_cast<typename KV::V *>(stage + St::IN_ELEMS);
     (void)kstage;
+    auto kf_ptr = [&](int tile) -> const typename KV::V * {   // this thread's first K^F vector of `tile`
+        int ktile, ktid;
+        kf_slot<G>(prm, tile, tid, t, p, ktile, ktid);
+        return kint + (size_t)ktile * NKV * G::NT + ktid;
+    };
     auto issue_k = [&](int tile) {
-        const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1 + prm.k_g0 * prm.tiles_per_g) * NKV * G::NT + tid;
+        const typename KV::V *kp = kf_ptr(tile);
         static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; cp_async_vec16(kstage + q * G::NT + tid, kp + (size_t)q * G::NT, pol); });
     };
     tile_loop<G, Buf, St::ON, (St::KON ? 1 : 0)>(bid, nb, prm.n_tiles, prm.pdl_trigger == 1,
@@ -940,11 +964,11 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
             if constexpr (St::ON) { PF_TILE_COORDS fetch_A<G, PRUNED, St>(b, stage, t, p, valid); }
             else fetch_fwd<G, PRUNED, false>(b, prm, tile, c);
             if (G::KLATE && !St::KON && KPREF && (prm.prefetch & 2)) {   // start this tile's K^F on its way DRAM -> L2 now
-                const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1 + prm.k_g0 * prm.tiles_per_g) * NKV * G::NT + tid;
+                const typename KV::V *kp = kf_ptr(tile);
                 static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; prefetch_l2(kp + (size_t)q * G::NT); });
             }
             if constexpr (K_EARLY) {
-                const typename KV::V *kp = kint + (size_t)(tile % prm.n_tiles1 + prm.k_g0 * prm.tiles_per_g) * NKV * G::NT + tid;
+                const typename KV::V *kp = kf_ptr(tile);
                 static_for<NKV>([&](auto qc) { constexpr int q = decltype(qc)::value; kvec_get(ld_stream_vec(kp + (size_t)q * G::NT), b.k + q * KV::N); });
             }
         },
@@ -957,7 +981,9 @@ PF_HD void body_f3(const PassParams &prm, int bid, int nb, int tid, void *smem) 
                     if (tile + nb < prm.n_tiles) issue_k(tile + nb);
                     cp_async_commit();
                 } else if constexpr (G::KLATE) {
-                    kmul_global<G>(v, prm.kint, tile % prm.n_tiles1 + prm.k_g0 * prm.tiles_per_g, tid);
+                    int ktile, ktid;
+                    kf_slot<G>(prm, tile, tid, t, p, ktile, ktid);
+                    kmul_global<G>(v, prm.kint, ktile, ktid);
                 } else {
                     static_for<G::V>([&](auto rc) { constexpr int r = decltype(rc)::value; v[r] = scale(v[r], b.k[r]); });
                 }

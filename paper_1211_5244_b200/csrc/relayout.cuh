@@ -12,6 +12,7 @@ namespace pfft {
 struct RelayoutParams {
     int RA, RB, TPP, P, V, NT, lanes_p;
     int tiles_per_g, n_p;
+    int fold;             // 0, or S_b: only pencils 0 .. S_b / 2 are stored (K^F even along axis b, poisson_set_kernel_even)
     int g0;               // first k_a plane held (sharded plans keep only their own planes; else 0)
     int a_axis, c_axis;   // the pencil index pp runs along the remaining axis
     int sx, sy, sz;
@@ -29,7 +30,7 @@ PF_HD T relayout_value(const T *kuser, const RelayoutParams &q, long long idx) {
     if (q.lanes_p) { p = tid % q.P; t = tid / q.P; } else { t = tid % q.TPP; p = tid / q.TPP; }
     const long long g = tile / q.tiles_per_g + q.g0;
     const long long pp = (tile % q.tiles_per_g) * q.P + p;
-    if (pp >= q.n_p) return (T)0;
+    if (pp >= q.n_p || (q.fold && pp > q.fold / 2)) return (T)0;   // folded storage keeps pencils 0 .. S_b / 2 (q.tiles_per_g tiles of them)
     const int i = r / q.RB, k1 = r % q.RB;
     if (t + q.TPP * i >= q.RA) return (T)0;      // ragged last column of layout B: this thread owns no k2 there
     const int kc = (t + q.TPP * i) + q.RA * k1;  // layout B of passes.cuh: k = k2 + RA*k1

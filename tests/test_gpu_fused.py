@@ -320,3 +320,86 @@ def test_tuner_reports_graph_shape(pk):
     finally:
         plan.close()
     assert rel_l2(V, oracle.solve(rho, Kf, (0, 0, 0))) <= 1e-12
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_even_kernel_folded_storage(pk, monkeypatch, prec):
+    """poisson_set_kernel_even (less K^F traffic): K^F of a kernel that is even along every axis is kept for
+    the pencils k_b <= S_b / 2 only; pass F3 reads the mirror pencil's values for the rest.  Same values, same arithmetic:
+    bitwise the result of poisson_set_kernel, for all 8 BCs (contiguous and strided F3, ragged tiles), in a forced graph of
+    parallel chains, through the batch route and plane chunks; the K^F buffer shrinks; switching back and forth works; a kernel
+    that is NOT even per axis differs (the evenness is the caller's statement)."""
+    import itertools
+    import torch
+    dt = np.float64 if prec == "fp64" else np.float32
+    prec_id = pk.FP64 if prec == "fp64" else pk.FP32
+    for n, env in (((24, 16, 32), {}), ((20, 40, 36), {"POISSON_GRAPH": "1", "POISSON_BRANCHES": "3"}), ((32, 12, 20), {"POISSON_CHUNK": "4"})):
+        for k in ("POISSON_GRAPH", "POISSON_BRANCHES", "POISSON_CHUNK"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        for bc in itertools.product((0, 1), repeat=3):
+            rng = np.random.default_rng(4242 + sum(n) + sum(b << i for i, b in enumerate(bc)))
+            s = gen.padded_shape(n, bc)
+            Kf = oracle.kernel_spectrum(_even_kernel(rng, s)).astype(dt)
+            # the computed spectrum is even along y and z up to rounding only: make it so exactly (a + b == b + a), so that
+            # the mirror pencil holds the SAME values and the comparison below can be bitwise
+            Kf = 0.5 * (Kf + np.roll(np.flip(Kf, axis=1), 1, axis=1))
+            Kf = np.ascontiguousarray(0.5 * (Kf + np.roll(np.flip(Kf, axis=0), 1, axis=0))).astype(dt)
+            rhos = [torch.from_numpy(rng.standard_normal((n[2], n[1], n[0])).astype(dt)).cuda() for _ in range(3)]
+            Kf_t = torch.from_numpy(Kf).cuda()
+            plan = pk.PoissonPlan(n, bc, 0.25, prec_id)
+            try:
+                plan.set_kernel(Kf_t)
+                refs = [plan.solve(r).clone() for r in rhos]
+                plan.solve_batch(rhos)                         # the batch route allocates its own intermediates: before the sizes are compared
+                torch.cuda.synchronize()
+                full_ws = plan.workspace_bytes()
+                plan.set_kernel_even(Kf_t)
+                assert plan.workspace_bytes() <= full_ws      # whole tiles of pencils are kept: tiny planes may not shrink
+                for rep in range(2):
+                    for r, ref in zip(rhos, refs):
+                        assert torch.equal(plan.solve(r), ref), (n, bc, prec)
+                for v, ref in zip(plan.solve_batch(rhos), refs):
+                    torch.cuda.synchronize()
+                    assert torch.equal(v, ref)
+                plan.set_kernel(Kf_t)                       # back to the full layout
+                assert plan.workspace_bytes() == full_ws
+                assert torch.equal(plan.solve(rhos[0]), refs[0])
+            finally:
+                plan.close()
+            if bc == (0, 1, 0) and not env:
+                ref = oracle.solve(rhos[0].cpu().numpy().astype(np.float64), Kf.astype(np.float64), bc)
+                assert rel_l2(refs[0].cpu().numpy().astype(np.float64), ref) <= (1e-12 if prec == "fp64" else 1e-5)
+    # a grid with many tiles per plane: the K^F copy shrinks to (S_b / 2 + 1) / S_b of its size, rounded up to whole tiles
+    plan = pk.PoissonPlan((64, 64, 64), (0, 0, 0), 0.2, prec_id)
+    try:
+        rng = np.random.default_rng(8)
+        Kf_t = torch.from_numpy(rng.standard_normal((128, 128, 65)).astype(dt)).cuda()
+        Kf_t = 0.5 * (Kf_t + torch.roll(torch.flip(Kf_t, dims=(1,)), 1, dims=(1,))).contiguous()     # even along y (= axis b)
+        rho = torch.from_numpy(rng.standard_normal((64, 64, 64)).astype(dt)).cuda()
+        plan.set_kernel(Kf_t)
+        full_ws = plan.workspace_bytes()
+        ref = plan.solve(rho).clone()
+        plan.set_kernel_even(Kf_t)
+        k_bytes = 65 * 128 * 128 * (8 if prec == "fp64" else 4)
+        assert full_ws - plan.workspace_bytes() >= 0.3 * k_bytes
+        assert torch.equal(plan.solve(rho), ref)
+    finally:
+        plan.close()
+    # inversion symmetric but not even per axis: the folded copy is a different kernel
+    n, bc = (8, 12, 4), (0, 1, 0)
+    rng = np.random.default_rng(5)
+    s = gen.padded_shape(n, bc)
+    K = rng.standard_normal((s[2], s[1], s[0]))
+    K = 0.5 * (K + np.roll(np.flip(K, axis=(0, 1, 2)), 1, axis=(0, 1, 2)))
+    Kf_t = torch.from_numpy(oracle.kernel_spectrum(K).astype(dt)).cuda()
+    rho = torch.from_numpy(rng.standard_normal((n[2], n[1], n[0])).astype(dt)).cuda()
+    plan = pk.PoissonPlan(n, bc, 0.3, prec_id)
+    try:
+        plan.set_kernel(Kf_t)
+        a = plan.solve(rho).clone()
+        plan.set_kernel_even(Kf_t)
+        assert not torch.equal(plan.solve(rho), a)
+    finally:
+        plan.close()

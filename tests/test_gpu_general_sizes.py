@@ -178,3 +178,48 @@ def test_general_sizes_through_batches_and_host_entry(pk):
             assert torch.equal(w, Vs[1])
         finally:
             plan.close()
+
+
+@pytest.mark.parametrize("n,bc", [((128, 16, 12), (0, 0, 0)), ((7, 5, 6), (1, 0, 1)), ((32, 6, 9), (0, 0, 1)), ((24, 20, 10), (1, 1, 0))])
+@pytest.mark.parametrize("pdl", [False, True], ids=["graph", "graph_pdl"])
+def test_kernel_kinds_in_a_shaped_graph(pk, monkeypatch, n, bc, pdl):
+    """One plan whose solve graph is FORCED into parallel chains (3 plane ranges x 2 x ranges where x ranges apply): real K^F,
+    folded even K^F, complex K^F (pass F3 switches to the any-length kernel: the graph is rebuilt, x ranges fall away), real
+    again -- every switch rebuilds the graph around pass F3's new parameters, and every result matches the oracle."""
+    import torch
+    monkeypatch.setenv("POISSON_GRAPH", "1")
+    monkeypatch.setenv("POISSON_BRANCHES", "3")
+    monkeypatch.setenv("POISSON_XCHAINS", "2")
+    if pdl:
+        monkeypatch.setenv("POISSON_PDL", "1")
+    rng = np.random.default_rng(77 + sum(n))
+    s = gen.padded_shape(n, bc)
+    rho = rng.standard_normal((n[2], n[1], n[0]))
+    Kfe = oracle.kernel_spectrum(_even_kernel(rng, s))
+    Kfe = 0.5 * (Kfe + np.roll(np.flip(Kfe, axis=1), 1, axis=1))
+    Kfe = np.ascontiguousarray(0.5 * (Kfe + np.roll(np.flip(Kfe, axis=0), 1, axis=0)))       # exactly even along y and z
+    Kc = oracle.kernel_spectrum_complex(rng.standard_normal((s[2], s[1], s[0])))
+    ref_real, ref_c = oracle.solve(rho, Kfe, bc), oracle.solve_complex(rho, Kc, bc)
+    plan = pk.PoissonPlan(n, bc, 0.25, pk.FP64)
+    try:
+        assert plan.launch_mode()[0] == ("graph_pdl" if pdl else "graph")
+        J, R = plan.graph_shape()
+        assert J == min(3, plan.info.half_len) and R in (1, 2)
+        r = torch.from_numpy(rho).cuda()
+        plan.set_kernel(torch.from_numpy(Kfe).cuda())
+        v1 = plan.solve(r).cpu().numpy()
+        try:
+            plan.set_kernel_even(torch.from_numpy(Kfe).cuda())
+            v2 = plan.solve(r).cpu().numpy()
+            assert np.array_equal(v1, v2)
+        except pk.PoissonError as e:
+            assert e.status == 2                      # pass F3 of this grid runs the any-length kernel: folded storage refused
+        plan.set_kernel_complex(torch.from_numpy(Kc).cuda())
+        v3 = plan.solve(r).cpu().numpy()
+        assert plan.graph_shape()[0] == J             # still chains over plane ranges
+        plan.set_kernel(torch.from_numpy(Kfe).cuda())
+        v4 = plan.solve(r).cpu().numpy()
+    finally:
+        plan.close()
+    assert rel_l2(v1, ref_real) <= 1e-12 and rel_l2(v4, ref_real) <= 1e-12
+    assert rel_l2(v3, ref_c) <= 1e-12

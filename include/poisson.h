@@ -236,7 +236,8 @@ POISSON_API int poisson_plan_launch_mode(const poisson_plan *plan, int *mode /* 
  * grid hands its SM slots to that successor while its siblings still run, which hides the ramp-up and tail of the
  * passes inside ONE solve (128^3 -> 256^3 fp64 on B200: 98.4 us as a chain, 92.3 with J = 4, 90.6 with J = R = 2).
  * poisson_plan_create times a few shapes together with the launch modes; POISSON_BRANCHES=J / POISSON_XCHAINS=R fix one.
- * x ranges need x as the last-processed axis and whole tiles per range, else R = 1.  Outputs 1, 1 in the other modes.
+ * When x is processed second (surface grids) the R ranges run along the other axis F1 / F2 / I2 / I1 do not couple on (the split axis o)
+ * instead of x.  Ranges must hold whole tiles, else R = 1.  Outputs 1, 1 in the other modes.
  * Errors: EINVAL. */
 POISSON_API int poisson_plan_graph_shape(const poisson_plan *plan, int *plane_chains /* host, out */, int *x_chains /* host, out */);
 

@@ -967,8 +967,9 @@ static int run_passes(poisson_plan *pl, const void *rho, void *V, cudaStream_t s
 }
 
 // Builds the graph of one solve on the plan's own intermediates (explicit kernel nodes, plain dependencies).
-// Parameters of pass q restricted to the k_a planes [g0, g0 + ng) (middle passes F2, F3, I2) and / or to the pencils
-// x in [x0, x0 + nx) (F1, F2, I2, I1 when their pencil index is the x axis; nx = 0: all) of the full-size arrays.
+// Parameters of pass q restricted to the k_a planes [g0, g0 + ng) (middle passes F2, F3, I2) and / or to the range
+// [x0, x0 + nx) (nx = 0: all) of the axis along which F1 / F2 / I2 / I1 do not couple: x when x is processed last (their pencil
+// index), else the axis o (b = x: F1 / I1's group index, F2 / I2's pencil index) -- on the full-size arrays.
 static PassParams range_params(const poisson_plan *pl, int q, const Lane *ln, int g0, int ng, int x0 = 0, int nx = 0) {
     const size_t cplx = 2 * pl->elem_real;
     PassParams prm = pass_params(pl, q, nullptr, nullptr, ln);
@@ -982,7 +983,10 @@ static PassParams range_params(const poisson_plan *pl, int q, const Lane *ln, in
     }
     if (nx > 0) {
         const int e = pl->k[q]->P;
-        if (ends) {   // pencils are x-pairs: rho / V in pairs, A1 in complex numbers (two per pair)
+        if (ends && pl->d.order[1] == 0) {   // b = x: the range runs along F1 / I1's group index g (the axis o, which is F2 / I2's pencil index)
+            ng = nx;
+            off_in += (long long)x0 * prm.gs_in; off_out += (long long)x0 * prm.gs_out;
+        } else if (ends) {   // c = x: pencils are x-pairs: rho / V in pairs, A1 in complex numbers (two per pair)
             const int x0p = x0 / 2, nxp = nx / 2;
             prm.n_p = nxp; prm.tiles_per_g = (nxp + e - 1) / e;
             if (q == POISSON_PASS_F1) { off_in += (long long)x0p * prm.ps_in; off_out += 2LL * x0p * prm.ps_out; }
@@ -1029,16 +1033,19 @@ static int build_graph(poisson_plan *pl, GraphSolve &g, const Lane *ln) {
     const bool shaped = pl->n_chunks <= 1 && !ln;   // batch lanes already overlap each other: plain chains there (measured: 90.3 vs 92.8 us)
     const int B = shaped ? (pl->branches < pl->d.H ? pl->branches : pl->d.H) : 1;
     int R = shaped ? pl->xchains : 1;
-    {   // x chains need: no plane chunks, the register engine everywhere, x as the pencil index of F1 / F2 / I2 / I1, whole tiles per range
-        bool ok = R > 1 && pl->n_chunks <= 1 && pl->d.order[2] == 0;
+    int n_chain = pl->d.n[0];   // points of the chain axis: x when it is processed last, else the axis o (= c when b = x)
+    {   // x chains need: no plane chunks, the register engine everywhere, whole tiles per range
+        bool ok = R > 1 && pl->n_chunks <= 1;
         for (int q = 0; q < 5 && ok; ++q) ok = !pl->k[q]->generic;
-        if (ok) ok = pl->d.n[0] % (R * 2 * pl->k[0]->P) == 0 && pl->d.n[0] % (R * pl->k[1]->P) == 0;
+        if (ok && pl->d.order[2] == 0) ok = pl->d.n[0] % (R * 2 * pl->k[0]->P) == 0 && pl->d.n[0] % (R * pl->k[1]->P) == 0;
+        else if (ok && pl->d.order[1] == 0) { n_chain = pl->d.n[pl->d.order[2]]; ok = n_chain % (R * pl->k[1]->P) == 0; }
+        else ok = false;
         if (!ok) R = 1;
     }
     if (R > 1) {
         // F1_r -> F2_{r,j} -> F3_j -> I2_{r,j} -> I1_r: r = range of x (F1 / F2 / I2 / I1 tiles only couple along y resp. k_a),
         // j = range of k_a planes (F3 couples along x).  Every kernel except F3 has a successor that only needs part of the grid.
-        const int J = B > 1 ? B : 1, nxr = pl->d.n[0] / R;
+        const int J = B > 1 ? B : 1, nxr = n_chain / R;
         std::vector<cudaGraphNode_t> f1(R), i1(R), f2(R * J), f3(J), i2(R * J);
         g.node_f1 = nullptr; g.node_i1 = nullptr;   // rho / V are patched into R nodes each: see run_graph
         g.xr = R;

@@ -249,7 +249,9 @@ def test_shaped_graph_bitwise_and_vs_oracle(pk, monkeypatch, shape, pdl):
     import torch
     J, R = shape
     # x ranges need whole tiles: 128 x values = 4 ranges of 2 P = 32 reals in F1 / I1 (S = 64: 8 threads per pencil, P = 16)
-    cases = [((128, 32, 32), (0, 0, 0), True), ((128, 32, 64), (0, 0, 1), True), ((32, 24, 16), (1, 1, 0), False), ((15, 12, 10), (0, 1, 0), False)]
+    # the surface grid processes x second: its chains run over ranges of z (F1 / I1's group index, F2 / I2's pencil index), 64 = 4 x 16 pencils
+    cases = [((128, 32, 32), (0, 0, 0), True), ((128, 32, 64), (0, 0, 1), True), ((64, 16, 64), (1, 1, 0), True), ((64, 64, 12), (1, 0, 0), True),
+             ((32, 24, 16), (1, 1, 0), False), ((15, 12, 10), (0, 1, 0), False)]
     for n, bc, x_ok in cases:
         rng = np.random.default_rng(77 + sum(n) + J + 10 * R)
         s = gen.padded_shape(n, bc)

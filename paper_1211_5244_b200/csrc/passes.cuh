@@ -36,6 +36,15 @@ enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4,
                 KIND_F1S = 5, KIND_I2S = 6 };
 PF_CE int base_kind(int kind) { return kind == KIND_F1S ? KIND_F1 : (kind == KIND_I2S ? KIND_I2 : kind); }
 
+// Which transforms take two-level inter-pass twiddles (Geo::TW2F / TW2I): fp64, twiddled radix 8 .. 16.  Measured on B200 (DESIGN.md
+// section 10c): the load/store pipe is the busiest unit of these kernels (74 % in F3 at S = 256) and 25 % of its work is twiddle loads;
+// rows 1, 2, 3, 4, 8, 12 of the table and one more complex multiply per element instead of 15 rows: 128^3 -> 256^3 94.4 -> 90.0 us per
+// solve, 256^3 -> 512^3 797 -> 770.  Radix 32 (10 loads, 21 more multiplies) loses, fp32 is issue bound: both keep one load per element.
+#ifndef PF_TW2
+#define PF_TW2 1     // 0: every twiddle from the table (A/B builds)
+#endif
+PF_CE bool tw2_radix(int R, int real_bytes) { return PF_TW2 != 0 && real_bytes == 8 && R >= 8 && R <= 16; }
+
 // ------------------------------------------------------------------ geometry
 // NBUF_   : exchange buffers (2 = one barrier per exchange, 1 = half the shared memory, one more barrier)
 // TWS_    : twiddles w_S^{n1 k2} read from a shared-memory table (true) or held in registers (false)
@@ -62,6 +71,11 @@ struct Geo {
     static constexpr bool WARP_LOCAL = !LANES_P_ && (32 % TPP_ == 0);
     static PF_HD void xsync() { if (WARP_LOCAL) warp_sync(); else cta_sync(); }
     static constexpr bool TWS = TWS_ && RB_ > 1;
+    // two-level twiddles (shared-memory tables only): w^{n1 k2} = w^{n1 (k2 mod 4)} * w^{n1 4 floor(k2 / 4)} -- rows 1, 2, 3 and
+    // 4, 8, 12, ... of the table instead of all of them: 3 + (R - 1) / 4 loads per column instead of R - 1, one more complex
+    // multiply for the elements with both factors (tw2_radix)
+    static constexpr bool TW2F = TWS && tw2_radix(RA_, (int)sizeof(T_));   // forward direction: the RA outputs of the first pass are twiddled
+    static constexpr bool TW2I = TWS && tw2_radix(RB_, (int)sizeof(T_));   // inverse direction: the RB outputs of its first pass
     static_assert(NBUF == 1 || NBUF == 2, "one or two exchange buffers");
     static_assert(RA * RB == S, "S = RA * RB");
     // TPP divides RB; it need not divide RA: a thread then owns ceil(RA / TPP) columns k2 = t + TPP*i of layout B,
@@ -236,10 +250,24 @@ PF_HD void fwd_AtoB(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::
         if constexpr (RB > 1) {
             const int n1 = t + G::TPP * i;
             xb[G::xidx(p, n1, 0)] = u[0];
-            static_for<RA - 1>([&](auto kc) {
-                constexpr int k2 = decltype(kc)::value + 1;
-                xb[G::xidx(p, n1, k2)] = u[k2] * tw.template fwd<i, k2>(t);
-            });
+            if constexpr (G::TW2F) {
+                constexpr int NH = (RA - 1) / 4;
+                cx<T> wl[3], wh[NH > 0 ? NH : 1];
+                static_for<3>([&](auto jc) { constexpr int j = decltype(jc)::value; if constexpr (j + 1 < RA) wl[j] = tw.template fwd<i, j + 1>(t); });
+                static_for<NH>([&](auto ac) { constexpr int a = decltype(ac)::value; wh[a] = tw.template fwd<i, 4 * (a + 1)>(t); });
+                static_for<RA - 1>([&](auto kc) {
+                    constexpr int k2 = decltype(kc)::value + 1;
+                    cx<T> val = u[k2];
+                    if constexpr (k2 % 4 != 0) val = val * wl[k2 % 4 - 1];
+                    if constexpr (k2 / 4 != 0) val = val * wh[k2 / 4 - 1];
+                    xb[G::xidx(p, n1, k2)] = val;
+                });
+            } else {
+                static_for<RA - 1>([&](auto kc) {
+                    constexpr int k2 = decltype(kc)::value + 1;
+                    xb[G::xidx(p, n1, k2)] = u[k2] * tw.template fwd<i, k2>(t);
+                });
+            }
         }
     });
     if constexpr (RB > 1) {
@@ -273,10 +301,24 @@ PF_HD void inv_BtoA(cx<typename G::T> *v, const Twiddles<G> &tw, cx<typename G::
             if (G::template b_on<i>(t)) {
                 dft<T, RB, true>(g);
                 xb[G::xidx(p, 0, k2)] = g[0];
-                static_for<RB - 1>([&](auto nc) {
-                    constexpr int n1 = decltype(nc)::value + 1;
-                    xb[G::xidx(p, n1, k2)] = mul_conj(g[n1], tw.template inv<i, n1>(t));
-                });
+                if constexpr (G::TW2I) {
+                    constexpr int NH = (RB - 1) / 4;
+                    cx<T> wl[3], wh[NH > 0 ? NH : 1];
+                    static_for<3>([&](auto jc) { constexpr int j = decltype(jc)::value; if constexpr (j + 1 < RB) wl[j] = tw.template inv<i, j + 1>(t); });
+                    static_for<NH>([&](auto ac) { constexpr int a = decltype(ac)::value; wh[a] = tw.template inv<i, 4 * (a + 1)>(t); });
+                    static_for<RB - 1>([&](auto nc) {
+                        constexpr int n1 = decltype(nc)::value + 1;
+                        cx<T> val = g[n1];
+                        if constexpr (n1 % 4 != 0) val = mul_conj(val, wl[n1 % 4 - 1]);
+                        if constexpr (n1 / 4 != 0) val = mul_conj(val, wh[n1 / 4 - 1]);
+                        xb[G::xidx(p, n1, k2)] = val;
+                    });
+                } else {
+                    static_for<RB - 1>([&](auto nc) {
+                        constexpr int n1 = decltype(nc)::value + 1;
+                        xb[G::xidx(p, n1, k2)] = mul_conj(g[n1], tw.template inv<i, n1>(t));
+                    });
+                }
             }
         });
         G::xsync();

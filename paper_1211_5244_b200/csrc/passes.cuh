@@ -36,14 +36,18 @@ enum PassKind { KIND_F1 = 0, KIND_F2 = 1, KIND_F3 = 2, KIND_I2 = 3, KIND_I1 = 4,
                 KIND_F1S = 5, KIND_I2S = 6 };
 PF_CE int base_kind(int kind) { return kind == KIND_F1S ? KIND_F1 : (kind == KIND_I2S ? KIND_I2 : kind); }
 
-// Which transforms take two-level inter-pass twiddles (Geo::TW2F / TW2I): fp64, twiddled radix 8 .. 16.  Measured on B200 (DESIGN.md
+// Which transforms take two-level inter-pass twiddles (Geo::TW2F / TW2I): fp64, twiddled radix 8 .. 24.  Measured on B200 (DESIGN.md
 // section 10c): the load/store pipe is the busiest unit of these kernels (74 % in F3 at S = 256) and 25 % of its work is twiddle loads;
 // rows 1, 2, 3, 4, 8, 12 of the table and one more complex multiply per element instead of 15 rows: 128^3 -> 256^3 94.4 -> 90.0 us per
-// solve, 256^3 -> 512^3 797 -> 770.  Radix 32 (10 loads, 21 more multiplies) loses, fp32 is issue bound: both keep one load per element.
+// solve, 256^3 -> 512^3 797 -> 770; radix 24 (8 rows instead of 23): 96^3 -> 192^3 49.2 -> 47.2.  Radix 32 (10 loads, 21 more multiplies)
+// loses, fp32 is issue bound: both keep one load per element.
 #ifndef PF_TW2
 #define PF_TW2 1     // 0: every twiddle from the table (A/B builds)
 #endif
-PF_CE bool tw2_radix(int R, int real_bytes) { return PF_TW2 != 0 && real_bytes == 8 && R >= 8 && R <= 16; }
+#ifndef PF_TW2_MAXR
+#define PF_TW2_MAXR 24
+#endif
+PF_CE bool tw2_radix(int R, int real_bytes) { return PF_TW2 != 0 && real_bytes == 8 && R >= 8 && R <= PF_TW2_MAXR; }
 
 // ------------------------------------------------------------------ geometry
 // NBUF_   : exchange buffers (2 = one barrier per exchange, 1 = half the shared memory, one more barrier)

@@ -553,9 +553,14 @@ def run_ours(args):
         for key in ("c0", "c2", "c3", "c4a", "c4b", "c4p"):
             if key == args.config:
                 continue
+            smp = ClockSampler(local)
+            smp.start()
             r = time_config(pk, torch, key, min(steps, 200), 5, with_e2e=True, with_cold=False)
+            clk = smp.stop()
             i2 = r["info"]
             others[key] = {"workload": WORKLOAD_TEXT[key], "ms_per_step": r["single"]["ms"],
+                           "ms_per_step_min": r["single"]["min"], "ms_per_step_max": r["single"]["max"], "timed_regions": r["single"]["regions"],
+                           "clocks": clk,
                            "solves_per_sec": 1e3 / r["single"]["ms"],
                            "hbm_frac": i2.bytes_total / (r["single"]["ms"] * 1e-3) / 1e9 / peak,
                            "batched_ms_per_step": r["batch"]["ms"],

@@ -836,11 +836,17 @@ PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
     unpack_A<G, PRUNED>(v, b);
     fwd_AtoB<G, PRUNED>(v, c.tw, c.xbufs.next(), t, p);
     cx<T> *xn = c.xbufs.next();
+    // A thread's layout-B values are Z_k for k = t + TPP m', m' = i + CB k1 -- exactly the k = t + TPP m it writes out below (when TPP
+    // divides RA), so Z_k is already in its registers and only Z_{S-k} has to come from another thread: the exchange carries the upper
+    // half of the spectrum (k > S/2) only, half the shared-memory stores and half the loads of a full natural-order exchange.
+    constexpr bool LEAN = !G::RAGGED_B && (S / 2) % G::TPP == 0;
+    constexpr int HM = S / 2 / G::TPP;        // m' >= HM  <=>  k >= S/2
     static_for<G::CB>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         static_for<G::RB>([&](auto kc) {
             constexpr int k1 = decltype(kc)::value;
-            if (G::template b_on<i>(t)) xn[G::nidx(p, (t + G::TPP * i) + G::RA * k1)] = v[i * G::RB + k1];
+            if constexpr (!LEAN || i + G::CB * k1 >= HM)
+                if (G::template b_on<i>(t)) xn[G::nidx(p, (t + G::TPP * i) + G::RA * k1)] = v[i * G::RB + k1];
         });
     });
     cta_sync();
@@ -850,7 +856,14 @@ PF_HD void process_f1(BufA<G, PRUNED> &b, const PassParams &prm, int tile, TileC
         constexpr int m = decltype(mc)::value;
         const int k = t + G::TPP * m;
         if (k < NK && valid) {
-            const cx<T> zk = xn[G::nidx(p, k)], zp = xn[G::nidx(p, (S - k) % S)];
+            cx<T> zk, zp;
+            if constexpr (LEAN) {
+                zk = v[(m % G::CB) * G::RB + m / G::CB];
+                const cx<T> zr = xn[G::nidx(p, (S - k) % S)];                  // in range for every k (slot 0 is never written: not used)
+                zp = (k == 0 || 2 * k == S) ? zk : zr;                         // Z_0 and Z_{S/2} pair with themselves
+            } else {
+                zk = xn[G::nidx(p, k)]; zp = xn[G::nidx(p, (S - k) % S)];
+            }
             const T hf = (T)0.5;
             // A = (Z_k + conj Z_{S-k})/2 ; B = -i (Z_k - conj Z_{S-k})/2
             const cx<T> fa = mk<T>(hf * (zk.re + zp.re), hf * (zk.im - zp.im)), fb = mk<T>(hf * (zk.im + zp.im), hf * (zp.re - zk.re));

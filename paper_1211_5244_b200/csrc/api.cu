@@ -69,10 +69,10 @@ static const void *generic_func(int kind) {
 }
 
 // Radices of S for the Stockham passes: the fewest passes over the tile with radices the kernel holds in registers
-// ({2,3,4,5,6,8,10,12,16} via fft_core.cuh, 7 / 11 / 13 as written-out sums); larger radices first (their twiddle-free last
+// ({2,3,4,5,6,8,10,12,14,15,16} via fft_core.cuh, 7 / 11 / 13 as written-out sums); larger radices first (their twiddle-free last
 // stage is the cheapest); any other prime factor runs the one-output-per-thread fallback.
 static int generic_factors(int S, int fac[16]) {
-    static const int allowed[] = {16, 13, 12, 11, 10, 8, 7, 6, 5, 4, 3, 2};
+    static const int allowed[] = {16, 15, 14, 13, 12, 11, 10, 8, 7, 6, 5, 4, 3, 2};
     int n = 0, rest = S;
     // strip the prime factors the register butterflies do not cover (17 and up)
     int big[16], nbig = 0;
@@ -81,17 +81,22 @@ static int generic_factors(int S, int fac[16]) {
         for (int p : {2, 3, 5, 7, 11, 13}) while (r % p == 0) r /= p;
         for (int p = 17; r > 1; p += 2) while (r % p == 0) { if (nbig == 16) return -1; big[nbig++] = p; r /= p; rest /= p; }
     }
-    // fewest stages for the smooth part: depth-first over the allowed radices, non-increasing order
-    int best[16], nbest = 99, cur[16];
+    // fewest stages for the smooth part: depth-first over the allowed radices, non-increasing order; among equally short lists the
+    // one with the smallest sum of radices (balanced radices: every stage is one sweep over the tile, whatever its radix, so a
+    // radix-2 stage buys nothing -- 300 = 5 x 5 x 12 rather than 2 x 10 x 15)
+    int best[16], nbest = 99, cur[16], best_sum = 1 << 30;
     struct Rec {
-        static void go(int r, int start, int depth, int *cur, int *best, int &nbest, const int *allowed) {
-            if (r == 1) { if (depth < nbest) { nbest = depth; for (int i = 0; i < depth; ++i) best[i] = cur[i]; } return; }
-            if (depth + 1 >= nbest || depth >= 15) return;
-            for (int i = start; i < 12; ++i)
-                if (r % allowed[i] == 0) { cur[depth] = allowed[i]; go(r / allowed[i], i, depth + 1, cur, best, nbest, allowed); }
+        static void go(int r, int start, int depth, int sum, int *cur, int *best, int &nbest, int &best_sum, const int *allowed) {
+            if (r == 1) {
+                if (depth < nbest || (depth == nbest && sum < best_sum)) { nbest = depth; best_sum = sum; for (int i = 0; i < depth; ++i) best[i] = cur[i]; }
+                return;
+            }
+            if (depth + 1 > nbest || depth >= 15) return;
+            for (int i = start; i < 14; ++i)
+                if (r % allowed[i] == 0) { cur[depth] = allowed[i]; go(r / allowed[i], i, depth + 1, sum + allowed[i], cur, best, nbest, best_sum, allowed); }
         }
     };
-    Rec::go(rest, 0, 0, cur, best, nbest, allowed);
+    Rec::go(rest, 0, 0, 0, cur, best, nbest, best_sum, allowed);
     if (nbest == 99) return rest == 1 ? 0 : -1;
     if (nbest + nbig > 16) return -1;
     for (int i = 0; i < nbig; ++i) fac[n++] = big[i];         // the slow radices first (their pass has w_n^{jk} anyway)

@@ -250,7 +250,7 @@ template <typename T, bool INV> struct Dft<T, 7, INV> {
 
 // first factor A of the Cooley-Tukey split R = A * B used for composite radices
 PF_CE int split_a(int R) {
-    return R == 6 ? 2 : R == 8 ? 2 : R == 10 ? 2 : R == 12 ? 3 : R == 14 ? 2 : R == 16 ? 4 : R == 20 ? 4
+    return R == 6 ? 2 : R == 8 ? 2 : R == 10 ? 2 : R == 12 ? 3 : R == 14 ? 2 : R == 15 ? 3 : R == 16 ? 4 : R == 20 ? 4
          : R == 24 ? 3 : R == 28 ? 4 : R == 32 ? 4 : 0;
 }
 

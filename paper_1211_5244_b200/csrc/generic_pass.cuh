@@ -11,7 +11,7 @@
 //         y[q + s (R j + k)] = w_n^{j k}  sum_{r < R}  x[q + s (j + m r)]  w_R^{r k}      j < m, q < s, k < R
 //         swap(x, y);  n = m;  s = s R
 //
-// (natural order in, natural order out, no bit reversal).  The radices are chosen by the plan from {16, 12, 10, 8, 6, 5, 4,
+// (natural order in, natural order out, no bit reversal).  The radices are chosen by the plan from {16, 15, 14, 12, 10, 8, 6, 5, 4,
 // 3, 2} (the in-register DFTs of fft_core.cuh: a thread holds a whole butterfly), 7 / 11 / 13 (the R-term sums written
 // out in registers) and, for any other prime factor p, a fallback that forms one output per thread per step -- O(p) per
 // point.  Lengths up to 1024 with a prime factor >= 17 instead take Bluestein's chirp-z (gen_transform below): two smooth
@@ -73,7 +73,7 @@ __device__ __noinline__ void gen_stage(const cx<T> *x, cx<T> *y, const cx<T> *tw
         cx<T> a[R];
         const cx<T> *src = x + (q + s * j) * PP + p;
         static_for<R>([&](auto rc) { constexpr int r = decltype(rc)::value; a[r] = src[r * istride]; });
-        if constexpr (R == 7 || R == 11 || R == 13) gen_dft_prime<T, R, INV>(a, tw, S / R);
+        if constexpr (R == 11 || R == 13) gen_dft_prime<T, R, INV>(a, tw, S / R);   // radix 7 has literal twiddles in fft_core.cuh
         else dft<T, R, INV>(a);
         cx<T> *dst = y + (q + s * R * j) * PP + p;
         dst[0] = a[0];
@@ -126,6 +126,8 @@ PF_HD void gen_stage_dispatch(const cx<T> *x, cx<T> *y, const cx<T> *tw, int S, 
         case 11: gen_stage<T, 11, INV>(x, y, tw, S, P, n, s, tid); break;
         case 12: gen_stage<T, 12, INV>(x, y, tw, S, P, n, s, tid); break;
         case 13: gen_stage<T, 13, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 14: gen_stage<T, 14, INV>(x, y, tw, S, P, n, s, tid); break;
+        case 15: gen_stage<T, 15, INV>(x, y, tw, S, P, n, s, tid); break;
         case 16: gen_stage<T, 16, INV>(x, y, tw, S, P, n, s, tid); break;
         default: gen_stage_any<T>(x, y, tw, S, P, n, s, R, INV, tid); break;
     }

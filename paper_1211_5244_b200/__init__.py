@@ -14,6 +14,7 @@ __all__ = [
     "FREE", "PERIODIC", "FP64", "FP32", "PoissonError", "PlanInfo", "lib_path", "load_library",
     "poisson_plan_describe", "poisson_plan_create", "poisson_set_kernel", "poisson_solve",
     "poisson_solve_host", "poisson_plan_destroy", "poisson_measure_fma_peak", "PoissonPlan", "EXPORTED_SYMBOLS",
+    "poisson_set_kernel_even", "poisson_set_kernel_complex", "poisson_shard_describe", "ShardInfo", "ShardPlan", "ShardedSolver",
 ]
 
 FREE, PERIODIC = 0, 1

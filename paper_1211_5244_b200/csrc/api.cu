@@ -1261,16 +1261,26 @@ static int tune_plan(poisson_plan *pl) {
     }
     if ((e_tune && e_tune[0] == '0') || e_pdl || (e_fused && e_fused[0] == '1')) return POISSON_OK;   // forced / off
     const size_t bytes = (size_t)pl->d.n[0] * pl->d.n[1] * pl->d.n[2] * pl->elem_real;
-    void *rho = nullptr, *V = nullptr;
+    // rho / V rotate over a ring whose footprint exceeds the L2 (as a caller's fresh densities do: a ring that stays L2 resident makes
+    // F1 look faster than it is and shifts the choice between close candidates); grids whose single density already exceeds half
+    // the L2 take one buffer each
+    int nring = (int)(((size_t)160 << 20) / (2 * bytes)) + 1;
+    if (nring > 8) nring = 8;
+    void *ring = nullptr, *rho = nullptr, *V = nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     cudaStream_t ts = nullptr;   // a private non-blocking stream: tuning never synchronises with the caller's streams
     int rc = POISSON_OK;
-    auto cleanup = [&] { cudaFree(rho); cudaFree(V); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); if (ts) cudaStreamDestroy(ts); };
+    auto cleanup = [&] { cudaFree(ring); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); if (ts) cudaStreamDestroy(ts); };
     if (cudaStreamCreateWithFlags(&ts, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return POISSON_OK; }
-    if (cudaMalloc(&rho, bytes) != cudaSuccess || cudaMalloc(&V, bytes) != cudaSuccess) {   // no room to tune: keep defaults
-        cudaGetLastError(); cleanup(); return POISSON_OK;
+    const size_t slot = (bytes + 255) & ~(size_t)255;
+    if (cudaMalloc(&ring, 2 * slot * nring) != cudaSuccess) {
+        cudaGetLastError(); nring = 1;
+        if (cudaMalloc(&ring, 2 * slot) != cudaSuccess) { cudaGetLastError(); cleanup(); return POISSON_OK; }   // no room to tune: keep defaults
     }
-    cudaMemsetAsync(rho, 0, bytes, ts);
+    rho = ring; V = static_cast<char *>(ring) + slot * nring;
+    auto ring_rho = [&](int i) { return static_cast<const void *>(static_cast<const char *>(rho) + slot * (i % nring)); };
+    auto ring_V = [&](int i) { return static_cast<void *>(static_cast<char *>(V) + slot * (i % nring)); };
+    cudaMemsetAsync(ring, 0, 2 * slot * nring, ts);
     cudaMemsetAsync(pl->kint, 0, (size_t)pl->kint_elems * pl->elem_real, ts);
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { cudaGetLastError(); cleanup(); return POISSON_OK; }
     const bool modes[5][3] = {{false, false, false}, {true, false, false}, {false, true, false}, {false, false, true}, {true, false, true}};   // {pdl, fused, graph}
@@ -1281,7 +1291,7 @@ static int tune_plan(poisson_plan *pl) {
         float ms = 0.f, best_round = 1e30f;
         for (int round = 0; round < 3 && rc == POISSON_OK; ++round) {   // round 0: warm-up + pick the repeat count; then the faster of two
             cudaEventRecord(e0, ts);
-            for (int i = 0; i < reps && rc == POISSON_OK; ++i) rc = run_solve(pl, rho, V, ts);
+            for (int i = 0; i < reps && rc == POISSON_OK; ++i) rc = run_solve(pl, ring_rho(i), ring_V(i), ts);
             cudaEventRecord(e1, ts);
             if (cudaEventSynchronize(e1) != cudaSuccess) { rc = cuda_fail(cudaGetLastError(), "tuning solve"); return 0.f; }
             cudaEventElapsedTime(&ms, e0, e1);
@@ -1318,7 +1328,13 @@ static int tune_plan(poisson_plan *pl) {
         if (modes[m][2] && !(modes[m][0] ? pl->gs_pdl.exec : pl->gs.exec)) continue;
         pl->use_pdl = modes[m][0]; pl->use_fused = modes[m][1]; pl->use_graph = modes[m][2];
         const float ms = time_mode();
-        if (rc == POISSON_OK) { pl->tune_ms[m] = ms; if (ms < 0.99f * best_ms) { best_ms = ms; best = m; } }   // a later mode must win by more than the timing noise
+        if (rc == POISSON_OK) {
+            pl->tune_ms[m] = ms;
+            // the timing loop queues launches ahead of the device; a caller that issues one solve at a time pays the host cost of five
+            // stream launches (about 4 us each with the call around them) against one graph launch: stream modes count as >= 20 us
+            const float eff = (!modes[m][1] && !modes[m][2] && ms < 0.020f) ? 0.020f : ms;
+            if (eff < 0.99f * best_ms) { best_ms = eff; best = m; }   // a later mode must win by more than the timing noise
+        }
     }
     pl->use_pdl = modes[best][0]; pl->use_fused = modes[best][1]; pl->use_graph = modes[best][2];
     cleanup();

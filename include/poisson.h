@@ -309,6 +309,37 @@ POISSON_API int poisson_shard_forward(poisson_plan *plan, const void *rho_local_
 POISSON_API int poisson_shard_middle(poisson_plan *plan, void *stream);
 POISSON_API int poisson_shard_inverse(poisson_plan *plan, void *V_local_dev, void *stream);
 
+/* ---- One solve for callers that cannot allocate device memory.
+ * Everything above needs a plan, and a plan is made of cudaMalloc'ed buffers (intermediates, its copy of K^F, twiddle
+ * tables).  Some programs cannot give it that: a simulation code that took all of the GPU's memory for its own pool at
+ * start-up, so that a cudaMalloc made by a library it calls simply fails; a process held to a fixed memory budget by
+ * its job scheduler; or an inner loop (an SCF cycle, a time step) in which the device-wide synchronisation hidden in
+ * cudaMalloc / cudaFree, or an out-of-memory error at step 10 000, is not acceptable.  For them this ONE call does a
+ * whole solve -- K^F re-layout, F1, F2, F3, I2, I1: the same kernels, the same kernel choice, hence the same bits as
+ * poisson_plan_create + poisson_set_kernel + poisson_solve -- and calls no cudaMalloc, cudaFree or other allocating
+ * routine.  Its scratch is a fixed array of POISSON_STATIC_SCRATCH_BYTES that is part of the library image: every GPU
+ * on which the process uses this library holds that much from the moment the library's code is loaded there until the
+ * process exits, whether or not this function is ever called.
+ *   nx, ny, nz, bc, precision: the problem, as for poisson_plan_create (no h: it is metadata there)
+ *   K_f_dev : device, the spectrum exactly as poisson_set_kernel takes it (real, even kernel; [S_z][S_y][S_x/2+1]);
+ *             it is re-laid on EVERY call -- there is no plan to remember it -- which costs one extra sweep over K^F
+ *   rho_dev, V_dev: device, as for poisson_solve (16-byte aligned, rho_dev == V_dev allowed)
+ * Limit: tables (576 KiB) + A1 + A2 + the K^F copy must fit the array.  32^3 -> 64^3 free (3.3 MB) and 64^3 -> 128^3
+ * free in fp64 (21.9 MB) fit, 96^3 -> 192^3 fp64 does not; a grid that does not fit is refused with POISSON_EUNSUPPORTED
+ * and poisson_last_error() says how many bytes it would need.  Nothing is launched in that case.
+ * Sharing: there is one array per GPU and every call on that GPU uses it.  Two calls whose GPU work can overlap (two
+ * streams, two host threads with their own streams) overwrite each other's intermediates: order them yourself (same
+ * stream, or an event between them).  The host side is serialised by a mutex.  The array keeps what the last call left
+ * in it; no call depends on that (each call writes every byte before it reads it -- nothing has to be zeroed), except
+ * the twiddle tables, which are kept on purpose and re-uploaded only when a transform length or the precision changes.
+ * First call on a device: resolves the array's device address (cudaGetSymbolAddress, with that device current) and
+ * checks the architecture; the first call for a new set of transform lengths copies their tables from ordinary host
+ * memory, which makes the host wait for the work already queued on `stream`.  Make that first call outside any
+ * stream capture.  Asynchronous otherwise.  Errors: EINVAL, EUNSUPPORTED (also: over the limit), ECUDA, EARCH. */
+#define POISSON_STATIC_SCRATCH_BYTES (32u << 20)
+POISSON_API int poisson_solve_static(int nx, int ny, int nz, const int bc[3] /* host; x,y,z */, int precision,
+                                     const void *K_f_dev, const void *rho_dev, void *V_dev, void *stream);
+
 POISSON_API const char *poisson_status_string(int status);
 /* Text of the last CUDA error seen by this thread's most recent failing call ("" if none). */
 POISSON_API const char *poisson_last_error(void);

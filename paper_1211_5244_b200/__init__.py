@@ -15,6 +15,7 @@ __all__ = [
     "poisson_plan_describe", "poisson_plan_create", "poisson_set_kernel", "poisson_solve",
     "poisson_solve_host", "poisson_plan_destroy", "poisson_measure_fma_peak", "PoissonPlan", "EXPORTED_SYMBOLS",
     "poisson_set_kernel_even", "poisson_set_kernel_complex", "poisson_shard_describe", "ShardInfo", "ShardPlan", "ShardedSolver",
+    "poisson_solve_static", "STATIC_SCRATCH_BYTES",
 ]
 
 FREE, PERIODIC = 0, 1
@@ -26,6 +27,7 @@ EXPORTED_SYMBOLS = (
     "poisson_set_kernel", "poisson_set_kernel_complex", "poisson_solve", "poisson_solve_host", "poisson_debug_workspace",
     "poisson_debug_run_passes", "poisson_solve_profiled", "poisson_profile_read", "poisson_plan_launches_per_solve", "poisson_measure_fma_peak", "poisson_plan_workspace_bytes",
     "poisson_plan_destroy", "poisson_status_string", "poisson_last_error", "poisson_build_arch", "poisson_plan_launch_mode", "poisson_plan_graph_shape", "poisson_set_kernel_even", "poisson_shard_describe", "poisson_shard_plan_create", "poisson_shard_get_info", "poisson_shard_set_slabs", "poisson_shard_set_kernel", "poisson_shard_forward", "poisson_shard_middle", "poisson_shard_inverse", "poisson_solve_batch", "poisson_solve_batch_host", "poisson_plan_batch_lanes", "poisson_plan_batch_width",
+    "poisson_solve_static",
 )
 
 _PKG = Path(__file__).resolve().parent
@@ -118,6 +120,7 @@ def load_library():
     lib.poisson_shard_forward.argtypes = [vp, vp, vp]
     lib.poisson_shard_middle.argtypes = [vp, vp]
     lib.poisson_shard_inverse.argtypes = [vp, vp, vp]
+    lib.poisson_solve_static.argtypes = [i, i, i, i3, i, vp, vp, vp, vp]
     lib.poisson_plan_workspace_bytes.argtypes = [vp]
     lib.poisson_plan_workspace_bytes.restype = ctypes.c_size_t
     lib.poisson_plan_destroy.argtypes = [vp]
@@ -171,6 +174,20 @@ def poisson_solve(plan: int, rho_dev_ptr: int, V_dev_ptr: int, stream: int = 0) 
 
 def poisson_solve_host(plan: int, rho_host_ptr: int, V_host_ptr: int, stream: int = 0) -> None:
     _check(load_library().poisson_solve_host(plan, rho_host_ptr, V_host_ptr, stream), "poisson_solve_host")
+
+
+STATIC_SCRATCH_BYTES = 32 << 20   # POISSON_STATIC_SCRATCH_BYTES of include/poisson.h
+
+
+def poisson_solve_static(nx: int, ny: int, nz: int, bc, precision: int, K_f_dev_ptr: int, rho_dev_ptr: int, V_dev_ptr: int,
+                         stream: int = 0) -> None:
+    """A whole solve without a plan and without any device allocation, for callers that cannot cudaMalloc (all device
+    memory already in the application's own pool, a fixed memory budget, an inner loop that must not hit an allocation
+    failure or cudaMalloc's device-wide synchronisation).  Scratch is the library's fixed STATIC_SCRATCH_BYTES array, one
+    per GPU, shared by every call: grids that do not fit raise PoissonError (status 2), and calls whose GPU work could
+    overlap must be ordered by the caller.  Same kernels and bits as PoissonPlan.solve.  See include/poisson.h."""
+    _check(load_library().poisson_solve_static(nx, ny, nz, (ctypes.c_int * 3)(*bc), precision, K_f_dev_ptr, rho_dev_ptr,
+                                               V_dev_ptr, stream), "poisson_solve_static")
 
 
 def poisson_measure_fma_peak(precision: int = FP64) -> float:

@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1783,6 +1784,153 @@ int poisson_shard_inverse(poisson_plan *pl, void *V_local_dev, void *stream) {
     const int rc = shard_ready(pl);
     if (rc != POISSON_OK) return rc;
     return shard_launch(pl, POISSON_PASS_I1, nullptr, V_local_dev, reinterpret_cast<cudaStream_t>(stream));
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// poisson_solve_static: one whole solve that allocates NO device memory (include/poisson.h has the user-facing text).
+//
+// The five passes are the same kernels poisson_solve launches; what differs is where their scratch lives.  A plan keeps
+// the intermediates A1 / A2, the re-laid K^F copy and the twiddle tables in buffers it cudaMalloc'ed.  Here all of them
+// sit in ONE file-scope device array that is part of the library image, so a process that may not (or cannot) allocate
+// device memory -- its HBM is already handed out to its own pool, or an allocation failure / the implicit device
+// synchronisation of cudaMalloc / cudaFree is not acceptable where the call sits -- can still solve a small grid.
+// Price: every device that loads this library holds POISSON_STATIC_SCRATCH_BYTES until the process exits.
+//
+// Host code must not pass `pf_static_scratch` itself to a kernel: in host code that name is the host-side shadow of
+// the symbol, not a device address.  The device address is asked for once per device (static_device_state below) with
+// cudaGetSymbolAddress while that device is current, and only that pointer is handed to the kernels.
+static __device__ __align__(256) unsigned char pf_static_scratch[POISSON_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr size_t PF_STATIC_SLOT = (size_t)PF_GENERIC_MAX_S * 16;   // one table of the longest length, fp64 complex
+constexpr size_t PF_STATIC_TABLES = 9 * PF_STATIC_SLOT;            // per axis: twiddles, Bluestein chirp, Bluestein spectrum
+constexpr int PF_STATIC_MAX_DEV = 64;
+
+struct StaticDeviceState {
+    bool ready;               // cudaGetSymbolAddress done for this device
+    unsigned char *base;      // device address of pf_static_scratch ON THIS DEVICE
+    int num_sms;
+    int tab_S[3], tab_L[3], tab_prec[3];   // what the three table slots of this device's array hold right now (0 = nothing)
+    poisson_plan *pl;         // host-side description of the last grid solved here; owns NO device memory (never free_plan it)
+};
+StaticDeviceState g_static_dev[PF_STATIC_MAX_DEV];
+std::mutex g_static_mutex;
+
+inline size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+}  // namespace
+
+// First call on a device: checks the architecture and resolves the array's device address.  No allocation.
+static int static_device_state(StaticDeviceState **out) {
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); g_last_error = "no CUDA device"; return POISSON_EARCH; }
+    int dev = 0;
+    PF_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= PF_STATIC_MAX_DEV) { g_last_error = "device ordinal above 63"; return POISSON_EUNSUPPORTED; }
+    StaticDeviceState &sd = g_static_dev[dev];
+    if (!sd.ready) {
+        int major = 0, sms = 0;
+        PF_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        PF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        if (major != 10) { g_last_error = "device is not compute capability 10.x, kernels are sm_100a"; return POISSON_EARCH; }
+        void *ptr = nullptr;
+        const cudaError_t ce = cudaGetSymbolAddress(&ptr, pf_static_scratch);   // the address on the CURRENT device
+        if (ce != cudaSuccess || !ptr) return cuda_fail(ce, "cudaGetSymbolAddress(pf_static_scratch)");
+        sd.base = static_cast<unsigned char *>(ptr);
+        sd.num_sms = sms;
+        sd.ready = true;
+    }
+    *out = &sd;
+    return POISSON_OK;
+}
+
+int poisson_solve_static(int nx, int ny, int nz, const int bc[3], int precision, const void *K_f_dev, const void *rho_dev,
+                         void *V_dev, void *stream) {
+    if (!bc || !K_f_dev || !rho_dev || !V_dev) return POISSON_EINVAL;
+    if (reinterpret_cast<size_t>(K_f_dev) % 16 || reinterpret_cast<size_t>(rho_dev) % 16 || reinterpret_cast<size_t>(V_dev) % 16) return POISSON_EINVAL;
+    PlanDesc d;
+    int st = plan_build(nx, ny, nz, bc, precision, d);
+    if (st != POISSON_OK) return st;
+    cudaStream_t cs = reinterpret_cast<cudaStream_t>(stream);
+
+    std::lock_guard<std::mutex> guard(g_static_mutex);   // the host-side records below are shared by every caller
+    StaticDeviceState *sd = nullptr;
+    st = static_device_state(&sd);
+    if (st != POISSON_OK) return st;
+
+    // host-side description of the grid (kernels, tiles, grids): rebuilt only when the grid differs from the last call's
+    poisson_plan *pl = sd->pl;
+    const bool same = pl && pl->d.prec == precision && !std::memcmp(pl->d.n, d.n, sizeof(d.n)) && !std::memcmp(pl->d.bc, d.bc, sizeof(d.bc));
+    if (!same) {
+        delete pl;             // plain delete: its pointers are offsets into the static array, there is nothing to cudaFree
+        sd->pl = nullptr;
+        pl = new (std::nothrow) poisson_plan();
+        if (!pl) return POISSON_ENOMEM;
+        std::memset(static_cast<void *>(pl), 0, sizeof(*pl));
+        int dev = 0;
+        cudaGetDevice(&dev);
+        pl->d = d; pl->h = 1.0; pl->device = dev; pl->num_sms = sd->num_sms;
+        pl->elem_real = precision == POISSON_FP64 ? 8 : 4;
+        pl->late_tw = 1; pl->pdl_trigger = 1; pl->branches = 1; pl->xchains = 1; pl->env_lanes = -1; pl->env_wide = -1;
+        pl->pf_min_bytes = (size_t)96 << 20;
+        for (int q = 0; q < 5; ++q) pl->pf_force[q] = -1;
+        for (int q = 0; q < 5; ++q) {
+            st = setup_pass(pl, q, false);                 // same kernel choice as poisson_plan_create
+            if (st != POISSON_OK) { delete pl; return st; }
+        }
+        pl->chunk_planes = d.H; pl->n_chunks = 1; pl->a2_alloc_elems = d.a2_elems;
+        pl->kint_elems = kint_reals(pl);
+        // carve the array: [tables | A1 | A2 | K^F copy], 256-byte aligned pieces
+        const size_t cplx = 2 * pl->elem_real;
+        const size_t o_a1 = PF_STATIC_TABLES;
+        const size_t o_a2 = o_a1 + align256((size_t)d.a1_elems * cplx);
+        const size_t o_k = o_a2 + align256((size_t)d.a2_elems * cplx);
+        const size_t need = o_k + align256((size_t)pl->kint_elems * pl->elem_real);
+        if (need > (size_t)POISSON_STATIC_SCRATCH_BYTES) {
+            g_last_error = "poisson_solve_static: this grid needs " + std::to_string(need) + " bytes of scratch, the static array holds " +
+                           std::to_string((size_t)POISSON_STATIC_SCRATCH_BYTES) + " (use a plan: poisson_plan_create / poisson_solve)";
+            delete pl;
+            return POISSON_EUNSUPPORTED;
+        }
+        pl->a1 = sd->base + o_a1; pl->a2 = sd->base + o_a2; pl->kint = sd->base + o_k;
+        for (int q = 0; q < 3; ++q) {
+            pl->tw[q] = sd->base + (size_t)(3 * q) * PF_STATIC_SLOT;
+            pl->chirp[q] = sd->base + (size_t)(3 * q + 1) * PF_STATIC_SLOT;
+            pl->bspec[q] = sd->base + (size_t)(3 * q + 2) * PF_STATIC_SLOT;
+        }
+        pl->workspace_bytes = need;
+        pl->d.info.workspace_bytes = (long long)need;
+        sd->pl = pl;
+    }
+
+    // twiddle tables: the array keeps the last call's, so an axis is uploaded only when its length or precision changed.
+    // Stream-ordered on the caller's stream, in front of the passes that read them.
+    for (int q = 0; q < 3; ++q) {
+        int M = 0;
+        for (int ps = 0; ps < 5; ++ps) if (d.pass[ps].axis == q && pl->k[ps]->generic && pl->k[ps]->gen_blue) M = pl->k[ps]->gen_L;
+        const int L = M ? M : d.s[q];
+        if (sd->tab_S[q] == d.s[q] && sd->tab_L[q] == L && sd->tab_prec[q] == precision + 1) continue;
+        sd->tab_S[q] = 0;                                   // not valid while the upload may fail half way
+        std::vector<unsigned char> host;
+        fill_twiddles(host, L, precision);
+        PF_CUDA(cudaMemcpyAsync(pl->tw[q], host.data(), host.size(), cudaMemcpyHostToDevice, cs));
+        if (M) {
+            std::vector<unsigned char> hc, hb;
+            fill_bluestein(hc, hb, d.s[q], M, precision);
+            PF_CUDA(cudaMemcpyAsync(pl->chirp[q], hc.data(), hc.size(), cudaMemcpyHostToDevice, cs));
+            PF_CUDA(cudaMemcpyAsync(pl->bspec[q], hb.data(), hb.size(), cudaMemcpyHostToDevice, cs));
+        }
+        // pageable source: the runtime has staged the bytes when cudaMemcpyAsync returns, the vectors may go
+        sd->tab_S[q] = d.s[q]; sd->tab_L[q] = L; sd->tab_prec[q] = precision + 1;
+    }
+
+    // K^F of THIS call into the order pass F3 streams it in (nothing of an earlier call's copy is reused: the caller may
+    // have changed the kernel), then the five passes.  Every byte of A1 / A2 / the K^F copy that a pass reads was written
+    // earlier in this same call, so nothing in the array has to be cleared between calls.
+    st = relayout_kernel_spectrum(pl, K_f_dev, false, cs);
+    if (st != POISSON_OK) return st;
+    return run_passes(pl, rho_dev, V_dev, cs, 0, 4);
 }
 
 }  // extern "C"

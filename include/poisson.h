@@ -251,6 +251,17 @@ POISSON_API int poisson_plan_launches_per_solve(const poisson_plan *plan);
  * ALU bound of DESIGN.md, not a tensor-core figure.  Synchronous.  Errors: EINVAL, EARCH, ECUDA. */
 POISSON_API int poisson_measure_fma_peak(int precision, double *tflops /* host, out */);
 
+/* Environment variables.  All are read ONCE, inside poisson_plan_create (the solve path never calls getenv); none is
+ * needed for normal use -- the defaults are what the plan-time timing run picks.  For users:
+ *   POISSON_TUNE=0            skip the plan-time timing run (plan creation in microseconds instead of milliseconds; mode FIVE)
+ *   POISSON_PDL=0|1, POISSON_FUSED=0|1, POISSON_GRAPH=1          force a launch mode (poisson_plan_launch_mode)
+ *   POISSON_BRANCHES=J, POISSON_XCHAINS=R                         force the graph shape (poisson_plan_graph_shape)
+ *   POISSON_CHUNK=n | POISSON_CHUNK_MB=m                          plane-chunked middle passes (poisson_solve), smaller workspace
+ *   POISSON_LANES=1..8, POISSON_WIDE=0|n                          batch routes (poisson_solve_batch)
+ * For the library's own experiments and tests (no stability promise; results stay correct with any value):
+ *   POISSON_VARIANT, POISSON_GRID, POISSON_PREFETCH (one value, or one per pass "f1,f2,f3,i2,i1"), POISSON_LATE_TW,
+ *   POISSON_PDL_TRIGGER, POISSON_FUSED_SKEW, POISSON_LANE_GRAPH=0, and POISSON_TEST_MAX_LANES=n, which makes the allocation
+ *   of a batch lane beyond the n-th fail as if device memory had run out (tests of the fall-back to fewer lanes). */
 POISSON_API size_t poisson_plan_workspace_bytes(const poisson_plan *plan);
 POISSON_API int poisson_plan_destroy(poisson_plan *plan);
 
@@ -275,7 +286,9 @@ POISSON_API int poisson_plan_destroy(poisson_plan *plan);
  * overwrites the slabs pass I1 reads only after the next barrier A, which every rank enqueues after its own I1.
  * Partition: rank s of R owns [floor(T s / R), floor(T (s + 1) / R)) of T = N_o points resp. T = H planes.
  * Supported: grids whose five passes all run the compiled register-engine kernels, even N_x, R <= min(N_o, H, 32);
- * else POISSON_EUNSUPPORTED.  Results are bitwise those of poisson_solve (same kernels, same arithmetic per pencil). */
+ * else POISSON_EUNSUPPORTED.  Results are bitwise those of poisson_solve (same kernels, same arithmetic per pencil), with one
+ * exception: shard plans always take a length's default factorisation, while poisson_solve runs passes F2 / I2 of length 192 in
+ * fp64 in a second, faster one (12 x 16) -- on grids with S_b = 192 the two agree to rounding (1e-15), not bit for bit. */
 typedef struct poisson_shard_info {
     int rank, nranks;
     int split_axis;         /* o: rho / V are distributed along this axis (1 = y, 2 = z)                          */
@@ -299,7 +312,8 @@ POISSON_API int poisson_shard_plan_create(poisson_plan **out, int nx, int ny, in
                                           int rank, int nranks);
 POISSON_API int poisson_shard_get_info(const poisson_plan *plan, poisson_shard_info *info /* host, out */);
 /* mid_of_rank[s] / back_of_rank[s]: device pointers, valid on THIS device, to rank s's exchange slabs (host arrays of
- * nranks pointers; entry [rank] is the rank's own slab).  16-byte aligned.  The plan keeps the pointers, not the memory. */
+ * nranks pointers; entry [rank] is the rank's own slab).  32-byte aligned (passes F1 / I2 store 256-bit pairs into them), else
+ * EINVAL; EINVAL also when the current device is not the plan's.  The plan keeps the pointers, not the memory. */
 POISSON_API int poisson_shard_set_slabs(poisson_plan *plan, void *const *mid_of_rank /* host */, void *const *back_of_rank /* host */);
 /* K_f_dev: the WHOLE spectrum [S_z][S_y][S_x/2+1] as for poisson_set_kernel; only the rank's planes are kept. */
 POISSON_API int poisson_shard_set_kernel(poisson_plan *plan, const void *K_f_dev, void *stream);

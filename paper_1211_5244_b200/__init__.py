@@ -441,7 +441,12 @@ class ShardedSolver:
     """One solve over the GPUs of a torch.distributed process group (one process per GPU, NCCL): this rank's ShardPlan, its two
     exchange slabs in symmetric memory (every peer's slab mapped into this process over NVLink), and the two barriers as
     one-element all-reduces on the compute stream.  torch supplies memory, peer mapping and the barrier; every step of the
-    path runs in the library's kernels, which store straight into the peers' slabs."""
+    path runs in the library's kernels, which store straight into the peers' slabs.
+
+    EXPERIMENTAL for world > 1: that branch (symmetric-memory allocation, rendezvous, all-reduce as the barrier) has never
+    run on hardware -- no box with two GPUs was available to this build; only world == 1 and the library's own sharded
+    passes (virtual ranks on one GPU, tests/test_gpu_shard.py) are verified.  Every process must have made ITS GPU current
+    (torch.cuda.set_device(local_rank)) before constructing this object: the plan binds to the current device."""
 
     def __init__(self, n, bc, h: float, precision: int = FP64, group=None):
         import torch
@@ -449,6 +454,12 @@ class ShardedSolver:
         self.group = group
         self.rank = dist.get_rank(group) if dist.is_initialized() else 0
         self.world = dist.get_world_size(group) if dist.is_initialized() else 1
+        if self.world > 1:
+            import os
+            local = os.environ.get("LOCAL_RANK")
+            if local is not None and torch.cuda.device_count() > 1 and torch.cuda.current_device() != int(local):
+                raise RuntimeError(f"ShardedSolver: current CUDA device {torch.cuda.current_device()} is not LOCAL_RANK {local}: "
+                                   "call torch.cuda.set_device(local_rank) first (the plan and its slabs bind to the current device)")
         self.plan = ShardPlan(n, bc, h, precision, self.rank, self.world)
         info = self.plan.info
         if self.world == 1:

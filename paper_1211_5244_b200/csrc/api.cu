@@ -256,6 +256,7 @@ struct poisson_plan {
     int xchains;               // graph mode: F1 / F2 / I2 / I1 split over this many ranges of x (POISSON_XCHAINS)
     int branches;              // graph mode: the middle passes as this many parallel chains over ranges of k_a planes (POISSON_BRANCHES)
     int env_lanes, env_wide;   // POISSON_LANES / POISSON_WIDE as read at plan creation (-1: not set)
+    int test_max_lanes;        // POISSON_TEST_MAX_LANES=n (tests only): allocating a batch lane beyond the n-th fails as if device memory had run out
     bool env_lane_graph;       // POISSON_LANE_GRAPH=0 at plan creation: plain launches on the batch lanes (experiments)
     void *wide_a1, *wide_a2;   // intermediates of wide_w densities (several small solves per launch), allocated on first use
     int wide_w;
@@ -264,6 +265,7 @@ struct poisson_plan {
     void *chirp[3], *bspec[3];   // Bluestein axes only (generic_pass.cuh: gen_transform)
     void *rho_stage, *v_stage;
     const FusedEntry *fused;   // one-launch solve kernel compiled for this combination of axes, or NULL
+    const FusedEntry *fused_saved; bool use_fused_saved;   // what poisson_set_kernel_even set aside (the one-launch kernel reads the full K^F layout); poisson_set_kernel puts it back
     bool use_fused;            // launch mode picked for poisson_solve: fused kernel, else 5 launches (with or without PDL)
     bool use_graph;            // ... or the five launches as one CUDA graph launch (use_pdl: with programmatic edges)
     GraphSolve gs, gs_pdl;
@@ -537,6 +539,7 @@ int poisson_plan_create(poisson_plan **out, int nx, int ny, int nz, const int bc
     { const char *env = std::getenv("POISSON_LANES"); pl->env_lanes = env ? std::atoi(env) : -1; }
     { const char *env = std::getenv("POISSON_WIDE"); pl->env_wide = env ? std::atoi(env) : -1; }
     { const char *env = std::getenv("POISSON_LANE_GRAPH"); pl->env_lane_graph = !(env && env[0] == '0'); }
+    { const char *env = std::getenv("POISSON_TEST_MAX_LANES"); pl->test_max_lanes = env ? std::atoi(env) : 0; }
     pl->pf_min_bytes = (size_t)96 << 20;
 
     for (int q = 0; q < 5; ++q) {
@@ -771,7 +774,13 @@ static int switch_kernel_fold(poisson_plan *pl, bool even) {
     pl->kernel_set = false;
     destroy_graph(pl->gs); destroy_graph(pl->gs_pdl);
     if (pl->lanes) for (Lane &ln : *pl->lanes) if (ln.gs) destroy_graph(*ln.gs);
-    if (even) { pl->fused = nullptr; pl->use_fused = false; }   // the one-launch kernel addresses the full layout
+    if (even) {   // the one-launch kernel addresses the full layout: set it (and the tuned choice) aside while the copy is folded
+        pl->fused_saved = pl->fused; pl->use_fused_saved = pl->use_fused;
+        pl->fused = nullptr; pl->use_fused = false;
+    } else if (pl->fused_saved) {
+        pl->fused = pl->fused_saved; pl->use_fused = pl->use_fused_saved;
+        pl->fused_saved = nullptr;
+    }
     if (pl->use_graph) { if ((pl->use_pdl ? build_graph_pdl(pl, pl->gs_pdl, nullptr) : build_graph(pl, pl->gs, nullptr)) != POISSON_OK) cudaGetLastError(); }
     return POISSON_OK;
 }
@@ -818,7 +827,7 @@ int poisson_set_kernel_complex(poisson_plan *pl, const void *K_f_dev, void *stre
         PF_CUDA(cudaDeviceSynchronize());   // no solve of this plan may still be using the buffers replaced below
         destroy_graph(pl->gs); destroy_graph(pl->gs_pdl);
         if (pl->lanes) for (Lane &ln : *pl->lanes) if (ln.gs) destroy_graph(*ln.gs);
-        pl->fused = nullptr; pl->use_fused = false;
+        pl->fused = nullptr; pl->use_fused = false; pl->fused_saved = nullptr;   // for good: pass F3 leaves the register engine
         if (!pl->k[2]->generic) { const int rc = setup_pass(pl, 2, true); if (rc != POISSON_OK) return rc; }
         pl->kcplx = true;
         const long long need = kint_reals(pl);
@@ -1421,14 +1430,17 @@ static int ensure_lanes(poisson_plan *pl, int want, bool staging) {
         ln.owns_ws = !first;
         cudaError_t ce = cudaSuccess;
         if (first) { ln.a1 = pl->a1; ln.a2 = pl->a2; }
-        else {
+        else if (pl->test_max_lanes > 0 && (int)pl->lanes->size() >= pl->test_max_lanes) {
+            ce = cudaErrorMemoryAllocation;   // injected (tests): exercises the fall-back to the lanes that fit
+        } else {
             ce = cudaMalloc(&ln.a1, (size_t)pl->d.a1_elems * cplx);
             if (ce == cudaSuccess) ce = cudaMalloc(&ln.a2, (size_t)pl->a2_alloc_elems * cplx);
+            if (ce != cudaSuccess) { cudaFree(ln.a1); ln.a1 = nullptr; ln.a2 = nullptr; ln.owns_ws = false; }
         }
         if (ce == cudaSuccess) ce = cudaStreamCreateWithFlags(&ln.st, cudaStreamNonBlocking);
         if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&ln.done, cudaEventDisableTiming);
         if (ce != cudaSuccess) {
-            if (ln.owns_ws) { cudaFree(ln.a1); cudaFree(ln.a2); }
+            if (ln.owns_ws && ln.a1) { cudaFree(ln.a1); cudaFree(ln.a2); }
             if (ln.st) cudaStreamDestroy(ln.st);
             if (ln.done) cudaEventDestroy(ln.done);
             cudaGetLastError();
@@ -1528,6 +1540,8 @@ static int solve_batch_impl(poisson_plan *pl, const void *const *rho, void *cons
                 ln.gs = new (std::nothrow) GraphSolve();
                 if (!ln.gs) return POISSON_ENOMEM;
                 std::memset(ln.gs, 0, sizeof(GraphSolve));
+            }
+            if (!ln.gs->exec) {   // first use, or a kernel switch (set_kernel_even / _complex / back) dropped the lane's graph
                 rc1 = pl->use_pdl ? build_graph_pdl(pl, *ln.gs, &ln) : build_graph(pl, *ln.gs, &ln);
                 if (rc1 != POISSON_OK) return rc1;
             }
@@ -1690,6 +1704,7 @@ int poisson_shard_get_info(const poisson_plan *pl, poisson_shard_info *info) {
 
 int poisson_shard_set_slabs(poisson_plan *pl, void *const *mid_of_rank, void *const *back_of_rank) {
     if (!pl || !pl->shard || !mid_of_rank || !back_of_rank) return POISSON_EINVAL;
+    if (check_device(pl, true) != POISSON_OK) return POISSON_EINVAL;   // the pointers must be valid on the plan's device
     for (int s = 0; s < pl->shard->R; ++s) {
         if (!mid_of_rank[s] || !back_of_rank[s]) return POISSON_EINVAL;
         if (reinterpret_cast<size_t>(mid_of_rank[s]) % 32 || reinterpret_cast<size_t>(back_of_rank[s]) % 32) return POISSON_EINVAL;   // 256-bit pair stores

@@ -151,3 +151,73 @@ def test_config1_batch_in_the_bench_configuration(pk):
         assert rel_l2(Vs[3].cpu().numpy(), exp) <= 1e-12
     finally:
         plan.close()
+
+
+def test_lane_graphs_survive_a_kernel_switch(pk, monkeypatch):
+    """Lane path in graph mode: solve_batch -> set_kernel_even -> solve_batch -> set_kernel_complex -> solve_batch ->
+    set_kernel -> solve_batch.  Every kernel switch drops the lanes' instantiated graphs; the next batch must rebuild them
+    (it used to launch a NULL graph exec and return ECUDA) and solve with the NEW kernel."""
+    import torch
+    monkeypatch.setenv("POISSON_WIDE", "0")      # small grid, but the lane route (as grids above 16 MB per lane take)
+    monkeypatch.setenv("POISSON_GRAPH", "1")
+    n, bc = (48, 32, 32), (0, 0, 0)
+    rng = np.random.default_rng(99)
+    s = gen.padded_shape(n, bc)
+    Kf1 = oracle.kernel_spectrum(_even_kernel(rng, s))
+    Kf2 = oracle.kernel_spectrum(_even_kernel(rng, s))
+    rhos_np = [rng.standard_normal((n[2], n[1], n[0])) for _ in range(5)]
+    plan = pk.PoissonPlan(n, bc, 0.25, pk.FP64)
+    try:
+        assert plan.batch_width(5) == 0 and plan.batch_lanes(5) >= 2
+        rhos = [torch.from_numpy(r).cuda() for r in rhos_np]
+
+        def check(Kf):
+            Vs = plan.solve_batch(rhos)
+            torch.cuda.synchronize()
+            for i in (0, 4):
+                assert rel_l2(Vs[i].cpu().numpy(), oracle.solve(rhos_np[i], Kf, bc)) <= 1e-12
+
+        plan.set_kernel(torch.from_numpy(Kf1).cuda());        check(Kf1)
+        plan.set_kernel_even(torch.from_numpy(Kf2).cuda());   check(Kf2)
+        plan.set_kernel_complex(torch.from_numpy(Kf1.astype(np.complex128)).cuda()); check(Kf1)
+        plan.set_kernel(torch.from_numpy(Kf2).cuda());        check(Kf2)
+    finally:
+        plan.close()
+
+
+@pytest.mark.parametrize("max_lanes,host", [(1, False), (2, True)], ids=["device_1_of_2", "host_2_of_3"])
+def test_batch_falls_back_to_the_lanes_that_fit(pk, monkeypatch, max_lanes, host):
+    """ensure_lanes running out of device memory (injected: POISSON_TEST_MAX_LANES) must not fail the batch: it runs on the
+    lanes that could be allocated, the caller's stream stays ordered after them, and the results are those of single solves."""
+    import torch
+    monkeypatch.setenv("POISSON_WIDE", "0")
+    monkeypatch.setenv("POISSON_TEST_MAX_LANES", str(max_lanes))
+    n, bc = (32, 24, 40), (0, 0, 0)
+    rng = np.random.default_rng(17)
+    Kf = oracle.kernel_spectrum(_even_kernel(rng, gen.padded_shape(n, bc)))
+    rhos_np = [rng.standard_normal((n[2], n[1], n[0])) for _ in range(7)]
+    plan = pk.PoissonPlan(n, bc, 0.25, pk.FP64)
+    try:
+        plan.set_kernel(torch.from_numpy(Kf).cuda())
+        assert plan.batch_lanes(7, host=host) > max_lanes          # more lanes wanted than the injected limit allows
+        rhos = [torch.from_numpy(r).cuda() for r in rhos_np]
+        singles = [plan.solve(r).clone() for r in rhos]
+        torch.cuda.synchronize()
+        if host:
+            hin = [torch.from_numpy(r).pin_memory() for r in rhos_np]
+            hout = [torch.empty_like(r).pin_memory() for r in hin]
+            for rep in range(2):
+                plan.solve_batch_host(hin, hout)
+                for i in range(7):
+                    assert torch.equal(hout[i], singles[i].cpu())
+        else:
+            for rep in range(2):
+                Vs = plan.solve_batch(rhos)
+                after = Vs[6] + 0            # queued on the caller's stream: must see the finished batch
+                torch.cuda.synchronize()
+                assert torch.equal(after, singles[6])
+                for i in range(7):
+                    assert torch.equal(Vs[i], singles[i])
+        assert rel_l2(singles[3].cpu().numpy(), oracle.solve(rhos_np[3], Kf, bc)) <= 1e-12
+    finally:
+        plan.close()

@@ -405,3 +405,29 @@ def test_even_kernel_folded_storage(pk, monkeypatch, prec):
         assert not torch.equal(plan.solve(rho), a)
     finally:
         plan.close()
+
+
+def test_fused_mode_comes_back_after_an_even_kernel(pk, monkeypatch):
+    """poisson_set_kernel_even drops the one-launch FUSED mode (that kernel reads the full K^F layout); poisson_set_kernel
+    afterwards must put the plan back into the mode it was created in, as include/poisson.h says ("switches back")."""
+    import torch
+    monkeypatch.setenv("POISSON_FUSED", "1")
+    n, bc = (32, 32, 32), (0, 0, 0)
+    rng = np.random.default_rng(31)
+    Kf = torch.from_numpy(oracle.kernel_spectrum(_even_kernel(rng, gen.padded_shape(n, bc)))).cuda()
+    rho = torch.from_numpy(rng.standard_normal((n[2], n[1], n[0]))).cuda()
+    plan = pk.PoissonPlan(n, bc, 0.3, pk.FP64)
+    try:
+        assert plan.launch_mode()[0] == "fused"
+        plan.set_kernel(Kf)
+        ref = plan.solve(rho).clone()
+        plan.set_kernel_even(Kf)
+        assert plan.launch_mode()[0] != "fused"
+        V_even = plan.solve(rho).clone()
+        plan.set_kernel(Kf)
+        assert plan.launch_mode()[0] == "fused"
+        assert torch.equal(plan.solve(rho), ref)
+        torch.cuda.synchronize()
+        assert rel_l2(V_even.cpu().numpy(), ref.cpu().numpy()) <= 1e-12   # Kf is even to rounding only: not bitwise here
+    finally:
+        plan.close()

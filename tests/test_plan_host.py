@@ -159,3 +159,26 @@ def test_half_spectrum_length_and_rows_for_odd_sizes():
     assert list(info.s) == [7, 9, 10] and list(info.order) == [1, 0, 2] and info.half_len == 9 // 2 + 1
     assert list(info.rows) == [7 * 5, 5 * 5, 5 * 7, 5 * 5, 7 * 5]
     assert list(info.length) == [9, 7, 10, 7, 9]
+
+
+def test_reference_arm_of_the_bench_never_loads_the_product_library(lib):
+    """`bench.py --impl reference` times the oracle only: its `config` keys come from workloads/ and a restated axis-order
+    rule (equal to the planner's for all 8 BCs), and the process must not import the package or map libpoisson_b200.so."""
+    import itertools
+    import json
+    import subprocess
+    import sys
+    sys.path.insert(0, str(ROOT))
+    import bench
+    for bc in itertools.product((0, 1), repeat=3):
+        assert bench.reference_axis_order(bc) == list(pk.poisson_plan_describe(16, 16, 16, bc, pk.FP64).order)
+    code = ("import sys, json, argparse, bench\n"
+            "bench.run_reference(argparse.Namespace(config='c0', steps=1, warmup=0, gpus=1))\n"
+            "assert 'paper_1211_5244_b200' not in sys.modules\n"
+            "assert 'libpoisson_b200' not in open('/proc/self/maps').read()\n")
+    r = subprocess.run([sys.executable, "-c", code], cwd=ROOT, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    info = pk.poisson_plan_describe(32, 32, 32, (0, 0, 0), pk.FP64)
+    assert line["impl"] == "reference" and line["config"]["padded_grid"] == list(info.s)
+    assert line["config"]["axis_order"] == list(info.order)

@@ -282,6 +282,15 @@ def config_dict(key, cfg, info_s, order, world):
             "replicas": world}
 
 
+def reference_axis_order(bc):
+    """The planner's axis-order rule restated (tests/test_plan_host.py checks it against poisson_plan_describe)."""
+    per = [b != 0 for b in bc]
+    a = 2 if per[2] else (1 if per[1] else 2)
+    o = 1 if a == 2 else 2
+    b, c = ((0, o) if per[0] else (o, 0)) if per[0] != per[o] else (o, 0)
+    return [a, b, c]
+
+
 def run_reference(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -291,12 +300,11 @@ def run_reference(args):
     steps, warmup = max(1, args.steps), max(0, args.warmup)
     sec, desc, threads, extrap, frac, ntimed = oracle_steps(cfg, rho, kf, steps, warmup, 170.0)
     val = 1.0 / sec
-    try:   # the planner is host-only: same padded grid / axis order keys as the main arm
-        import paper_1211_5244_b200 as pk
-        info = pk.poisson_plan_describe(cfg.n[0], cfg.n[1], cfg.n[2], cfg.bc, pk.FP64)
-        s_pad, order = list(info.s), list(info.order)
-    except Exception:
-        s_pad, order = list(cfg.s), []
+    # Same `config` keys as the main arm WITHOUT loading the product library (this arm must map oracle/ only): the padded
+    # grid is S_i = N_i B_i, and the axis order is the planner's documented rule (include/poisson.h: periodic axes first,
+    # free axes last, never x first, the contiguous axis last on a tie) restated here.
+    s_pad = list(gen.padded_shape(cfg.n, cfg.bc))
+    order = reference_axis_order(cfg.bc)
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
         "warmup": warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -313,11 +321,43 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------ GPU timing
+def time_periodic_same_fft_size(pk, torch, cfg, steps, warmup):
+    """A fully periodic fp64 solve on the PADDED shape of `cfg` (the same FFT size, nothing skipped): the denominator of the
+    paper's Fig. 1 ratios.  Timing does not depend on the values: random density, K^F = 1."""
+    s = gen.padded_shape(cfg.n, cfg.bc)
+    plan = pk.PoissonPlan(s, (pk.PERIODIC,) * 3, cfg.h, pk.FP64)
+    try:
+        plan.set_kernel(torch.ones(plan.kernel_dims, dtype=torch.float64, device="cuda"))
+        nbuf = max(2, int(math.ceil(300e6 / (8.0 * s[0] * s[1] * s[2]))))      # rho / V ring larger than the 126 MB L2
+        rhos = [torch.randn((s[2], s[1], s[0]), dtype=torch.float64, device="cuda") for _ in range(nbuf)]
+        Vs = [torch.empty_like(r) for r in rhos]
+        for i in range(warmup):
+            plan.solve(rhos[i % nbuf], Vs[i % nbuf])
+        torch.cuda.synchronize()
+        best = []
+        for rep in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for i in range(steps):
+                plan.solve(rhos[i % nbuf], Vs[i % nbuf])
+            e1.record()
+            torch.cuda.synchronize()
+            best.append(e0.elapsed_time(e1) / steps)
+        best.sort()
+        return {"ms": best[len(best) // 2], "padded_grid": list(s), "bytes_total": plan.info.bytes_total}
+    finally:
+        plan.close()
+
+
 def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, with_profile=True, inputs=None, even_kernel=False):
     cfg, rho_np, kf_np = inputs if inputs is not None else build_inputs(key)
     prec = pk.FP64 if cfg.precision == "fp64" else pk.FP32
     np_dt = np.float64 if prec == pk.FP64 else np.float32
-    plan = pk.PoissonPlan(cfg.n, cfg.bc, cfg.h, prec)
+    torch.cuda.synchronize()
+    t_create = time.perf_counter()
+    plan = pk.PoissonPlan(cfg.n, cfg.bc, cfg.h, prec)       # allocates, uploads tables, and TIMES the launch modes / graph shapes
+    torch.cuda.synchronize()
+    plan_create_ms = (time.perf_counter() - t_create) * 1e3
     info = plan.info
     # even_kernel: the folded K^F copy (poisson_set_kernel_even; every BASELINE kernel is even along each axis)
     (plan.set_kernel_even if even_kernel else plan.set_kernel)(torch.from_numpy(np.ascontiguousarray(kf_np.astype(np_dt))).cuda())
@@ -381,6 +421,7 @@ def time_config(pk, torch, key, steps, warmup, with_e2e=True, with_cold=True, wi
            "info": info, "nbuf": nbuf, "rho_bytes": rho_bytes,
            "launch_mode": mode, "tune_ms": tune_ms, "graph_shape": list(plan.graph_shape()), "lanes": plan.batch_lanes(bsz),
            "width": plan.batch_width(bsz), "launches_per_solve": plan.launches_per_solve(), "workspace_bytes": plan.workspace_bytes()}
+    res["plan_create_ms"] = plan_create_ms
     if pass_ms is not None:
         res["pass_ms"] = pass_ms
 
@@ -479,6 +520,18 @@ def run_ours(args):
                     traffic_src = f"ncu --set full (L2 flushed before the launch: cold-L2 DRAM bytes), capture {row['source']}"
         except Exception:
             traffic = None
+    # executed FP64-pipe instructions of the dominant kernel (north_star: "evidenced by ncu counters"), from the tracked launch list
+    inst_fp64, inst_all, inst_src = None, None, None
+    ifile = ROOT / "profiles" / "inst_fp64.csv"
+    if ifile.exists():
+        try:
+            import csv
+            for row in csv.DictReader(ifile.open()):
+                if row["config"] == args.config and row["pass"] == dom_name:
+                    inst_fp64, inst_all = int(row["sm__inst_executed_pipe_fp64.sum"]), int(row["smsp__inst_executed.sum"])
+                    inst_src = f"ncu --metrics sm__inst_executed_pipe_fp64.sum,smsp__inst_executed.sum per launch (warp-level counts), {row['source']}"
+        except Exception:
+            inst_fp64 = None
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -507,6 +560,9 @@ def run_ours(args):
                             f"densities per launch={res['width']} (SURVEY.md 8f-1; pointer arrays marshalled before the timed region)")},
         "pass_us": {pk.PASS_NAMES[q]: res["pass_ms"][q] * 1e3 for q in range(5)},
         "pass_gbs": {pk.PASS_NAMES[q]: info.bytes[q] / (res["pass_ms"][q] * 1e-3) / 1e9 for q in range(5)},
+        "pass_hbm_frac": {pk.PASS_NAMES[q]: info.bytes[q] / (res["pass_ms"][q] * 1e-3) / 1e9 / peak for q in range(5)},
+        "plan_create_ms": res["plan_create_ms"],
+        "plan_create_note": "wall clock of poisson_plan_create: allocation, tables and the launch-mode / graph-shape timing runs (POISSON_TUNE=0 skips those)",
         "pass_us_note": ("poisson_solve_profiled: the five passes as five STREAM launches with a CUDA event between each (launch gaps "
                          "included), not the launch mode poisson_solve uses; their sum exceeds ms_per_step"),
         "cold_l2": {"ms_per_step": res["cold_ms_per_step"],
@@ -514,6 +570,8 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "kernel": dom_kernel,
                      "achieved": dom_gbs, "peak": peak, "unit": "GB/s", "frac": dom_gbs / peak, "traffic": traffic,
                      "traffic_source": traffic_src,
+                     "inst_fp64": inst_fp64, "inst_executed": inst_all, "inst_source": inst_src,
+                     "fp64_thread_inst_per_s": (inst_fp64 * 32 / (dom_us * 1e-6)) if inst_fp64 else None,
                      "dram_frac": (traffic / (dom_us * 1e-6) / 1e9 / peak) if traffic else None,
                      "algorithmic_bytes_per_launch": dom_bytes, "peak_source": peak_src,
                      "duration_us": dom_us, "duration_source": "CUDA events around the kernel's stream launch (pass_us)"},
@@ -537,11 +595,14 @@ def run_ours(args):
         line["config"]["kernel_storage"] = "folded: poisson_set_kernel_even (K^F kept for k_b <= S_b/2 only)"
     elif world == 1:
         # SURVEY.md 8f-2 (less K^F traffic): the same solves with the folded K^F copy, timed the same way
-        ev = time_config(pk, torch, args.config, steps, warmup, with_e2e=False, with_cold=False, with_profile=False, inputs=inputs,
-                         even_kernel=True)
-        line["even_kernel"] = {"ms_per_step": ev["single"]["ms"], "solves_per_sec": 1e3 / ev["single"]["ms"],
-                               "workspace_bytes": ev["workspace_bytes"], "workspace_bytes_full_kernel": res["workspace_bytes"],
-                               "api": "poisson_set_kernel_even + poisson_solve: K^F stored for k_b <= S_b/2 only (kernels even along every axis)"}
+        try:
+            ev = time_config(pk, torch, args.config, steps, warmup, with_e2e=False, with_cold=False, with_profile=False, inputs=inputs,
+                             even_kernel=True)
+            line["even_kernel"] = {"ms_per_step": ev["single"]["ms"], "solves_per_sec": 1e3 / ev["single"]["ms"],
+                                   "workspace_bytes": ev["workspace_bytes"], "workspace_bytes_full_kernel": res["workspace_bytes"],
+                                   "api": "poisson_set_kernel_even + poisson_solve: K^F stored for k_b <= S_b/2 only (kernels even along every axis)"}
+        except pk.PoissonError as e:   # e.g. EUNSUPPORTED: pass F3 of this grid runs the any-length kernel
+            line["even_kernel"] = {"unavailable": str(e), "status": e.status}
     if world == 1 and not args.no_cpu_baseline:
         sec, desc, threads, extrap, frac, ntimed = oracle_steps(cfg, inputs[1], inputs[2], 3, 0, 30.0)
         line["cpu_baseline"] = {"value": 1.0 / sec, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
@@ -566,11 +627,33 @@ def run_ours(args):
                            "batched_ms_per_step": r["batch"]["ms"],
                            "batched_hbm_frac": i2.bytes_total / (r["batch"]["ms"] * 1e-3) / 1e9 / peak,
                            "e2e_ms_per_step": r["e2e_ms_per_step"], "launch_mode": r["launch_mode"], "graph_shape": r["graph_shape"],
-                           "pass_us": {pk.PASS_NAMES[q]: r["pass_ms"][q] * 1e3 for q in range(5)}}
+                           "pass_us": {pk.PASS_NAMES[q]: r["pass_ms"][q] * 1e3 for q in range(5)},
+                           # each pass's algorithmic bytes over its event-bracketed stream launch, as a fraction of the HBM peak
+                           "pass_hbm_frac": {pk.PASS_NAMES[q]: (i2.bytes[q] / (r["pass_ms"][q] * 1e-3) / 1e9 / peak) if r["pass_ms"][q] > 0 else None
+                                             for q in range(5)},
+                           "plan_create_ms": r.get("plan_create_ms")}
         line["other_configs"] = others
-        if "c4a" in others and "c4p" in others:
-            # zero-skipping gain at equal FFT size would need periodic 512^3; report the paper-style pair we have
-            line["zero_skipping"] = {"free_256_phys_ms": others["c4a"]["ms_per_step"], "periodic_256_ms": others["c4p"]["ms_per_step"]}
+        # The paper's Fig. 1 comparison: a free / wire / surface solve against the FULLY PERIODIC solve of the
+        # SAME FFT size (free and wire: 58 %, surface: 66 % of the periodic time there).  Equal-size pairs: c1 (128^3 -> 256^3)
+        # against c4p (periodic 256^3); c2 / c3 against periodic runs of their padded shapes.
+        zs = {"paper_ratio": {"free": 0.58, "wire": 0.58, "surface": 0.66}, "cite": "PAPER.md:79", "pairs": {}}
+        ms_of = {args.config: ms}
+        ms_of.update({k: v["ms_per_step"] for k, v in others.items()})
+        bytes_of = {args.config: info.bytes_total}
+        bytes_of.update({k: pk.poisson_plan_describe(*gen.get_config(k).n, gen.get_config(k).bc, pk.FP64).bytes_total for k in others})
+        if "c1" in ms_of and "c4p" in ms_of:
+            zs["pairs"]["free_256"] = {"padded_grid": [256, 256, 256], "ms": ms_of["c1"], "periodic_ms": ms_of["c4p"],
+                                       "ratio_time": ms_of["c1"] / ms_of["c4p"], "ratio_bytes_model": bytes_of["c1"] / bytes_of["c4p"]}
+        for key, kind in (("c2", "surface"), ("c3", "wire")):
+            if key not in ms_of:
+                continue
+            try:
+                pr = time_periodic_same_fft_size(pk, torch, gen.get_config(key), min(steps, 200), 5)
+                zs["pairs"][f"{kind}_{key}"] = {"padded_grid": pr["padded_grid"], "ms": ms_of[key], "periodic_ms": pr["ms"],
+                                                "ratio_time": ms_of[key] / pr["ms"], "ratio_bytes_model": bytes_of[key] / pr["bytes_total"]}
+            except pk.PoissonError as e:
+                zs["pairs"][f"{kind}_{key}"] = {"unavailable": str(e)}
+        line["zero_skipping"] = zs
     print(json.dumps(line))
     return 0
 
